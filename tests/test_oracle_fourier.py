@@ -1,0 +1,122 @@
+"""Pins for oracle/fourier.py against what PAPER.md Section 5.3 and the mathematics fix."""
+import numpy as np
+import pytest
+from numpy.polynomial import legendre as npleg
+
+from oracle import basis, fourier
+
+
+def _lagrange_values(xi, x):
+    n = len(xi)
+    L = np.ones((n, len(x)))
+    for j in range(n):
+        for k in range(n):
+            if k != j:
+                L[j] *= (x - xi[k]) / (xi[j] - xi[k])
+    return L
+
+
+@pytest.mark.parametrize("n,N,pmax,lo,hi", [(4, 16, 16, 0.0, 4 * np.pi), (8, 8, 24, 0.0, 20 * np.pi),
+                                            (6, 5, 12, -1.0, 2.5), (10, 4, 10, 0.0, 1.0)])
+def test_transform_tensor_brute_force(n, N, pmax, lo, hi):
+    """Eq. 63 against c_p = (1/L) int f e^{-ikx} dx (Eq. 60) with f = l_j on element m, the
+    integral done by 80-point Gauss-Legendre quadrature."""
+    T = fourier.transform_tensor(lo, hi, N, n, pmax).reshape(pmax + 1, N, n)
+    xi, _ = basis.lgl_nodes_weights(n)
+    xg, wg = npleg.leggauss(80)
+    Lg = _lagrange_values(xi, xg)
+    L = hi - lo
+    dx = L / N
+    for p in range(pmax + 1):
+        kp = 2 * np.pi * p / L
+        for m in (0, N // 2, N - 1):
+            xbar = lo + (m + 0.5) * dx
+            integ = (Lg * (wg * np.exp(-1j * kp * (xbar + 0.5 * dx * xg)))[None, :]).sum(axis=1) * (0.5 * dx / L)
+            assert np.allclose(T[p, m], integ, atol=5e-16, rtol=1e-13), (p, m)
+
+
+def test_spherical_bessel_identity_eq62():
+    """Eq. 62: int P_s(xi) e^{-i z xi} dxi = 2 (-i)^s j_s(z), by quadrature."""
+    from scipy.special import spherical_jn
+    xg, wg = npleg.leggauss(60)
+    for z in (0.0, 1e-3, 0.7, 3.0, 12.5):
+        for s in range(10):
+            c = np.zeros(s + 1); c[s] = 1
+            lhs = np.sum(wg * npleg.legval(xg, c) * np.exp(-1j * z * xg))
+            assert abs(lhs - 2 * (-1j) ** s * spherical_jn(s, z)) < 5e-14
+
+
+def test_mean_mode_and_single_cosine():
+    """c_0 of f == 1 is 1 (reading C7); rho = 1 + A cos(kx + phi) gives c_m = (A/2) e^{i phi}
+    and E = -(A/k) sin(kx + phi)  (Eq. 68-71 with E = -Phi')."""
+    lo, hi, N, n = 0.0, 20 * np.pi, 32, 8
+    x = fourier.node_coordinates(lo, hi, N, n)
+    T = fourier.transform_tensor(lo, hi, N, n, 16)
+    c = fourier.fourier_project(T, np.ones_like(x))
+    assert abs(c[0] - 1) < 1e-14 and np.max(np.abs(c[1:])) < 1e-14
+    A, phi = 0.01, 0.3
+    for m in (1, 3, 5):
+        k = 2 * np.pi * m / (hi - lo)
+        rho = 1 + A * np.cos(k * x + phi)
+        c = fourier.fourier_project(T, rho)
+        assert abs(c[m] - 0.5 * A * np.exp(1j * phi)) < 1e-13 * 1 + 2e-15
+        E = fourier.poisson_E(lo, hi, x, c)
+        Eex = -(A / k) * np.sin(k * x + phi)
+        assert np.max(np.abs(E - Eex)) / np.max(np.abs(Eex)) < 1e-11, m
+
+
+def test_config1_grid_accuracy():
+    """n = 4, N = 16 (config 1): closed-form E only to ~1e-6 (discretisation)."""
+    lo, hi, N, n = 0.0, 4 * np.pi, 16, 4
+    x = fourier.node_coordinates(lo, hi, N, n)
+    T = fourier.transform_tensor(lo, hi, N, n, 16)
+    rho = 1 + 0.01 * np.cos(0.5 * x)
+    E = fourier.poisson_E(lo, hi, x, fourier.fourier_project(T, rho))
+    Eex = -0.02 * np.sin(0.5 * x)
+    err = np.max(np.abs(E - Eex)) / 0.02
+    assert 1e-10 < err < 2e-6
+
+
+def test_E_is_continuous_and_derivative_matches_source():
+    """The Fourier series is single valued: E agrees at duplicated interface nodes."""
+    lo, hi, N, n = 0.0, 2 * np.pi, 10, 8
+    rng = np.random.default_rng(5)
+    x = fourier.node_coordinates(lo, hi, N, n)
+    rho = np.sin(x) + rng.standard_normal(x.size)
+    T = fourier.transform_tensor(lo, hi, N, n, 10)
+    E = fourier.poisson_E(lo, hi, x, fourier.fourier_project(T, rho)).reshape(N, n)
+    assert np.allclose(E[:-1, -1], E[1:, 0], atol=1e-13)
+    assert abs(E[-1, -1] - E[0, 0]) < 1e-13
+
+
+def _broken_l2(err_fn, lo, hi, N):
+    """Eq. 72: (1/N) sum_m sqrt(int_m err^2) by 20-point Gauss quadrature per element."""
+    xg, wg = npleg.leggauss(20)
+    dx = (hi - lo) / N
+    tot = 0.0
+    for m in range(N):
+        xm = lo + (m + 0.5) * dx + 0.5 * dx * xg
+        tot += np.sqrt(np.sum(wg * err_fn(xm, m) ** 2) * 0.5 * dx)
+    return tot / N
+
+
+@pytest.mark.parametrize("n", [3, 4, 5, 6])
+def test_poisson_convergence_fig4(n):
+    """Fig. 4: Phi'' = sin(2 pi x) on [0,1], N = 10..25: error O(dx^{n+1/2}) in the
+    broken l2 norm of Eq. 72 (Phi interpolated on the element basis, Eq. 69)."""
+    lo, hi = 0.0, 1.0
+    errs, Ns = [], [10, 15, 20, 25]
+    xi, _ = basis.lgl_nodes_weights(n)
+    for N in Ns:
+        x = fourier.node_coordinates(lo, hi, N, n)
+        T = fourier.transform_tensor(lo, hi, N, n, N)
+        c = fourier.fourier_project(T, np.sin(2 * np.pi * x))
+        Phi = fourier.poisson_phi(lo, hi, x, c).reshape(N, n)
+        dx = 1.0 / N
+
+        def err(xm, m):
+            loc = (xm - (lo + (m + 0.5) * dx)) / (0.5 * dx)
+            return _lagrange_values(xi, loc).T @ Phi[m] + np.sin(2 * np.pi * xm) / (4 * np.pi ** 2)
+        errs.append(_broken_l2(err, lo, hi, N))
+    slope = np.polyfit(np.log(1.0 / np.array(Ns)), np.log(errs), 1)[0]
+    assert n - 0.2 < slope < n + 1.6, (slope, errs)
