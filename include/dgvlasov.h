@@ -1,0 +1,126 @@
+/* dgvlasov.h -- C ABI of the B200-native tensor-product DG Vlasov-Poisson hot path.
+ *
+ * Method: D. W. Crews, "Analysis of tensor-product discontinuous Galerkin operators for
+ * Vlasov-Poisson simulations and GPU implementation on Python", arXiv 2202.13532.
+ * Citations below are "PAPER.md:<line>" (the text under /root/reference) plus the equation.
+ *
+ * Conventions
+ *  - Phase-space dimensions d = 0,1,2 are (x, u, v) = (x, v_x, v_y)  [ndim = 3, 1D2V] or
+ *    (x, v) [ndim = 2, 1D1V]; ndim = 1 describes x only (field-solve-only context).
+ *  - N_d elements and n_d LGL nodes per element in dimension d; global node index
+ *    g_d = a_d * n_d + b_d (element a, node b).  Interface nodes are duplicated.
+ *  - The distribution is ONE dense row-major FP64 array f[g_x][g_u][g_v] (f[g_x][g_v] for
+ *    ndim = 2): the paper's u[a0,b0,a1,b1,a2,b2] in C order (Section 3.1).
+ *  - Every pointer named *_dev is a DEVICE pointer owned by the caller (e.g. a torch
+ *    tensor); the library never frees or reallocates it.  Pointers named *_host are host
+ *    memory.  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *  - Calls taking a stream only enqueue work on it and never synchronise.  Calls taking
+ *    host buffers synchronise before returning.
+ *  - Every call returns 0 (DG_OK) or a negative error code; dg_last_error() gives the
+ *    message of the calling thread's last failure.  There is NO CPU fallback: a shape the
+ *    kernels do not support is DG_ERR_UNSUPPORTED.
+ */
+#ifndef DGVLASOV_H
+#define DGVLASOV_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DG_OK                 0
+#define DG_ERR_INVALID_ARG   -1
+#define DG_ERR_UNSUPPORTED   -2
+#define DG_ERR_CUDA          -3
+#define DG_ERR_WORKSPACE     -4
+
+#define DG_MAX_ORDER         10   /* LGL nodes per element per dimension: 2..10 */
+
+typedef struct dg_ctx dg_ctx;
+
+typedef struct {
+  int32_t ndim;        /* 1 = x only (field solve), 2 = 1D1V (x,v), 3 = 1D2V (x,vx,vy) */
+  int32_t nelem[3];    /* N_d, elements per dimension (unused dims: 0) */
+  int32_t order[3];    /* n_d, LGL nodes per element per dimension, 2..DG_MAX_ORDER */
+  double  lo[3];       /* lower bounds; x is [lo,hi) periodic */
+  double  hi[3];       /* upper bounds */
+  int32_t bc[3];       /* 0 periodic (the paper's roll), 1 zero-inflow
+                          (exterior state 0); bc[0] must be 0 when the Poisson solve is used */
+  double  omega_c;     /* = B_ext of Eq. 28; ignored for ndim < 3 */
+  int32_t pmax;        /* Fourier modes kept, p = 0..pmax; 0 -> nelem[0] */
+  int32_t mass_mode;   /* 0 = the paper's exact LGL mass matrix (Eq. 51/53/54);
+                          1 = lumped (diagonal) LGL mass: Ups = (w_k/w_j) l_j'(xi_k), Xi = delta/w */
+  int32_t device;      /* CUDA device ordinal */
+} dg_grid_desc;
+
+/* Host setup (Eq. 45, 53, 54, 63): LGL nodes/weights, Upsilon, Xi, quadrature
+ * weights, node coordinates, the DG->Fourier tensor T (Eq. 63) and the synthesis matrix of
+ * Eq. 71; uploads them.  *out owns that device memory until dg_destroy. */
+int dg_create(const dg_grid_desc* desc, dg_ctx** out);
+int dg_destroy(dg_ctx* ctx);
+
+/* Scratch for dg_ssprk3_* and dg_poisson_E: two stage arrays of the size of f, density
+ * partials, rho, c_p, E.  The caller allocates `bytes >= dg_workspace_bytes(ctx)` of device
+ * memory (256-byte aligned) and keeps it alive while the context uses it. */
+size_t dg_workspace_bytes(const dg_ctx* ctx);
+int dg_set_workspace(dg_ctx* ctx, void* ws_dev, size_t bytes);
+
+/* Semi-discrete right-hand side, weak form Eq. 14 reduced by Eq. 20-21
+ * with the upwind flux Eq. 23 and the speeds of Eq. 28
+ * (PAPER.md:215):  dfdt = sum_d J_d ( a_d Ups_d f - Xi_d Flux_d ).
+ *   f_dev    [in]  distribution, layout above
+ *   E_dev    [in]  electric field at the x nodes, [N_x*n_x]; NULL means E = 0
+ *   dfdt_dev [out] same shape as f; must not alias f_dev */
+int dg_rhs(dg_ctx* ctx, const double* f_dev, const double* E_dev, double* dfdt_dev, void* stream);
+
+/* Shu-Osher SSP-RK3: u1 = u + dt L(u); u2 = 3/4 u + 1/4 (u1 + dt L(u1));
+ * u+ = 1/3 u + 2/3 (u2 + dt L(u2)), in place on f_dev.  self_consistent = 1: E is solved from
+ * each stage's input (density Eq. 27 -> c_p Eq. 63 -> E Eq. 71); 0: E = 0.  Needs a workspace.
+ * dg_ssprk3_run does `nsteps` steps in one call and is what lets the density partials of a
+ * stage's output, produced in that stage's epilogue, serve the next stage's field solve. */
+int dg_ssprk3_step(dg_ctx* ctx, double* f_dev, double dt, int32_t self_consistent, void* stream);
+int dg_ssprk3_run(dg_ctx* ctx, double* f_dev, double dt, int32_t nsteps, int32_t self_consistent, void* stream);
+/* Same with a HOST array: copies f in, runs nsteps, copies f back, synchronises. */
+int dg_ssprk3_run_host(dg_ctx* ctx, double* f_host, double dt, int32_t nsteps, int32_t self_consistent);
+
+/* Zeroth moment Eq. 27 by LGL quadrature: rho[g_x] = sum_{g_u,g_v}
+ * (w_{b_u}/J_u)(w_{b_v}/J_v) f.  rho_dev: [N_x*n_x].  Deterministic (no atomics). */
+int dg_density(dg_ctx* ctx, const double* f_dev, double* rho_dev, void* stream);
+
+/* c_p = T_p^{mj} rho_mj, Eq. 63, p = 0..pmax.
+ *   rho_dev [in]  [batch][N_x*n_x]
+ *   c_dev   [out] [batch][pmax+1][2]  (re, im) */
+int dg_fourier_project(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* c_dev, void* stream);
+
+/* E from the density by Eq. 63 + Eq. 71: E_mj = sum_{0<|p|<=pmax}
+ * -(c_p/(i k_p)) e^{i k_p x_mj}; the p = 0 mode (neutralising background of Eq. 27) is dropped.
+ *   rho_dev [in] [batch][N_x*n_x]     E_dev [out] [batch][N_x*n_x]
+ * batch > 1 needs workspace room for batch*(pmax+1)*2 doubles (see dg_field_workspace_bytes). */
+int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_dev, void* stream);
+size_t dg_field_workspace_bytes(const dg_ctx* ctx, int32_t batch);
+
+/* Introspection (host outputs; any pointer may be NULL to skip it). */
+int dg_get_operators(const dg_ctx* ctx, int32_t dim, double* xi_host /*[n]*/, double* w_host /*[n]*/,
+                     double* upsilon_host /*[n][n], row j = output node, reference element*/,
+                     double* lift_host /*[n][2]: (L,R)*/);
+int dg_get_nodes(const dg_ctx* ctx, int32_t dim, double* coords_host /*[N_d*n_d]*/);
+int dg_get_transform(const dg_ctx* ctx, int32_t p_first, int32_t p_count, double* T_host /*[p_count][N_x*n_x][2]*/);
+/* Largest dt with sum_d |a_d| dt / Delta_d <= the SSP-RK3 limit of this order and mass mode
+ * at |E| <= E_bound (PAPER.md:477 defers the CFL numbers to its ref. [39]). */
+double dg_max_stable_dt(const dg_ctx* ctx, double E_bound);
+
+/* Options and counters. */
+#define DG_OPT_RHS_KERNEL   1   /* 0 auto (tiled when supported), 1 generic, 2 tiled (error if unsupported) */
+#define DG_OPT_FIELD_KERNEL 2   /* 0 auto, 1 simple kernels, 2 tiled GEMM kernels */
+int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value);
+int64_t dg_launch_count(const dg_ctx* ctx);      /* kernels launched through this context so far */
+const char* dg_last_kernel(const dg_ctx* ctx);   /* name of the RHS kernel variant last used */
+const char* dg_last_error(void);
+const char* dg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DGVLASOV_H */

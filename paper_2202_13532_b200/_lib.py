@@ -1,0 +1,67 @@
+"""ctypes loader for libdgvlasov.so -- the C ABI declared in include/dgvlasov.h.
+
+There is no fallback: if the library has not been built (python -m paper_2202_13532_b200.build)
+importing the binding raises."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libdgvlasov.so")
+
+
+class GridDesc(C.Structure):
+    _fields_ = [
+        ("ndim", C.c_int32),
+        ("nelem", C.c_int32 * 3),
+        ("order", C.c_int32 * 3),
+        ("lo", C.c_double * 3),
+        ("hi", C.c_double * 3),
+        ("bc", C.c_int32 * 3),
+        ("omega_c", C.c_double),
+        ("pmax", C.c_int32),
+        ("mass_mode", C.c_int32),
+        ("device", C.c_int32),
+    ]
+
+
+_vp, _dp, _i32, _i64, _dbl = C.c_void_p, C.POINTER(C.c_double), C.c_int32, C.c_int64, C.c_double
+
+# name -> (restype, argtypes); must list every symbol include/dgvlasov.h declares
+SIGNATURES = {
+    "dg_create": (C.c_int, [C.POINTER(GridDesc), C.POINTER(_vp)]),
+    "dg_destroy": (C.c_int, [_vp]),
+    "dg_workspace_bytes": (C.c_size_t, [_vp]),
+    "dg_field_workspace_bytes": (C.c_size_t, [_vp, _i32]),
+    "dg_set_workspace": (C.c_int, [_vp, _vp, C.c_size_t]),
+    "dg_rhs": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "dg_ssprk3_step": (C.c_int, [_vp, _vp, _dbl, _i32, _vp]),
+    "dg_ssprk3_run": (C.c_int, [_vp, _vp, _dbl, _i32, _i32, _vp]),
+    "dg_ssprk3_run_host": (C.c_int, [_vp, _vp, _dbl, _i32, _i32]),
+    "dg_density": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "dg_fourier_project": (C.c_int, [_vp, _vp, _i32, _vp, _vp]),
+    "dg_poisson_E": (C.c_int, [_vp, _vp, _i32, _vp, _vp]),
+    "dg_get_operators": (C.c_int, [_vp, _i32, _dp, _dp, _dp, _dp]),
+    "dg_get_nodes": (C.c_int, [_vp, _i32, _dp]),
+    "dg_get_transform": (C.c_int, [_vp, _i32, _i32, _dp]),
+    "dg_max_stable_dt": (_dbl, [_vp, _dbl]),
+    "dg_set_option": (C.c_int, [_vp, _i32, _i64]),
+    "dg_launch_count": (_i64, [_vp]),
+    "dg_last_kernel": (C.c_char_p, [_vp]),
+    "dg_last_error": (C.c_char_p, []),
+    "dg_version": (C.c_char_p, []),
+}
+
+
+def load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2202_13532_b200.build` "
+            "(there is no CPU or PyTorch fallback for the DG kernels)")
+    lib = C.CDLL(LIB_PATH)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)          # AttributeError if the symbol is not exported
+        fn.restype = res
+        fn.argtypes = args
+    return lib

@@ -1,0 +1,164 @@
+"""Thin Python binding over the C ABI (include/dgvlasov.h): argument marshalling only.
+
+torch provides device memory and streams; every step of the path runs in the library's kernels.
+Method names mirror the C entry points (dg_rhs -> DGContext.rhs, ...)."""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+import torch
+
+from . import _lib
+
+_L = _lib.load()
+
+OPT_RHS_KERNEL = 1
+OPT_FIELD_KERNEL = 2
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
+
+
+class DGError(RuntimeError):
+    pass
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise DGError(f"{what} failed ({rc}): {_L.dg_last_error().decode()}")
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise DGError("expected a contiguous float64 CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream(device):
+    return torch.cuda.current_stream(device).cuda_stream
+
+
+def version() -> str:
+    return _L.dg_version().decode()
+
+
+class DGContext:
+    """dg_create / dg_destroy plus one method per C entry point."""
+
+    def __init__(self, nelem, order, lo, hi, bc=None, omega_c=0.0, pmax=0, mass_mode=0, device=0,
+                 workspace=True, field_batch=1):
+        ndim = len(nelem)
+        if bc is None:
+            bc = (0,) + (1,) * (ndim - 1)
+        d = _lib.GridDesc()
+        d.ndim = ndim
+        for i in range(3):
+            d.nelem[i] = int(nelem[i]) if i < ndim else 0
+            d.order[i] = int(order[i]) if i < ndim else 0
+            d.lo[i] = float(lo[i]) if i < ndim else 0.0
+            d.hi[i] = float(hi[i]) if i < ndim else 0.0
+            d.bc[i] = int(bc[i]) if i < ndim else 0
+        d.omega_c, d.pmax, d.mass_mode, d.device = float(omega_c), int(pmax), int(mass_mode), int(device)
+        self._h = C.c_void_p()
+        _check(_L.dg_create(C.byref(d), C.byref(self._h)), "dg_create")
+        self.ndim, self.nelem, self.order = ndim, tuple(nelem), tuple(order)
+        self.device = torch.device("cuda", device)
+        self.flat_shape = tuple(int(nelem[i]) * int(order[i]) for i in range(ndim))
+        self.pmax = int(pmax) if pmax > 0 else int(nelem[0])
+        self._ws = None
+        if workspace:
+            nbytes = _L.dg_field_workspace_bytes(self._h, int(field_batch))
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            _check(_L.dg_set_workspace(self._h, base, nbytes), "dg_set_workspace")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            _L.dg_destroy(self._h)
+            self._h = C.c_void_p()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # --- compute entry points -----------------------------------------------------------------
+    def rhs(self, f, E=None, out=None):
+        out = torch.empty_like(f) if out is None else out
+        _check(_L.dg_rhs(self._h, _ptr(f), _ptr(E), _ptr(out), _stream(self.device)), "dg_rhs")
+        return out
+
+    def ssprk3_step(self, f, dt, self_consistent=True):
+        _check(_L.dg_ssprk3_step(self._h, _ptr(f), float(dt), int(bool(self_consistent)), _stream(self.device)), "dg_ssprk3_step")
+        return f
+
+    def ssprk3_run(self, f, dt, nsteps, self_consistent=True):
+        _check(_L.dg_ssprk3_run(self._h, _ptr(f), float(dt), int(nsteps), int(bool(self_consistent)), _stream(self.device)), "dg_ssprk3_run")
+        return f
+
+    def ssprk3_run_host(self, f_host, dt, nsteps, self_consistent=True):
+        """f_host: contiguous float64 CPU tensor or NumPy array, updated in place."""
+        if isinstance(f_host, np.ndarray):
+            assert f_host.dtype == np.float64 and f_host.flags["C_CONTIGUOUS"]
+            p = f_host.ctypes.data
+        else:
+            assert f_host.dtype == torch.float64 and f_host.is_contiguous() and not f_host.is_cuda
+            p = f_host.data_ptr()
+        _check(_L.dg_ssprk3_run_host(self._h, p, float(dt), int(nsteps), int(bool(self_consistent))), "dg_ssprk3_run_host")
+        return f_host
+
+    def density(self, f, out=None):
+        out = torch.empty(self.flat_shape[0], dtype=torch.float64, device=self.device) if out is None else out
+        _check(_L.dg_density(self._h, _ptr(f), _ptr(out), _stream(self.device)), "dg_density")
+        return out
+
+    def fourier_project(self, rho, out=None):
+        rho2 = rho.reshape(-1, self.flat_shape[0])
+        batch = rho2.shape[0]
+        out = torch.empty((batch, self.pmax + 1, 2), dtype=torch.float64, device=self.device) if out is None else out
+        _check(_L.dg_fourier_project(self._h, _ptr(rho2), batch, _ptr(out), _stream(self.device)), "dg_fourier_project")
+        return out
+
+    def poisson_E(self, rho, out=None):
+        rho2 = rho.reshape(-1, self.flat_shape[0])
+        batch = rho2.shape[0]
+        out = torch.empty_like(rho2) if out is None else out
+        _check(_L.dg_poisson_E(self._h, _ptr(rho2), batch, _ptr(out), _stream(self.device)), "dg_poisson_E")
+        return out.reshape(rho.shape)
+
+    # --- introspection ------------------------------------------------------------------------
+    def operators(self, dim):
+        n = self.order[dim]
+        xi, w = np.empty(n), np.empty(n)
+        ups, lift = np.empty((n, n)), np.empty((n, 2))
+        dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+        _check(_L.dg_get_operators(self._h, dim, dp(xi), dp(w), dp(ups), dp(lift)), "dg_get_operators")
+        return xi, w, ups, lift
+
+    def nodes(self, dim):
+        x = np.empty(self.flat_shape[dim])
+        _check(_L.dg_get_nodes(self._h, dim, x.ctypes.data_as(C.POINTER(C.c_double))), "dg_get_nodes")
+        return x
+
+    def transform(self, p_first=0, p_count=None):
+        p_count = self.pmax + 1 - p_first if p_count is None else p_count
+        T = np.empty((p_count, self.flat_shape[0], 2))
+        _check(_L.dg_get_transform(self._h, p_first, p_count, T.ctypes.data_as(C.POINTER(C.c_double))), "dg_get_transform")
+        return T[..., 0] + 1j * T[..., 1]
+
+    def max_stable_dt(self, E_bound=0.0):
+        return float(_L.dg_max_stable_dt(self._h, float(E_bound)))
+
+    def set_option(self, key, value):
+        _check(_L.dg_set_option(self._h, int(key), int(value)), "dg_set_option")
+
+    @property
+    def launch_count(self):
+        return int(_L.dg_launch_count(self._h))
+
+    @property
+    def last_kernel(self):
+        return _L.dg_last_kernel(self._h).decode()

@@ -1,0 +1,424 @@
+// C-ABI entry points of libdgvlasov (see include/dgvlasov.h).  Argument checking, workspace carving
+// and kernel launches only; all arithmetic of the path runs in the kernels.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "dg_context.hpp"
+#include "dg_kernels_generic.cuh"
+#include "dg_kernels_tiled.cuh"
+#include "dg_kernels_field.cuh"
+
+static thread_local std::string g_err;
+
+static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+
+#define CUDA_TRY(expr)                                                                   \
+  do {                                                                                   \
+    cudaError_t _e = (expr);                                                             \
+    if (_e != cudaSuccess)                                                               \
+      return fail(DG_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(_e));      \
+  } while (0)
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static int check_launch(dg_ctx* ctx, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  ctx->launches += 1;
+  return DG_OK;
+}
+
+extern "C" const char* dg_last_error(void) { return g_err.c_str(); }
+extern "C" const char* dg_version(void) { return "dgvlasov-b200 0.1 (sm_100a)"; }
+
+// ------------------------------------------------------------------------------------------------
+// create / destroy
+// ------------------------------------------------------------------------------------------------
+extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
+  if (!desc || !out) return fail(DG_ERR_INVALID_ARG, "dg_create: null argument");
+  *out = nullptr;
+  if (desc->ndim < 1 || desc->ndim > 3) return fail(DG_ERR_INVALID_ARG, "dg_create: ndim must be 1, 2 or 3");
+  for (int d = 0; d < desc->ndim; ++d) {
+    if (desc->nelem[d] < 1) return fail(DG_ERR_INVALID_ARG, "dg_create: nelem must be >= 1");
+    if (desc->order[d] < 2 || desc->order[d] > DG_MAX_ORDER)
+      return fail(DG_ERR_UNSUPPORTED, "dg_create: order must be 2..10");
+    if (!(desc->hi[d] > desc->lo[d])) return fail(DG_ERR_INVALID_ARG, "dg_create: hi must exceed lo");
+    if (desc->bc[d] != 0 && desc->bc[d] != 1) return fail(DG_ERR_INVALID_ARG, "dg_create: bc must be 0 or 1");
+  }
+  if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dg_create: mass_mode must be 0 or 1");
+  if (desc->pmax < 0) return fail(DG_ERR_INVALID_ARG, "dg_create: pmax must be >= 0");
+  CUDA_TRY(cudaSetDevice(desc->device));
+
+  dg_ctx* ctx = new (std::nothrow) dg_ctx();
+  if (!ctx) return fail(DG_ERR_CUDA, "dg_create: out of host memory");
+  ctx->desc = *desc;
+  ctx->ndim = desc->ndim;
+  size_t dof = 1;
+  for (int d = 0; d < desc->ndim; ++d) {
+    ctx->N[d] = desc->nelem[d];
+    ctx->n[d] = desc->order[d];
+    ctx->G[d] = ctx->N[d] * ctx->n[d];
+    ctx->J[d] = 2.0 * ctx->N[d] / (desc->hi[d] - desc->lo[d]);
+    dof *= (size_t)ctx->G[d];
+  }
+  ctx->dof = desc->ndim >= 2 ? dof : 0;
+  ctx->pmax = desc->pmax > 0 ? desc->pmax : desc->nelem[0];
+  ctx->P1 = ctx->pmax + 1;
+
+  std::vector<double> T, S, x;
+  try {
+    for (int d = 0; d < desc->ndim; ++d) ctx->basis[d] = dgsetup::make_basis(ctx->n[d], desc->mass_mode);
+    dgsetup::make_fourier(ctx->basis[0], ctx->N[0], desc->lo[0], desc->hi[0], ctx->pmax, T, S, x);
+  } catch (const std::exception& e) {
+    delete ctx;
+    return fail(DG_ERR_INVALID_ARG, std::string("dg_create: setup failed: ") + e.what());
+  }
+  // node coordinates and quadrature weights per flat node
+  std::vector<double> wq[3];
+  for (int d = 0; d < desc->ndim; ++d) {
+    const int n = ctx->n[d];
+    ctx->coord_h[d].resize(ctx->G[d]);
+    wq[d].resize(ctx->G[d]);
+    const long double dx = ((long double)desc->hi[d] - (long double)desc->lo[d]) / ctx->N[d];
+    for (int m = 0; m < ctx->N[d]; ++m)
+      for (int j = 0; j < n; ++j) {
+        ctx->coord_h[d][m * n + j] = (double)((long double)desc->lo[d] + (m + 0.5L) * dx + 0.5L * dx * ctx->basis[d].xi_ld[j]);
+        wq[d][m * n + j] = (double)(ctx->basis[d].w_ld[j] * dx * 0.5L);      // w_b / J_d
+      }
+  }
+  ctx->coord_h[0] = x;
+
+  // one device block for all constants
+  size_t off = 0;
+  size_t o_ups[3], o_lift[3], o_coord[3], o_wq[3];
+  for (int d = 0; d < desc->ndim; ++d) {
+    o_ups[d] = off;   off = align_up(off + sizeof(double) * ctx->n[d] * ctx->n[d], 256);
+    o_lift[d] = off;  off = align_up(off + sizeof(double) * ctx->n[d] * 2, 256);
+    o_coord[d] = off; off = align_up(off + sizeof(double) * ctx->G[d], 256);
+    o_wq[d] = off;    off = align_up(off + sizeof(double) * ctx->G[d], 256);
+  }
+  const size_t o_T = off; off = align_up(off + sizeof(double) * T.size(), 256);
+  const size_t o_S = off; off = align_up(off + sizeof(double) * S.size(), 256);
+  cudaError_t e = cudaMalloc(&ctx->dev_block, off);
+  if (e != cudaSuccess) { delete ctx; return fail(DG_ERR_CUDA, std::string("dg_create: cudaMalloc: ") + cudaGetErrorString(e)); }
+  char* base = (char*)ctx->dev_block;
+  bool ok = true;
+  for (int d = 0; d < desc->ndim && ok; ++d) {
+    ctx->d_ups[d] = (double*)(base + o_ups[d]);
+    ctx->d_lift[d] = (double*)(base + o_lift[d]);
+    ctx->d_coord[d] = (double*)(base + o_coord[d]);
+    ctx->d_wq[d] = (double*)(base + o_wq[d]);
+    ok = ok && cudaMemcpy(ctx->d_ups[d], ctx->basis[d].ups.data(), sizeof(double) * ctx->n[d] * ctx->n[d], cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = ok && cudaMemcpy(ctx->d_lift[d], ctx->basis[d].lift.data(), sizeof(double) * ctx->n[d] * 2, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = ok && cudaMemcpy(ctx->d_coord[d], ctx->coord_h[d].data(), sizeof(double) * ctx->G[d], cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = ok && cudaMemcpy(ctx->d_wq[d], wq[d].data(), sizeof(double) * ctx->G[d], cudaMemcpyHostToDevice) == cudaSuccess;
+  }
+  ctx->d_T = (double*)(base + o_T);
+  ctx->d_S = (double*)(base + o_S);
+  ok = ok && cudaMemcpy(ctx->d_T, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+  ok = ok && cudaMemcpy(ctx->d_S, S.data(), sizeof(double) * S.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+  if (!ok) {
+    cudaFree(ctx->dev_block);
+    delete ctx;
+    return fail(DG_ERR_CUDA, "dg_create: upload failed");
+  }
+  if (T.size() <= (size_t)1 << 22) ctx->T_h.swap(T);     // small tensors stay on the host for introspection
+  *out = ctx;
+  return DG_OK;
+}
+
+extern "C" int dg_destroy(dg_ctx* ctx) {
+  if (!ctx) return DG_OK;
+  if (ctx->dev_block) cudaFree(ctx->dev_block);
+  if (ctx->f_stage) cudaFree(ctx->f_stage);
+  delete ctx;
+  return DG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// workspace
+// ------------------------------------------------------------------------------------------------
+static size_t partials_doubles(const dg_ctx* ctx) {
+  // density partials: at most 1024 chunks per x node (generic kernel) or one per tile (tiled kernel)
+  if (ctx->ndim < 2) return 0;
+  size_t per_gx = 1024;
+  return (size_t)ctx->G[0] * per_gx;
+}
+
+static size_t fixed_ws_bytes(const dg_ctx* ctx) {
+  size_t b = 0;
+  b += 2 * align_up(ctx->dof * sizeof(double), 256);
+  b += align_up(partials_doubles(ctx) * sizeof(double), 256);
+  b += 2 * align_up((size_t)ctx->G[0] * sizeof(double), 256);   // rho, E
+  return b;
+}
+
+extern "C" size_t dg_field_workspace_bytes(const dg_ctx* ctx, int32_t batch) {
+  if (!ctx || batch < 1) return 0;
+  return fixed_ws_bytes(ctx) + align_up((size_t)batch * 2 * ctx->P1 * sizeof(double), 256);
+}
+
+extern "C" size_t dg_workspace_bytes(const dg_ctx* ctx) { return dg_field_workspace_bytes(ctx, 1); }
+
+extern "C" int dg_set_workspace(dg_ctx* ctx, void* ws_dev, size_t bytes) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_workspace: null context");
+  if (!ws_dev || ((uintptr_t)ws_dev & 255) != 0) return fail(DG_ERR_INVALID_ARG, "dg_set_workspace: pointer must be non-null and 256-byte aligned");
+  if (bytes < dg_workspace_bytes(ctx)) return fail(DG_ERR_WORKSPACE, "dg_set_workspace: too small, see dg_workspace_bytes");
+  char* p = (char*)ws_dev;
+  ctx->ws = ws_dev; ctx->ws_bytes = bytes;
+  ctx->u1 = (double*)p; p += align_up(ctx->dof * sizeof(double), 256);
+  ctx->u2 = (double*)p; p += align_up(ctx->dof * sizeof(double), 256);
+  ctx->partials_doubles = partials_doubles(ctx);
+  ctx->partials = (double*)p; p += align_up(ctx->partials_doubles * sizeof(double), 256);
+  ctx->rho = (double*)p; p += align_up((size_t)ctx->G[0] * sizeof(double), 256);
+  ctx->E = (double*)p; p += align_up((size_t)ctx->G[0] * sizeof(double), 256);
+  ctx->cbuf = (double*)p;
+  ctx->cbuf_doubles = (bytes - (size_t)(p - (char*)ws_dev)) / sizeof(double);
+  return DG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// internal launch helpers
+// ------------------------------------------------------------------------------------------------
+static int launch_rhs_generic(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out,
+                              int mode, double c0, double c1, double dt, cudaStream_t st) {
+  dgk::GenericParams p;
+  memset(&p, 0, sizeof(p));
+  p.ndim = ctx->ndim;
+  for (int d = 0; d < 3; ++d) {
+    p.N[d] = ctx->N[d]; p.n[d] = ctx->n[d]; p.G[d] = ctx->G[d]; p.bc[d] = ctx->desc.bc[d];
+    p.ups[d] = ctx->d_ups[d]; p.lift[d] = ctx->d_lift[d]; p.coord[d] = ctx->d_coord[d]; p.J[d] = ctx->J[d];
+  }
+  p.omega_c = ctx->desc.omega_c;
+  p.E = E; p.f = f; p.fn = fn; p.out = out; p.c0 = c0; p.c1 = c1; p.dt = dt; p.mode = mode;
+  p.dof = (long long)ctx->dof;
+  long long blocks = ((long long)ctx->dof + 255) / 256;
+  if (blocks > 148LL * 64) blocks = 148LL * 64;
+  dgk::rhs_generic_kernel<<<(unsigned)blocks, 256, 0, st>>>(p);
+  ctx->last_kernel = "rhs_generic";
+  return check_launch(ctx, "rhs_generic_kernel");
+}
+
+// One RHS (+ optional stage combination, + optional density partials of `out` when the tiled kernel
+// runs).  *partials_written is set when the kernel left per-tile density partials of `out` in
+// ctx->partials (ntile chunks per x node).
+static int launch_rhs(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
+                      double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
+  if (partial_chunks) *partial_chunks = 0;
+  const bool tiled_ok = dgt::tiled_supported(ctx);
+  if (ctx->opt_rhs_kernel == 2 && !tiled_ok) return fail(DG_ERR_UNSUPPORTED, "tiled RHS kernel does not support this grid");
+  if (tiled_ok && ctx->opt_rhs_kernel != 1) {
+    int rc = dgt::launch_rhs_tiled(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    if (rc != DG_OK) return fail(rc, std::string("tiled RHS launch failed: ") + dgt::last_error());
+    return check_launch(ctx, "rhs_tiled_kernel");
+  }
+  return launch_rhs_generic(ctx, f, fn, E, out, mode, c0, c1, dt, st);
+}
+
+static int launch_density(dg_ctx* ctx, const double* f, double* rho, double* partial, size_t partial_cap, cudaStream_t st) {
+  const int G0 = ctx->G[0], G1 = ctx->G[1], G2 = ctx->ndim == 3 ? ctx->G[2] : 1;
+  // chunking of the G1 rows of each velocity plane
+  int nchunks, rows;
+  if (G2 == 1) { rows = 4096; nchunks = (G1 + rows - 1) / rows; }
+  else {
+    int target = (int)((148LL * 8 + G0 - 1) / G0);         // enough CTAs to fill the chip
+    if (target < 1) target = 1;
+    if (target > G1) target = G1;
+    rows = (G1 + target - 1) / target;
+    nchunks = (G1 + rows - 1) / rows;
+  }
+  if ((size_t)nchunks * G0 > partial_cap) return fail(DG_ERR_WORKSPACE, "density partial buffer too small");
+  dim3 grid(nchunks, G0);
+  dgk::density_partial_kernel<<<grid, 256, 0, st>>>(f, ctx->d_wq[1], ctx->ndim == 3 ? ctx->d_wq[2] : nullptr, G1, G2, rows, partial);
+  int rc = check_launch(ctx, "density_partial_kernel");
+  if (rc) return rc;
+  dgk::density_finish_kernel<<<(G0 + 3) / 4, 128, 0, st>>>(partial, nchunks, G0, rho);
+  return check_launch(ctx, "density_finish_kernel");
+}
+
+static int launch_density_finish(dg_ctx* ctx, const double* partial, int nchunks, double* rho, cudaStream_t st) {
+  dgk::density_finish_kernel<<<(ctx->G[0] + 3) / 4, 128, 0, st>>>(partial, nchunks, ctx->G[0], rho);
+  return check_launch(ctx, "density_finish_kernel");
+}
+
+static int launch_project(dg_ctx* ctx, const double* rho, int batch, double* c, cudaStream_t st) {
+  const int G = ctx->G[0], P1 = ctx->P1;
+  const bool big = dgf::gemm_worthwhile(batch, 2 * P1, G);
+  if (ctx->opt_field_kernel == 2 || (ctx->opt_field_kernel == 0 && big)) {
+    // C[batch][2*P1] = rho[batch][G] * T[2*P1][G]^T
+    int rc = dgf::launch_gemm_tn(rho, ctx->d_T, c, batch, 2 * P1, G, st);
+    if (rc != DG_OK) return fail(rc, "projection GEMM launch failed");
+    return check_launch(ctx, "field_gemm_kernel");
+  }
+  dim3 grid(P1, batch);
+  dgk::project_simple_kernel<<<grid, 128, 0, st>>>(ctx->d_T, rho, G, P1, c);
+  return check_launch(ctx, "project_simple_kernel");
+}
+
+static int launch_synth(dg_ctx* ctx, const double* c, int batch, double* E, cudaStream_t st) {
+  const int G = ctx->G[0], Q = 2 * ctx->P1;
+  const bool big = dgf::gemm_worthwhile(batch, G, Q);
+  if (ctx->opt_field_kernel == 2 || (ctx->opt_field_kernel == 0 && big)) {
+    // E[batch][G] = c[batch][Q] * S[G][Q]^T
+    int rc = dgf::launch_gemm_tn(c, ctx->d_S, E, batch, G, Q, st);
+    if (rc != DG_OK) return fail(rc, "synthesis GEMM launch failed");
+    return check_launch(ctx, "field_gemm_kernel");
+  }
+  dim3 grid((G + 3) / 4, batch);
+  dgk::synth_simple_kernel<<<grid, 128, 0, st>>>(ctx->d_S, c, G, Q, E);
+  return check_launch(ctx, "synth_simple_kernel");
+}
+
+// ------------------------------------------------------------------------------------------------
+// public compute entry points
+// ------------------------------------------------------------------------------------------------
+extern "C" int dg_rhs(dg_ctx* ctx, const double* f_dev, const double* E_dev, double* dfdt_dev, void* stream) {
+  if (!ctx || !f_dev || !dfdt_dev) return fail(DG_ERR_INVALID_ARG, "dg_rhs: null argument");
+  if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_rhs: field-only context (ndim = 1)");
+  if (f_dev == dfdt_dev) return fail(DG_ERR_INVALID_ARG, "dg_rhs: dfdt must not alias f");
+  return launch_rhs(ctx, f_dev, nullptr, E_dev, dfdt_dev, 0, 0.0, 1.0, 0.0, false, nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int dg_density(dg_ctx* ctx, const double* f_dev, double* rho_dev, void* stream) {
+  if (!ctx || !f_dev || !rho_dev) return fail(DG_ERR_INVALID_ARG, "dg_density: null argument");
+  if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_density: field-only context (ndim = 1)");
+  if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_density: set a workspace first (partials live there)");
+  return launch_density(ctx, f_dev, rho_dev, ctx->partials, ctx->partials_doubles, (cudaStream_t)stream);
+}
+
+extern "C" int dg_fourier_project(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* c_dev, void* stream) {
+  if (!ctx || !rho_dev || !c_dev) return fail(DG_ERR_INVALID_ARG, "dg_fourier_project: null argument");
+  if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_fourier_project: batch must be >= 1");
+  return launch_project(ctx, rho_dev, batch, c_dev, (cudaStream_t)stream);
+}
+
+extern "C" int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_dev, void* stream) {
+  if (!ctx || !rho_dev || !E_dev) return fail(DG_ERR_INVALID_ARG, "dg_poisson_E: null argument");
+  if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_poisson_E: batch must be >= 1");
+  if (ctx->desc.bc[0] != 0) return fail(DG_ERR_INVALID_ARG, "dg_poisson_E: x must be periodic");
+  if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_poisson_E: set a workspace first");
+  if ((size_t)batch * 2 * ctx->P1 > ctx->cbuf_doubles)
+    return fail(DG_ERR_WORKSPACE, "dg_poisson_E: workspace too small for this batch, see dg_field_workspace_bytes");
+  int rc = launch_project(ctx, rho_dev, batch, ctx->cbuf, (cudaStream_t)stream);
+  if (rc) return rc;
+  return launch_synth(ctx, ctx->cbuf, batch, E_dev, (cudaStream_t)stream);
+}
+
+static int field_from_partials_or_f(dg_ctx* ctx, const double* f, int partial_chunks, cudaStream_t st) {
+  int rc;
+  if (partial_chunks > 0) rc = launch_density_finish(ctx, ctx->partials, partial_chunks, ctx->rho, st);
+  else rc = launch_density(ctx, f, ctx->rho, ctx->partials, ctx->partials_doubles, st);
+  if (rc) return rc;
+  rc = launch_project(ctx, ctx->rho, 1, ctx->cbuf, st);
+  if (rc) return rc;
+  return launch_synth(ctx, ctx->cbuf, 1, ctx->E, st);
+}
+
+extern "C" int dg_ssprk3_run(dg_ctx* ctx, double* f_dev, double dt, int32_t nsteps, int32_t self_consistent, void* stream) {
+  if (!ctx || !f_dev) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: null argument");
+  if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_ssprk3: field-only context (ndim = 1)");
+  if (nsteps < 0 || !(dt == dt)) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: bad nsteps or dt");
+  if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_ssprk3: set a workspace first");
+  if (self_consistent && ctx->desc.bc[0] != 0) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: self-consistent E needs periodic x");
+  cudaStream_t st = (cudaStream_t)stream;
+  int chunks = 0;          // > 0: ctx->partials holds density partials of the current stage input
+  for (int s = 0; s < nsteps; ++s) {
+    const double* E = nullptr;
+    int rc;
+    // stage 1: u1 = u + dt L(u)
+    if (self_consistent) { rc = field_from_partials_or_f(ctx, f_dev, chunks, st); if (rc) return rc; E = ctx->E; }
+    rc = launch_rhs(ctx, f_dev, nullptr, E, ctx->u1, 1, 0.0, 1.0, dt, self_consistent != 0, &chunks, st);
+    if (rc) return rc;
+    // stage 2: u2 = 3/4 u + 1/4 (u1 + dt L(u1))
+    if (self_consistent) { rc = field_from_partials_or_f(ctx, ctx->u1, chunks, st); if (rc) return rc; }
+    rc = launch_rhs(ctx, ctx->u1, f_dev, E, ctx->u2, 1, 0.75, 0.25, dt, self_consistent != 0, &chunks, st);
+    if (rc) return rc;
+    // stage 3: u = 1/3 u + 2/3 (u2 + dt L(u2)), in place (each node of u is read and written by one thread)
+    if (self_consistent) { rc = field_from_partials_or_f(ctx, ctx->u2, chunks, st); if (rc) return rc; }
+    rc = launch_rhs(ctx, ctx->u2, f_dev, E, f_dev, 1, 1.0 / 3.0, 2.0 / 3.0, dt, self_consistent != 0, &chunks, st);
+    if (rc) return rc;
+  }
+  return DG_OK;
+}
+
+extern "C" int dg_ssprk3_step(dg_ctx* ctx, double* f_dev, double dt, int32_t self_consistent, void* stream) {
+  return dg_ssprk3_run(ctx, f_dev, dt, 1, self_consistent, stream);
+}
+
+extern "C" int dg_ssprk3_run_host(dg_ctx* ctx, double* f_host, double dt, int32_t nsteps, int32_t self_consistent) {
+  if (!ctx || !f_host) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3_run_host: null argument");
+  if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_ssprk3_run_host: field-only context (ndim = 1)");
+  const size_t bytes = ctx->dof * sizeof(double);
+  if (!ctx->f_stage) CUDA_TRY(cudaMalloc(&ctx->f_stage, bytes));
+  CUDA_TRY(cudaMemcpyAsync(ctx->f_stage, f_host, bytes, cudaMemcpyHostToDevice, 0));
+  int rc = dg_ssprk3_run(ctx, ctx->f_stage, dt, nsteps, self_consistent, nullptr);
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(f_host, ctx->f_stage, bytes, cudaMemcpyDeviceToHost, 0));
+  CUDA_TRY(cudaStreamSynchronize(0));
+  return DG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// introspection / options
+// ------------------------------------------------------------------------------------------------
+extern "C" int dg_get_operators(const dg_ctx* ctx, int32_t dim, double* xi, double* w, double* ups, double* lift) {
+  if (!ctx || dim < 0 || dim >= ctx->ndim) return fail(DG_ERR_INVALID_ARG, "dg_get_operators: bad argument");
+  const dgsetup::Basis1D& b = ctx->basis[dim];
+  if (xi) memcpy(xi, b.xi.data(), sizeof(double) * b.n);
+  if (w) memcpy(w, b.w.data(), sizeof(double) * b.n);
+  if (ups) memcpy(ups, b.ups.data(), sizeof(double) * b.n * b.n);
+  if (lift) memcpy(lift, b.lift.data(), sizeof(double) * b.n * 2);
+  return DG_OK;
+}
+
+extern "C" int dg_get_nodes(const dg_ctx* ctx, int32_t dim, double* coords) {
+  if (!ctx || !coords || dim < 0 || dim >= ctx->ndim) return fail(DG_ERR_INVALID_ARG, "dg_get_nodes: bad argument");
+  memcpy(coords, ctx->coord_h[dim].data(), sizeof(double) * ctx->G[dim]);
+  return DG_OK;
+}
+
+extern "C" int dg_get_transform(const dg_ctx* ctx, int32_t p_first, int32_t p_count, double* T_host) {
+  if (!ctx || !T_host || p_first < 0 || p_count < 0 || p_first + p_count > ctx->P1)
+    return fail(DG_ERR_INVALID_ARG, "dg_get_transform: bad argument");
+  const int G = ctx->G[0];
+  std::vector<double> rows((size_t)2 * p_count * G);
+  CUDA_TRY(cudaMemcpy(rows.data(), ctx->d_T + (size_t)2 * p_first * G, sizeof(double) * rows.size(), cudaMemcpyDeviceToHost));
+  for (int p = 0; p < p_count; ++p)
+    for (int g = 0; g < G; ++g) {
+      T_host[((size_t)p * G + g) * 2] = rows[(size_t)(2 * p) * G + g];
+      T_host[((size_t)p * G + g) * 2 + 1] = rows[(size_t)(2 * p + 1) * G + g];
+    }
+  return DG_OK;
+}
+
+extern "C" double dg_max_stable_dt(const dg_ctx* ctx, double E_bound) {
+  if (!ctx || ctx->ndim < 2) return 0.0;
+  dg_ctx* c = const_cast<dg_ctx*>(ctx);
+  // per-dimension limits add: sum_d |a_d|_max / (nu_d Delta_d) * dt <= 1
+  double sum = 0.0;
+  auto vmax = [&](int d) { return std::fmax(std::fabs(ctx->desc.lo[d]), std::fabs(ctx->desc.hi[d])); };
+  double amax[3] = {0, 0, 0};
+  if (ctx->ndim == 2) { amax[0] = vmax(1); amax[1] = std::fabs(E_bound); }
+  else { amax[0] = vmax(1); amax[1] = std::fabs(E_bound) + std::fabs(ctx->desc.omega_c) * vmax(2); amax[2] = std::fabs(ctx->desc.omega_c) * vmax(1); }
+  for (int d = 0; d < ctx->ndim; ++d) {
+    const double nu = dgsetup::rk3_cfl_limit(c->basis[d]);
+    const double delta = (ctx->desc.hi[d] - ctx->desc.lo[d]) / ctx->N[d];
+    sum += amax[d] / (nu * delta);
+  }
+  return sum > 0.0 ? 1.0 / sum : INFINITY;
+}
+
+extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_option: null context");
+  if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
+  if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 2) { ctx->opt_field_kernel = (int)value; return DG_OK; }
+  return fail(DG_ERR_INVALID_ARG, "dg_set_option: unknown key or value");
+}
+
+extern "C" int64_t dg_launch_count(const dg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" const char* dg_last_kernel(const dg_ctx* ctx) { return ctx ? ctx->last_kernel.c_str() : "none"; }

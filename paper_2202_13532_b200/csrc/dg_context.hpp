@@ -1,0 +1,46 @@
+// Internal context of the C-ABI library (not part of the public boundary).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/dgvlasov.h"
+#include "dg_setup.hpp"
+
+struct dg_ctx {
+  dg_grid_desc desc;
+  int ndim = 0;
+  int N[3] = {0, 0, 0};       // elements per dim
+  int n[3] = {0, 0, 0};       // nodes per element per dim
+  int G[3] = {1, 1, 1};       // flat nodes per dim (1 for unused dims)
+  size_t dof = 0;             // prod G over used dims (0 for ndim == 1)
+  int pmax = 0, P1 = 1;
+  double J[3] = {0, 0, 0};    // 2 / Delta_d                                     (Eq. 61)
+  dgsetup::Basis1D basis[3];
+  std::vector<double> coord_h[3];
+  std::vector<double> T_h;    // kept on the host only until uploaded, then for dg_get_transform
+
+  // device constants (one allocation, carved)
+  void* dev_block = nullptr;
+  double* d_ups[3] = {nullptr, nullptr, nullptr};    // reference Upsilon [n][n]
+  double* d_lift[3] = {nullptr, nullptr, nullptr};   // reference Xi [n][2]
+  double* d_coord[3] = {nullptr, nullptr, nullptr};  // node coordinates [G_d]
+  double* d_wq[3] = {nullptr, nullptr, nullptr};     // quadrature weight w_b / J_d per flat node [G_d]
+  double* d_T = nullptr;      // [2*P1][G0]   rows 2p / 2p+1 = Re / Im of T_p (Eq. 63)
+  double* d_S = nullptr;      // [G0][2*P1]   synthesis rows of Eq. 71 with -1/(i k_p) folded in
+
+  // caller-provided workspace
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  double *u1 = nullptr, *u2 = nullptr, *partials = nullptr, *rho = nullptr, *E = nullptr, *cbuf = nullptr;
+  size_t cbuf_doubles = 0, partials_doubles = 0;
+
+  // library-owned staging for the host entry point
+  double* f_stage = nullptr;
+
+  int64_t launches = 0;
+  int opt_rhs_kernel = 0, opt_field_kernel = 0;
+  std::string last_kernel = "none";
+  double cfl_limit = -1.0;    // lazily computed
+};

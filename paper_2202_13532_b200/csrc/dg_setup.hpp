@@ -1,0 +1,27 @@
+// Host-side setup of the LGL basis, DG operators and the DG->Fourier tensor (see dg_setup.cpp).
+#pragma once
+#include <vector>
+
+namespace dgsetup {
+
+struct Basis1D {
+  int n = 0;
+  std::vector<double> xi, w;        // LGL nodes / weights on [-1,1]            (Eq. 45)
+  std::vector<long double> xi_ld, w_ld;
+  std::vector<double> ups;          // Upsilon[j*n + k], reference element      (Eq. 53)
+  std::vector<double> lift;         // Xi[j*2 + {0:L,1:R}]                      (Eq. 54)
+};
+
+Basis1D make_basis(int n, int mass_mode);
+
+// T[(2p+c)*G + g]   : c = 0 real, 1 imaginary part of T_p^{mj} of Eq. 63, g = m*n + j
+// S[g*2*(pmax+1) + 2p + c] : synthesis row of Eq. 71 with the Poisson factor -1/(i k_p) folded in,
+//                     so that E[g] = sum_{p,c} S[g][2p+c] * c_p[c]; columns of p = 0 are zero.
+// x[g]              : node coordinates.
+void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
+                  std::vector<double>& T, std::vector<double>& S, std::vector<double>& x);
+
+// Largest a*dt/dx for which SSP-RK3 is stable on the 1-D periodic upwind DG operator built from `b`.
+double rk3_cfl_limit(const Basis1D& b);
+
+}  // namespace dgsetup
