@@ -1,0 +1,282 @@
+#!/usr/bin/env python
+"""bench.py -- DOF-updates/s per RK stage of the fused DG RHS + SSP-RK3 step (with the Poisson
+solve every stage) on the 1D2V production grid, through the C ABI (libdgvlasov.so).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A step = one SSP-RK3 step = 3 x (density -> c_p -> E -> fused RHS + stage combine) over the whole
+grid.  Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "FP64 phase-space DOF-updates/s per RK stage"
+UNIT = "DOF-updates/s"
+K_WAVE = 0.1
+
+WORKLOADS = {
+    # BASELINE.json configs[2]: the production grid the north_star's 70 % target is quoted on
+    "config3_1d2v_512^3": dict(nelem=(64, 64, 64), order=(8, 8, 8), dt=5e-4, noise=1e-4),
+    # BASELINE.json configs[1]
+    "config2_1d2v_256^3": dict(nelem=(32, 32, 32), order=(8, 8, 8), dt=1e-3, noise=0.0),
+    # small replica for quick checks
+    "small_1d2v_128^3": dict(nelem=(16, 16, 16), order=(8, 8, 8), dt=1e-3, noise=1e-4),
+}
+BYTES_PER_DOF_PER_STAGE = 64.0 / 3.0     # stage 1 reads f, writes u1 (16 B); stages 2,3 read f_s, f_n, write out (24 B)
+
+
+def grid_args(w):
+    return dict(nelem=w["nelem"], order=w["order"], lo=(0.0, -8.5, -8.5), hi=(2 * math.pi / K_WAVE, 8.5, 8.5),
+                bc=(0, 1, 1), omega_c=1.0, pmax=w["nelem"][0])
+
+
+def make_f0(x, vx, vy, w):
+    import workloads as wl
+    f0 = wl.ring_f0(x, vx, vy, K_WAVE)
+    if w["noise"]:
+        f0 = wl.add_uniform_noise(f0, wl.SEED_CFG3_NOISE, w["noise"])
+    return np.ascontiguousarray(f0)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for l in self.lines:
+            p = [s.strip() for s in l.split(",")]
+            if len(p) < 8:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peak_hbm():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# -----------------------------------------------------------------------------------------------
+# reference arm: the oracle on the host cores, bounded sample of the same workload
+# -----------------------------------------------------------------------------------------------
+def oracle_sample(w, steps, warmup, x_elems=2):
+    """One SSP-RK3 step of the oracle on an x-slab (x_elems of the N_x elements, full velocity grid,
+    periodic in x within the slab) of the workload.  Returns (DOF-updates/s per stage, cores, description)."""
+    from oracle import vlasov as ov
+    import workloads as wl
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+    ga = grid_args(w)
+    nelem = (x_elems,) + tuple(ga["nelem"][1:])
+    hi = (ga["hi"][0] * x_elems / ga["nelem"][0],) + tuple(ga["hi"][1:])
+    g = ov.Grid(nelem=nelem, order=ga["order"], lo=ga["lo"], hi=hi, bc=ga["bc"], omega_c=ga["omega_c"], pmax=x_elems)
+    f = make_f0(g.coords[0].reshape(-1), g.coords[1].reshape(-1), g.coords[2].reshape(-1), w)
+    for _ in range(warmup):
+        ov.ssprk3_step(g, f, w["dt"])
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        f = ov.ssprk3_step(g, f, w["dt"])
+    dt_wall = time.perf_counter() - t0
+    dof = f.size
+    value = dof * 3.0 * steps / dt_wall
+    desc = (f"oracle.vlasov.ssprk3_step (NumPy), x-slab of {x_elems}/{ga['nelem'][0]} x-elements x full velocity grid "
+            f"= {dof} DOF, {steps} step(s)")
+    return value, cores, desc, dt_wall / max(steps, 1)
+
+
+def run_reference(args, w, name):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, min(args.steps, 3))
+    value, cores, desc, sec_per_step = oracle_sample(w, steps, min(args.warmup, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * sec_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "note": "CPU oracle on a bounded x-slab sample of the workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# -----------------------------------------------------------------------------------------------
+# our arm
+# -----------------------------------------------------------------------------------------------
+def run_ours(args, w, name):
+    import torch
+    import torch.distributed as dist
+    from paper_2202_13532_b200 import api
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the DG kernels have no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(v):
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    ga = grid_args(w)
+    ctx = api.DGContext(device=local, **ga)
+    f0 = make_f0(ctx.nodes(0), ctx.nodes(1), ctx.nodes(2), w)
+    dof = f0.size
+    dt = w["dt"]
+    f = torch.from_numpy(f0).to(dev)
+
+    # warm-up, then K timed steps, device-timed, barrier + synchronize on both sides
+    ctx.ssprk3_run(f, dt, args.warmup, True)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = ctx.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    ctx.ssprk3_run(f, dt, args.steps, True)
+    e1.record()
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1))
+    clocks = sampler.stop() if rank == 0 else None
+    launches = ctx.launch_count - l0
+    finite = bool(torch.isfinite(f).all().item())
+    value = world * dof * 3.0 * args.steps / (ms * 1e-3)
+
+    # roofline of the dominant kernel (fused RHS + stage): per-launch events inside the library
+    ctx.set_option(api.OPT_PROFILE, 1)
+    ctx.get_profile(reset=True)
+    psteps = max(1, min(args.steps, 10))
+    ctx.ssprk3_run(f, dt, psteps, True)
+    rhs_ms, rhs_n = ctx.get_profile(reset=True)
+    ctx.set_option(api.OPT_PROFILE, 0)
+    kernel = ctx.last_kernel
+    peak, peak_src = measured_peak_hbm()
+    avg_launch_s = rhs_ms * 1e-3 / max(rhs_n, 1)
+    achieved = BYTES_PER_DOF_PER_STAGE * dof / avg_launch_s / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "kernel": kernel, "avg_launch_ms": avg_launch_s * 1e3, "launches_timed": rhs_n,
+                "algorithmic_bytes_per_launch": BYTES_PER_DOF_PER_STAGE * dof, "peak_source": peak_src,
+                "rhs_share_of_step": (rhs_ms / psteps) / (ms / args.steps)}
+
+    # end to end through the host-buffer entry point: H2D of f, K steps of 1, D2H of f, every step
+    e2e_steps = max(1, min(args.steps, 3))
+    fh = torch.from_numpy(f0.copy()).pin_memory()
+    ctx.ssprk3_run_host(fh, dt, 1, True)          # warm-up (allocates the staging array)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ctx.ssprk3_run_host(fh, dt, 1, True)
+    barrier()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e = {"value": world * dof * 3.0 * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": dof * 8,
+           "d2h_bytes_per_step": dof * 8, "steps": e2e_steps, "api": "dg_ssprk3_run_host (pinned host buffer)"}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, cores, desc, _ = oracle_sample(w, 1, 0)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "grid": "x".join(str(n * o) for n, o in zip(w["nelem"], w["order"])), "dof": dof,
+                       "dt": dt, "self_consistent_poisson_each_stage": True, "mass_mode": 0,
+                       "l2": "inputs (3 x %.2f GB) larger than L2; no flush needed" % (dof * 8 / 1e9),
+                       "parallelism": "replicas x%d" % world, "finite": finite},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "hbm_gbs_algorithmic_whole_step": 64.0 * dof * args.steps / (ms * 1e-3) / 1e9,
+        }
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config3_1d2v_512^3", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = WORKLOADS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w, args.workload)
+    else:
+        run_ours(args, w, args.workload)
+
+
+if __name__ == "__main__":
+    main()

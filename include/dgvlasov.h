@@ -114,7 +114,11 @@ double dg_max_stable_dt(const dg_ctx* ctx, double E_bound);
 /* Options and counters. */
 #define DG_OPT_RHS_KERNEL   1   /* 0 auto (tiled when supported), 1 generic, 2 tiled (error if unsupported) */
 #define DG_OPT_FIELD_KERNEL 2   /* 0 auto, 1 simple kernels, 2 tiled GEMM kernels */
+#define DG_OPT_PROFILE      3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
 int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value);
+/* Profile mode: total device time (ms) and count of the RHS-kernel launches since the last reset.
+ * Synchronises on the recorded events. */
+int dg_get_profile(dg_ctx* ctx, double* rhs_ms_total_host, int64_t* rhs_launches_host, int32_t reset);
 int64_t dg_launch_count(const dg_ctx* ctx);      /* kernels launched through this context so far */
 const char* dg_last_kernel(const dg_ctx* ctx);   /* name of the RHS kernel variant last used */
 const char* dg_last_error(void);

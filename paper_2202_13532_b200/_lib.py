@@ -47,6 +47,7 @@ SIGNATURES = {
     "dg_get_transform": (C.c_int, [_vp, _i32, _i32, _dp]),
     "dg_max_stable_dt": (_dbl, [_vp, _dbl]),
     "dg_set_option": (C.c_int, [_vp, _i32, _i64]),
+    "dg_get_profile": (C.c_int, [_vp, _dp, C.POINTER(_i64), _i32]),
     "dg_launch_count": (_i64, [_vp]),
     "dg_last_kernel": (C.c_char_p, [_vp]),
     "dg_last_error": (C.c_char_p, []),

@@ -15,6 +15,7 @@ _L = _lib.load()
 
 OPT_RHS_KERNEL = 1
 OPT_FIELD_KERNEL = 2
+OPT_PROFILE = 3
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 
 
@@ -154,6 +155,11 @@ class DGContext:
 
     def set_option(self, key, value):
         _check(_L.dg_set_option(self._h, int(key), int(value)), "dg_set_option")
+
+    def get_profile(self, reset=True):
+        ms, cnt = C.c_double(0.0), C.c_int64(0)
+        _check(_L.dg_get_profile(self._h, C.byref(ms), C.byref(cnt), int(bool(reset))), "dg_get_profile")
+        return ms.value, cnt.value
 
     @property
     def launch_count(self):

@@ -136,6 +136,7 @@ extern "C" int dg_destroy(dg_ctx* ctx) {
   if (!ctx) return DG_OK;
   if (ctx->dev_block) cudaFree(ctx->dev_block);
   if (ctx->f_stage) cudaFree(ctx->f_stage);
+  for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
   delete ctx;
   return DG_OK;
 }
@@ -147,6 +148,7 @@ static size_t partials_doubles(const dg_ctx* ctx) {
   // density partials: at most 1024 chunks per x node (generic kernel) or one per tile (tiled kernel)
   if (ctx->ndim < 2) return 0;
   size_t per_gx = 1024;
+  if (dgt::tiled_supported(ctx) && (size_t)dgt::tiled_partial_chunks(ctx) > per_gx) per_gx = dgt::tiled_partial_chunks(ctx);
   return (size_t)ctx->G[0] * per_gx;
 }
 
@@ -207,8 +209,26 @@ static int launch_rhs_generic(dg_ctx* ctx, const double* f, const double* fn, co
 // One RHS (+ optional stage combination, + optional density partials of `out` when the tiled kernel
 // runs).  *partials_written is set when the kernel left per-tile density partials of `out` in
 // ctx->partials (ntile chunks per x node).
+static int launch_rhs_inner(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
+                            double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st);
+
+// In profile mode (DG_OPT_PROFILE) every RHS launch is bracketed by events on its own stream.
 static int launch_rhs(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                       double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
+  if (!ctx->opt_profile) return launch_rhs_inner(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  CUDA_TRY(cudaEventRecord(e0, st));
+  int rc = launch_rhs_inner(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+  CUDA_TRY(cudaEventRecord(e1, st));
+  ctx->prof_events.push_back(e0);
+  ctx->prof_events.push_back(e1);
+  return rc;
+}
+
+static int launch_rhs_inner(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
+                            double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
   if (partial_chunks) *partial_chunks = 0;
   const bool tiled_ok = dgt::tiled_supported(ctx);
   if (ctx->opt_rhs_kernel == 2 && !tiled_ok) return fail(DG_ERR_UNSUPPORTED, "tiled RHS kernel does not support this grid");
@@ -413,8 +433,27 @@ extern "C" double dg_max_stable_dt(const dg_ctx* ctx, double E_bound) {
   return sum > 0.0 ? 1.0 / sum : INFINITY;
 }
 
+extern "C" int dg_get_profile(dg_ctx* ctx, double* rhs_ms_total, int64_t* rhs_launches, int32_t reset) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_get_profile: null context");
+  for (size_t i = 0; i + 1 < ctx->prof_events.size(); i += 2) {
+    CUDA_TRY(cudaEventSynchronize(ctx->prof_events[i + 1]));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, ctx->prof_events[i], ctx->prof_events[i + 1]));
+    ctx->prof_rhs_ms += ms;
+    ctx->prof_rhs_launches += 1;
+    cudaEventDestroy(ctx->prof_events[i]);
+    cudaEventDestroy(ctx->prof_events[i + 1]);
+  }
+  ctx->prof_events.clear();
+  if (rhs_ms_total) *rhs_ms_total = ctx->prof_rhs_ms;
+  if (rhs_launches) *rhs_launches = ctx->prof_rhs_launches;
+  if (reset) { ctx->prof_rhs_ms = 0.0; ctx->prof_rhs_launches = 0; }
+  return DG_OK;
+}
+
 extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_option: null context");
+  if (key == DG_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
   if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 2) { ctx->opt_field_kernel = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg_set_option: unknown key or value");

