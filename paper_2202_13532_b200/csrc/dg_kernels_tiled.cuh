@@ -87,8 +87,16 @@ template <int NN, int KV>
 struct TileCfg {
   static constexpr int R = KV * NN;                 // row length (doubles)
   static constexpr int NT = NN * NN * KV;           // threads per CTA
-  static constexpr int a128(int b) { return (b + 127) / 128 * 128; }
+  static constexpr int ROWS = NN * NN;
+  // 256-byte rows are held as two 128-byte half-rows in TMA SWIZZLE_128B layout (16-byte chunk index
+  // XOR row mod 8), which makes the per-line 128-bit accesses of the v phase bank-conflict free.
+  static constexpr bool SWZ = (R == 32);
+  static constexpr int a128(int b) { return (b + 1023) / 1024 * 1024; }
   static constexpr int SZ_MAIN = a128(NN * NN * R * 8);
+  // offset (in doubles) of node (row = jx*NN + ju, c) inside a main-tile buffer
+  __host__ __device__ static constexpr int idx(int row, int c) {
+    return SWZ ? ((c >> 4) * (ROWS * 16) + row * 16 + (((((c & 15) >> 1) ^ (row & 7))) << 1) + (c & 1)) : (row * R + c);
+  }
   static constexpr int SZ_FACE = a128(NN * R * 8);
   static constexpr int SZ_V = a128(NN * NN * 2 * 8);
   static constexpr int OFF_F = 0;
@@ -102,7 +110,7 @@ struct TileCfg {
   static constexpr int OFF_VR = OFF_VL + SZ_V;
   static constexpr int OFF_RED = OFF_VR + SZ_V;
   static constexpr int OFF_BAR = OFF_RED + a128(NT * 8);
-  static constexpr int SMEM_BYTES = OFF_BAR + 128 + 128;   // + slack for manual 128-B alignment
+  static constexpr int SMEM_BYTES = OFF_BAR + 128 + 1024;  // + slack for manual 1024-B alignment
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -113,7 +121,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
   using Cfg = TileCfg<NN, KV>;
   constexpr int R = Cfg::R, NT = Cfg::NT;
   extern __shared__ unsigned char smem_raw[];
-  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   double* sF = reinterpret_cast<double*>(smem + Cfg::OFF_F);
   double* sN = reinterpret_cast<double*>(smem + Cfg::OFF_N);
   double* sA = reinterpret_cast<double*>(smem + Cfg::OFF_A);
@@ -161,7 +169,12 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
     if (av_pos) bytes += NN * NN * 2 * 8;
     if (av_neg) bytes += NN * NN * 2 * 8;
     mbar_expect_tx(bar, bytes);
-    tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
+    if (Cfg::SWZ) {
+      tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
+      tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
+    } else {
+      tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
+    }
     // Periodic wrap (the paper's roll) by coordinate; zero inflow by letting the box fall
     // outside the tensor, where TMA fills zeros (exterior state 0, reading C2).
     if (ax_pos) tma_load_3d(smem_u32(sXL), &P.m_xface, bar, c0, gu0, (ex > 0) ? gx0 - 1 : (P.bc0 == 0 ? P.G0 - 1 : -1));
@@ -173,7 +186,10 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
       const int cend = c0 + kvalid * NN;
       tma_load_3d(smem_u32(sVR), &P.m_vface, bar, (cend < P.G2) ? cend : (P.bc2 == 0 ? 0 : P.G2), gu0, gx0);
     }
-    if (P.has_fn) tma_load_3d(smem_u32(sN), &P.m_fn, bar, c0, gu0, gx0);
+    if (P.has_fn) {
+      tma_load_3d(smem_u32(sN), &P.m_fn, bar, c0, gu0, gx0);
+      if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
+    }
   }
   __syncthreads();           // barrier init visible to all waiters
   mbar_wait(bar, 0);
@@ -184,7 +200,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
     const double a = P.Jx * P.vx[gu0 + ju];                       // a_x = u            (Eq. 28)
     double f[NN];
 #pragma unroll
-    for (int k = 0; k < NN; ++k) f[k] = sF[(k * NN + ju) * R + c];
+    for (int k = 0; k < NN; ++k) f[k] = sF[Cfg::idx(k * NN + ju, c)];
     const double uL = (a > 0.0) ? sXL[ju * R + c] : f[0];          // upwind states, Eq. 23
     const double uR = (a < 0.0) ? sXR[ju * R + c] : f[NN - 1];
 #pragma unroll
@@ -193,7 +209,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
       s = fma(-P.liftR[j], uR, s);
 #pragma unroll
       for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
-      sA[(j * NN + ju) * R + c] = a * s;
+      sA[Cfg::idx(j * NN + ju, c)] = a * s;
     }
   }
   __syncthreads();
@@ -205,7 +221,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
     const double a = P.Ju * (-Ex - P.omega_c * P.vy[gv]);         // a_u = -E - omega_c v  (Eq. 28, E = -Phi')
     double f[NN];
 #pragma unroll
-    for (int k = 0; k < NN; ++k) f[k] = sF[(jx * NN + k) * R + c];
+    for (int k = 0; k < NN; ++k) f[k] = sF[Cfg::idx(jx * NN + k, c)];
     const double uL = (a > 0.0) ? sUL[jx * R + c] : f[0];
     const double uR = (a < 0.0) ? sUR[jx * R + c] : f[NN - 1];
 #pragma unroll
@@ -214,30 +230,32 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
       s = fma(-P.liftR[j], uR, s);
 #pragma unroll
       for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
-      const int o = (jx * NN + j) * R + c;
+      const int o = Cfg::idx(jx * NN + j, c);
       sA[o] = fma(a, s, sA[o]);
     }
   }
   __syncthreads();
   // ---------------- phase v: thread = (jx, ju, ev), line over the v nodes of element ev ----------------
   {
-    const int ev = t % KV, ju = (t / KV) % NN, jx = t / (KV * NN);
+    // ju fastest: the 8 lanes of a quarter warp read 8 different rows at the same c, which the swizzle
+    // spreads over all banks
+    const int ju = t % NN, ev = (t / NN) % KV, jx = t / (KV * NN);
     double psum = 0.0;
     if (ev < kvalid) {
-      const int row = (jx * NN + ju) * R;
-      const int o = row + ev * NN;
+      const int row = jx * NN + ju;
+      const int cl = ev * NN;
       const double a = P.Jv * (P.omega_c * P.vx[gu0 + ju]);       // a_v = omega_c u     (Eq. 28)
       double f[NN], acc[NN];
 #pragma unroll
       for (int k = 0; k < NN; k += 2) {
-        const double2 v2 = *reinterpret_cast<const double2*>(&sF[o + k]);
+        const double2 v2 = *reinterpret_cast<const double2*>(&sF[Cfg::idx(row, cl + k)]);
         f[k] = v2.x; f[k + 1] = v2.y;
-        const double2 a2 = *reinterpret_cast<const double2*>(&sA[o + k]);
+        const double2 a2 = *reinterpret_cast<const double2*>(&sA[Cfg::idx(row, cl + k)]);
         acc[k] = a2.x; acc[k + 1] = a2.y;
       }
       double uL = f[0], uR = f[NN - 1];
-      if (a > 0.0) uL = (ev > 0) ? sF[o - 1] : sVL[(jx * NN + ju) * 2 + 1];
-      if (a < 0.0) uR = (ev < kvalid - 1) ? sF[o + NN] : sVR[(jx * NN + ju) * 2];
+      if (a > 0.0) uL = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
+      if (a < 0.0) uR = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
       double outv[NN];
 #pragma unroll
       for (int j = 0; j < NN; ++j) {
@@ -254,14 +272,14 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
         if (P.has_fn) {
 #pragma unroll
           for (int k = 0; k < NN; k += 2) {
-            const double2 n2 = *reinterpret_cast<const double2*>(&sN[o + k]);
+            const double2 n2 = *reinterpret_cast<const double2*>(&sN[Cfg::idx(row, cl + k)]);
             outv[k] = fma(P.c0, n2.x, outv[k]);
             outv[k + 1] = fma(P.c0, n2.y, outv[k + 1]);
           }
         }
       }
 #pragma unroll
-      for (int k = 0; k < NN; k += 2) *reinterpret_cast<double2*>(&sN[o + k]) = make_double2(outv[k], outv[k + 1]);
+      for (int k = 0; k < NN; k += 2) *reinterpret_cast<double2*>(&sN[Cfg::idx(row, cl + k)]) = make_double2(outv[k], outv[k + 1]);
       if (P.want_partials) {
         // Eq. 27: LGL quadrature of the stage output over this thread's v line
         const double* w2 = P.wq2 + c0 + ev * NN;
@@ -276,6 +294,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
   __syncthreads();
   if (t == 0) {
     tma_store_3d(&P.m_out, smem_u32(sN), c0, gu0, gx0);
+    if (Cfg::SWZ) tma_store_3d(&P.m_out, smem_u32(sN + Cfg::ROWS * 16), c0 + 16, gu0, gx0);
     tma_store_commit_and_wait_read();
   }
   if (P.want_partials && t >= 32 && t < 32 + NN) {
@@ -322,7 +341,7 @@ inline EncodeTiledFn encode_fn() {
   return fn;
 }
 
-inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0, int b1, int b2) {
+inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0, int b1, int b2, bool swz128 = false) {
   EncodeTiledFn enc = encode_fn();
   if (!enc) { g_tiled_err = "cuTensorMapEncodeTiled not available"; return false; }
   const cuuint64_t dims[3] = {(cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)ctx->G[0]};
@@ -330,7 +349,7 @@ inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0
   const cuuint32_t box[3] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2};
   const cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, swz128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { g_tiled_err = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r); return false; }
   return true;
@@ -343,9 +362,10 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   TiledParams<NN> P;
   const int R = Cfg::R;
   if (((uintptr_t)f & 15) || ((uintptr_t)out & 15) || (fn && ((uintptr_t)fn & 15))) { g_tiled_err = "arrays must be 16-byte aligned"; return DG_ERR_INVALID_ARG; }
-  if (!make_map(&P.m_main, f, ctx, R, NN, NN) || !make_map(&P.m_xface, f, ctx, R, NN, 1) ||
+  const int RB = Cfg::SWZ ? 16 : R;      // swizzled tiles move as two 128-byte-wide boxes
+  if (!make_map(&P.m_main, f, ctx, RB, NN, NN, Cfg::SWZ) || !make_map(&P.m_xface, f, ctx, R, NN, 1) ||
       !make_map(&P.m_uface, f, ctx, R, 1, NN) || !make_map(&P.m_vface, f, ctx, 2, NN, NN) ||
-      !make_map(&P.m_fn, fn ? fn : f, ctx, R, NN, NN) || !make_map(&P.m_out, out, ctx, R, NN, NN))
+      !make_map(&P.m_fn, fn ? fn : f, ctx, RB, NN, NN, Cfg::SWZ) || !make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ))
     return DG_ERR_CUDA;
   const dgsetup::Basis1D& b = ctx->basis[0];
   for (int j = 0; j < NN; ++j) {
