@@ -70,13 +70,13 @@ struct alignas(64) TiledParams {
   double ups[NN * NN];   // reference Upsilon[j][k]   (Eq. 53)
   double liftL[NN];      // Xi[j][L]                   (Eq. 54)
   double liftR[NN];      // Xi[j][R]
+  double wref[NN];       // LGL weights on [-1,1]      (Eq. 45)
   const double* vx;      // node coordinates of dim 1 (u = v_x)
   const double* vy;      // node coordinates of dim 2 (v = v_y)
   const double* E;       // [G0] or nullptr
-  const double* wq1;     // quadrature weights w_b/J per flat node, dim 1
-  const double* wq2;     // dim 2
   double* partials;      // [G0][N1*tiles_v] density partials of the output (want_partials)
   double Jx, Ju, Jv, omega_c;
+  double wscale;         // 1/(J_u J_v): quadrature weight of node (b_u, b_v) = wref[b_u] wref[b_v] wscale
   double c0, c1, dt;     // out = c0*fn + c1*(f + dt*rhs)  (mode 1);  out = rhs (mode 0)
   int N0, N1, N2, G0, G1, G2;
   int bc0, bc1, bc2;
@@ -101,8 +101,7 @@ struct TileCfg {
   static constexpr int SZ_V = a128(NN * NN * 2 * 8);
   static constexpr int OFF_F = 0;
   static constexpr int OFF_N = OFF_F + SZ_MAIN;
-  static constexpr int OFF_A = OFF_N + SZ_MAIN;
-  static constexpr int OFF_XL = OFF_A + SZ_MAIN;
+  static constexpr int OFF_XL = OFF_N + SZ_MAIN;
   static constexpr int OFF_XR = OFF_XL + SZ_FACE;
   static constexpr int OFF_UL = OFF_XR + SZ_FACE;
   static constexpr int OFF_UR = OFF_UL + SZ_FACE;
@@ -110,7 +109,7 @@ struct TileCfg {
   static constexpr int OFF_VR = OFF_VL + SZ_V;
   static constexpr int OFF_RED = OFF_VR + SZ_V;
   static constexpr int OFF_BAR = OFF_RED + a128(NT * 8);
-  static constexpr int SMEM_BYTES = OFF_BAR + 128 + 1024;  // + slack for manual 1024-B alignment
+  static constexpr int SMEM_BYTES = OFF_BAR + 128;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -119,12 +118,10 @@ struct TileCfg {
 template <int NN, int KV>
 __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
   using Cfg = TileCfg<NN, KV>;
-  constexpr int R = Cfg::R, NT = Cfg::NT;
-  extern __shared__ unsigned char smem_raw[];
-  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  double* sF = reinterpret_cast<double*>(smem + Cfg::OFF_F);
-  double* sN = reinterpret_cast<double*>(smem + Cfg::OFF_N);
-  double* sA = reinterpret_cast<double*>(smem + Cfg::OFF_A);
+  constexpr int R = Cfg::R;
+  extern __shared__ __align__(1024) unsigned char smem[];
+  double* sF = reinterpret_cast<double*>(smem + Cfg::OFF_F);    // stage input tile
+  double* sN = reinterpret_cast<double*>(smem + Cfg::OFF_N);    // f_n tile -> accumulator -> output tile
   double* sXL = reinterpret_cast<double*>(smem + Cfg::OFF_XL);
   double* sXR = reinterpret_cast<double*>(smem + Cfg::OFF_XR);
   double* sUL = reinterpret_cast<double*>(smem + Cfg::OFF_UL);
@@ -145,6 +142,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
   const int gx0 = ex * NN, gu0 = eu * NN, c0 = ev0 * NN;
 
   if (t == 0) {
+    if (smem_u32(smem) & 1023u) __trap();             // the swizzled layout needs the 1024-byte alignment
     mbar_init(bar, 1);
     fence_mbar_init();
     // which upwind halos can be needed at all (signs of the speeds over the tile, Eq. 28)
@@ -169,12 +167,8 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
     if (av_pos) bytes += NN * NN * 2 * 8;
     if (av_neg) bytes += NN * NN * 2 * 8;
     mbar_expect_tx(bar, bytes);
-    if (Cfg::SWZ) {
-      tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
-      tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
-    } else {
-      tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
-    }
+    tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
+    if (Cfg::SWZ) tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
     // Periodic wrap (the paper's roll) by coordinate; zero inflow by letting the box fall
     // outside the tensor, where TMA fills zeros (exterior state 0, reading C2).
     if (ax_pos) tma_load_3d(smem_u32(sXL), &P.m_xface, bar, c0, gu0, (ex > 0) ? gx0 - 1 : (P.bc0 == 0 ? P.G0 - 1 : -1));
@@ -191,39 +185,48 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
       if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
     }
   }
+
+  // Per-thread advection speeds of the three phases (Eq. 28; E = -Phi', reading C15), scaled by the
+  // Jacobian J_d = 2/Delta_d (Eq. 61) and by cr, fetched while the TMA loads are in flight.
+  // out = c0*fn + cf*f + cr*rhs:  plain RHS (mode 0): cf = 0, cr = 1;  RK stage: cf = c1, cr = c1*dt.
+  const double cf = (P.mode != 0) ? P.c1 : 0.0;
+  const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
+  const int xu_hi = t / R, xu_c = t - xu_hi * R;                   // phase x: (ju, c);  phase u: (jx, c)
+  const int v_ju = t % NN, v_ev = (t / NN) % KV, v_jx = t / (KV * NN);
+  const double ax = cr * P.Jx * P.vx[gu0 + xu_hi];                                        // a_x = u
+  const double au = cr * P.Ju * (-(P.E ? P.E[gx0 + xu_hi] : 0.0) - P.omega_c * P.vy[min(c0 + xu_c, P.G2 - 1)]);  // a_u = -E - omega_c v
+  const double av = cr * P.Jv * (P.omega_c * P.vx[gu0 + v_ju]);                           // a_v = omega_c u
+
   __syncthreads();           // barrier init visible to all waiters
   mbar_wait(bar, 0);
 
   // ---------------- phase x: thread = (ju, c), line over jx ----------------
   {
-    const int ju = t / R, c = t - ju * R;
-    const double a = P.Jx * P.vx[gu0 + ju];                       // a_x = u            (Eq. 28)
+    const int ju = xu_hi, c = xu_c;
     double f[NN];
 #pragma unroll
     for (int k = 0; k < NN; ++k) f[k] = sF[Cfg::idx(k * NN + ju, c)];
-    const double uL = (a > 0.0) ? sXL[ju * R + c] : f[0];          // upwind states, Eq. 23
-    const double uR = (a < 0.0) ? sXR[ju * R + c] : f[NN - 1];
+    const double uL = (ax > 0.0) ? sXL[ju * R + c] : f[0];         // upwind states, Eq. 23
+    const double uR = (ax < 0.0) ? sXR[ju * R + c] : f[NN - 1];
 #pragma unroll
     for (int j = 0; j < NN; ++j) {
       double s = P.liftL[j] * uL;
       s = fma(-P.liftR[j], uR, s);
 #pragma unroll
       for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
-      sA[Cfg::idx(j * NN + ju, c)] = a * s;
+      const int o = Cfg::idx(j * NN + ju, c);
+      sN[o] = P.has_fn ? fma(P.c0, sN[o], ax * s) : ax * s;
     }
   }
   __syncthreads();
   // ---------------- phase u: thread = (jx, c), line over ju ----------------
   {
-    const int jx = t / R, c = t - jx * R;
-    const double Ex = P.E ? P.E[gx0 + jx] : 0.0;
-    const int gv = min(c0 + c, P.G2 - 1);
-    const double a = P.Ju * (-Ex - P.omega_c * P.vy[gv]);         // a_u = -E - omega_c v  (Eq. 28, E = -Phi')
+    const int jx = xu_hi, c = xu_c;
     double f[NN];
 #pragma unroll
     for (int k = 0; k < NN; ++k) f[k] = sF[Cfg::idx(jx * NN + k, c)];
-    const double uL = (a > 0.0) ? sUL[jx * R + c] : f[0];
-    const double uR = (a < 0.0) ? sUR[jx * R + c] : f[NN - 1];
+    const double uL = (au > 0.0) ? sUL[jx * R + c] : f[0];
+    const double uR = (au < 0.0) ? sUR[jx * R + c] : f[NN - 1];
 #pragma unroll
     for (int j = 0; j < NN; ++j) {
       double s = P.liftL[j] * uL;
@@ -231,7 +234,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
 #pragma unroll
       for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
       const int o = Cfg::idx(jx * NN + j, c);
-      sA[o] = fma(a, s, sA[o]);
+      sN[o] = fma(au, s, sN[o]);
     }
   }
   __syncthreads();
@@ -239,53 +242,37 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
   {
     // ju fastest: the 8 lanes of a quarter warp read 8 different rows at the same c, which the swizzle
     // spreads over all banks
-    const int ju = t % NN, ev = (t / NN) % KV, jx = t / (KV * NN);
+    const int ju = v_ju, ev = v_ev, jx = v_jx;
     double psum = 0.0;
     if (ev < kvalid) {
       const int row = jx * NN + ju;
       const int cl = ev * NN;
-      const double a = P.Jv * (P.omega_c * P.vx[gu0 + ju]);       // a_v = omega_c u     (Eq. 28)
-      double f[NN], acc[NN];
+      double f[NN], outv[NN];
 #pragma unroll
       for (int k = 0; k < NN; k += 2) {
         const double2 v2 = *reinterpret_cast<const double2*>(&sF[Cfg::idx(row, cl + k)]);
         f[k] = v2.x; f[k + 1] = v2.y;
-        const double2 a2 = *reinterpret_cast<const double2*>(&sA[Cfg::idx(row, cl + k)]);
-        acc[k] = a2.x; acc[k + 1] = a2.y;
+        const double2 a2 = *reinterpret_cast<const double2*>(&sN[Cfg::idx(row, cl + k)]);
+        outv[k] = a2.x; outv[k + 1] = a2.y;
       }
       double uL = f[0], uR = f[NN - 1];
-      if (a > 0.0) uL = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
-      if (a < 0.0) uR = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
-      double outv[NN];
+      if (av > 0.0) uL = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
+      if (av < 0.0) uR = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
 #pragma unroll
       for (int j = 0; j < NN; ++j) {
         double s = P.liftL[j] * uL;
         s = fma(-P.liftR[j], uR, s);
 #pragma unroll
         for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
-        const double rhs = fma(a, s, acc[j]);
-        outv[j] = rhs;
-      }
-      if (P.mode != 0) {
-#pragma unroll
-        for (int j = 0; j < NN; ++j) outv[j] = P.c1 * fma(P.dt, outv[j], f[j]);
-        if (P.has_fn) {
-#pragma unroll
-          for (int k = 0; k < NN; k += 2) {
-            const double2 n2 = *reinterpret_cast<const double2*>(&sN[Cfg::idx(row, cl + k)]);
-            outv[k] = fma(P.c0, n2.x, outv[k]);
-            outv[k + 1] = fma(P.c0, n2.y, outv[k + 1]);
-          }
-        }
+        outv[j] = fma(cf, f[j], fma(av, s, outv[j]));
       }
 #pragma unroll
       for (int k = 0; k < NN; k += 2) *reinterpret_cast<double2*>(&sN[Cfg::idx(row, cl + k)]) = make_double2(outv[k], outv[k + 1]);
       if (P.want_partials) {
-        // Eq. 27: LGL quadrature of the stage output over this thread's v line
-        const double* w2 = P.wq2 + c0 + ev * NN;
+        // Eq. 27: LGL quadrature of the stage output over this thread's v line, w_b/J_d weights
 #pragma unroll
-        for (int k = 0; k < NN; ++k) psum = fma(w2[k], outv[k], psum);
-        psum *= P.wq1[gu0 + ju];
+        for (int k = 0; k < NN; ++k) psum = fma(P.wref[k], outv[k], psum);
+        psum *= P.wref[ju] * P.wscale;
       }
     }
     if (P.want_partials) sRed[t] = psum;
@@ -298,7 +285,7 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
     tma_store_commit_and_wait_read();
   }
   if (P.want_partials && t >= 32 && t < 32 + NN) {
-    // fixed-order sum over the (ju, ev) threads of x node jx: deterministic
+    // fixed-order sum over the (ev, ju) threads of x node jx: deterministic
     const int jx = t - 32;
     double s = 0.0;
     for (int i = 0; i < NN * KV; ++i) s += sRed[jx * NN * KV + i];
@@ -372,10 +359,12 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
     for (int k = 0; k < NN; ++k) P.ups[j * NN + k] = b.ups[j * NN + k];
     P.liftL[j] = b.lift[2 * j];
     P.liftR[j] = b.lift[2 * j + 1];
+    P.wref[j] = b.w[j];
   }
-  P.vx = ctx->d_coord[1]; P.vy = ctx->d_coord[2]; P.E = E; P.wq1 = ctx->d_wq[1]; P.wq2 = ctx->d_wq[2];
+  P.vx = ctx->d_coord[1]; P.vy = ctx->d_coord[2]; P.E = E;
   P.partials = ctx->partials;
   P.Jx = ctx->J[0]; P.Ju = ctx->J[1]; P.Jv = ctx->J[2]; P.omega_c = ctx->desc.omega_c;
+  P.wscale = 1.0 / (ctx->J[1] * ctx->J[2]);
   P.c0 = c0; P.c1 = c1; P.dt = dt;
   P.N0 = ctx->N[0]; P.N1 = ctx->N[1]; P.N2 = ctx->N[2]; P.G0 = ctx->G[0]; P.G1 = ctx->G[1]; P.G2 = ctx->G[2];
   P.bc0 = ctx->desc.bc[0]; P.bc1 = ctx->desc.bc[1]; P.bc2 = ctx->desc.bc[2];
