@@ -59,17 +59,25 @@ __device__ __forceinline__ void tma_store_commit_and_wait_read() {
 // ------------------------------------------------------------------------------------------------
 // parameters
 // ------------------------------------------------------------------------------------------------
+// The n x n operator is applied in even-odd form.  Upsilon is centro-antisymmetric
+// (Ups[n-1-j][n-1-k] = -Ups[j][k]) and Xi centro-symmetric (Xi[n-1-j][R] = Xi[j][L]), so with
+// e_k = f_k + f_{n-1-k}, o_k = f_k - f_{n-1-k}, H = n/2:
+//   A_j = sum_{k<H} pe[j][k] e_k + la[j] (uL + uR),   B_j = sum_{k<H} qo[j][k] o_k + lb[j] (uL - uR),
+//   (Ups f - Xi_R uR + Xi_L uL)_j = B_j + A_j,   (...)_{n-1-j} = B_j - A_j,          j < H,
+// pe = (Ups[j][k] + Ups[j][n-1-k])/2, qo = (Ups[j][k] - Ups[j][n-1-k])/2,
+// la = (Xi_L[j] - Xi_R[j])/2, lb = (Xi_L[j] + Xi_R[j])/2: half the multiplies of the dense form.
 template <int NN>
 struct alignas(64) TiledParams {
-  CUtensorMap m_main;    // stage input f_s, box (R, NN, NN)
+  CUtensorMap m_main;    // stage input f_s, box (R or 16, NN, NN)
   CUtensorMap m_xface;   // f_s, box (R, NN, 1)
   CUtensorMap m_uface;   // f_s, box (R, 1, NN)
   CUtensorMap m_vface;   // f_s, box (2, NN, NN)
-  CUtensorMap m_fn;      // f_n, box (R, NN, NN)
-  CUtensorMap m_out;     // output, box (R, NN, NN)
-  double ups[NN * NN];   // reference Upsilon[j][k]   (Eq. 53)
-  double liftL[NN];      // Xi[j][L]                   (Eq. 54)
-  double liftR[NN];      // Xi[j][R]
+  CUtensorMap m_fn;      // f_n, box as m_main
+  CUtensorMap m_out;     // output, box as m_main
+  double pe[NN * NN / 4];
+  double qo[NN * NN / 4];
+  double la[NN / 2];
+  double lb[NN / 2];
   double wref[NN];       // LGL weights on [-1,1]      (Eq. 45)
   const double* vx;      // node coordinates of dim 1 (u = v_x)
   const double* vy;      // node coordinates of dim 2 (v = v_y)
@@ -86,19 +94,20 @@ struct alignas(64) TiledParams {
 template <int NN, int KV>
 struct TileCfg {
   static constexpr int R = KV * NN;                 // row length (doubles)
-  static constexpr int NT = NN * NN * KV;           // threads per CTA
+  static constexpr int H = NN / 2;
+  static constexpr int NT = NN * NN * KV / 2;       // threads per CTA: two lines per thread and phase
   static constexpr int ROWS = NN * NN;
   // 256-byte rows are held as two 128-byte half-rows in TMA SWIZZLE_128B layout (16-byte chunk index
   // XOR row mod 8), which makes the per-line 128-bit accesses of the v phase bank-conflict free.
   static constexpr bool SWZ = (R == 32);
-  static constexpr int a128(int b) { return (b + 1023) / 1024 * 1024; }
-  static constexpr int SZ_MAIN = a128(NN * NN * R * 8);
+  static constexpr int a1k(int b) { return (b + 1023) / 1024 * 1024; }
+  static constexpr int SZ_MAIN = a1k(NN * NN * R * 8);
   // offset (in doubles) of node (row = jx*NN + ju, c) inside a main-tile buffer
   __host__ __device__ static constexpr int idx(int row, int c) {
     return SWZ ? ((c >> 4) * (ROWS * 16) + row * 16 + (((((c & 15) >> 1) ^ (row & 7))) << 1) + (c & 1)) : (row * R + c);
   }
-  static constexpr int SZ_FACE = a128(NN * R * 8);
-  static constexpr int SZ_V = a128(NN * NN * 2 * 8);
+  static constexpr int SZ_FACE = a1k(NN * R * 8);
+  static constexpr int SZ_V = a1k(NN * NN * 2 * 8);
   static constexpr int OFF_F = 0;
   static constexpr int OFF_N = OFF_F + SZ_MAIN;
   static constexpr int OFF_XL = OFF_N + SZ_MAIN;
@@ -108,17 +117,49 @@ struct TileCfg {
   static constexpr int OFF_VL = OFF_UR + SZ_FACE;
   static constexpr int OFF_VR = OFF_VL + SZ_V;
   static constexpr int OFF_RED = OFF_VR + SZ_V;
-  static constexpr int OFF_BAR = OFF_RED + a128(NT * 8);
+  static constexpr int OFF_BAR = OFF_RED + a1k(NT * 8);
   static constexpr int SMEM_BYTES = OFF_BAR + 128;
 };
+
+// Two lines at once (the operator coefficients are fetched once for both):
+// s[l][j] = (Ups f_l - Xi_R uR_l + Xi_L uL_l)_j, reference element (Eq. 14 / 20 / 21).
+template <int NN>
+__device__ __forceinline__ void apply_lines2(const TiledParams<NN>& P, const double (&f)[2][NN], const double (&uL)[2],
+                                             const double (&uR)[2], double (&s)[2][NN]) {
+  constexpr int H = NN / 2;
+  double e[2][H], o[2][H], sp[2], dm[2];
+#pragma unroll
+  for (int l = 0; l < 2; ++l) {
+#pragma unroll
+    for (int k = 0; k < H; ++k) { e[l][k] = f[l][k] + f[l][NN - 1 - k]; o[l][k] = f[l][k] - f[l][NN - 1 - k]; }
+    sp[l] = uL[l] + uR[l];
+    dm[l] = uL[l] - uR[l];
+  }
+#pragma unroll
+  for (int j = 0; j < H; ++j) {
+    double A[2], B[2];
+#pragma unroll
+    for (int l = 0; l < 2; ++l) { A[l] = P.la[j] * sp[l]; B[l] = P.lb[j] * dm[l]; }
+#pragma unroll
+    for (int k = 0; k < H; ++k) {
+#pragma unroll
+      for (int l = 0; l < 2; ++l) {
+        A[l] = fma(P.pe[j * H + k], e[l][k], A[l]);
+        B[l] = fma(P.qo[j * H + k], o[l][k], B[l]);
+      }
+    }
+#pragma unroll
+    for (int l = 0; l < 2; ++l) { s[l][j] = B[l] + A[l]; s[l][NN - 1 - j] = B[l] - A[l]; }
+  }
+}
 
 // ------------------------------------------------------------------------------------------------
 // kernel
 // ------------------------------------------------------------------------------------------------
 template <int NN, int KV>
-__global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
+__global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
   using Cfg = TileCfg<NN, KV>;
-  constexpr int R = Cfg::R;
+  constexpr int R = Cfg::R, H = Cfg::H, RP = R / 2;
   extern __shared__ __align__(1024) unsigned char smem[];
   double* sF = reinterpret_cast<double*>(smem + Cfg::OFF_F);    // stage input tile
   double* sN = reinterpret_cast<double*>(smem + Cfg::OFF_N);    // f_n tile -> accumulator -> output tile
@@ -191,88 +232,111 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
   // out = c0*fn + cf*f + cr*rhs:  plain RHS (mode 0): cf = 0, cr = 1;  RK stage: cf = c1, cr = c1*dt.
   const double cf = (P.mode != 0) ? P.c1 : 0.0;
   const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
-  const int xu_hi = t / R, xu_c = t - xu_hi * R;                   // phase x: (ju, c);  phase u: (jx, c)
-  const int v_ju = t % NN, v_ev = (t / NN) % KV, v_jx = t / (KV * NN);
-  const double ax = cr * P.Jx * P.vx[gu0 + xu_hi];                                        // a_x = u
-  const double au = cr * P.Ju * (-(P.E ? P.E[gx0 + xu_hi] : 0.0) - P.omega_c * P.vy[min(c0 + xu_c, P.G2 - 1)]);  // a_u = -E - omega_c v
-  const double av = cr * P.Jv * (P.omega_c * P.vx[gu0 + v_ju]);                           // a_v = omega_c u
+  const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
+  const int v_ju = t % H, v_ev = (t / H) % KV, v_jx = t / (KV * H);  // phase v: rows ju and ju + H of (jx, ev)
+  const double ax = cr * P.Jx * P.vx[gu0 + xu_hi];                                         // a_x = u
+  const double Ex = P.E ? P.E[gx0 + xu_hi] : 0.0;
+  double au[2], av[2];
+#pragma unroll
+  for (int l = 0; l < 2; ++l) {
+    au[l] = cr * P.Ju * (-Ex - P.omega_c * P.vy[min(c0 + xu_c + l, P.G2 - 1)]);          // a_u = -E - omega_c v
+    av[l] = cr * P.Jv * (P.omega_c * P.vx[gu0 + v_ju + l * H]);                            // a_v = omega_c u
+  }
 
   __syncthreads();           // barrier init visible to all waiters
   mbar_wait(bar, 0);
 
-  // ---------------- phase x: thread = (ju, c), line over jx ----------------
+  // ---------------- phase x: thread = (ju, c..c+1), lines over jx ----------------
   {
     const int ju = xu_hi, c = xu_c;
-    double f[NN];
+    double f[2][NN], s[2][NN], uL[2], uR[2];
 #pragma unroll
-    for (int k = 0; k < NN; ++k) f[k] = sF[Cfg::idx(k * NN + ju, c)];
-    const double uL = (ax > 0.0) ? sXL[ju * R + c] : f[0];         // upwind states, Eq. 23
-    const double uR = (ax < 0.0) ? sXR[ju * R + c] : f[NN - 1];
-#pragma unroll
-    for (int j = 0; j < NN; ++j) {
-      double s = P.liftL[j] * uL;
-      s = fma(-P.liftR[j], uR, s);
-#pragma unroll
-      for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
-      const int o = Cfg::idx(j * NN + ju, c);
-      sN[o] = P.has_fn ? fma(P.c0, sN[o], ax * s) : ax * s;
+    for (int k = 0; k < NN; ++k) {
+      const double2 v = *reinterpret_cast<const double2*>(&sF[Cfg::idx(k * NN + ju, c)]);
+      f[0][k] = v.x; f[1][k] = v.y;
     }
-  }
-  __syncthreads();
-  // ---------------- phase u: thread = (jx, c), line over ju ----------------
-  {
-    const int jx = xu_hi, c = xu_c;
-    double f[NN];
-#pragma unroll
-    for (int k = 0; k < NN; ++k) f[k] = sF[Cfg::idx(jx * NN + k, c)];
-    const double uL = (au > 0.0) ? sUL[jx * R + c] : f[0];
-    const double uR = (au < 0.0) ? sUR[jx * R + c] : f[NN - 1];
-#pragma unroll
-    for (int j = 0; j < NN; ++j) {
-      double s = P.liftL[j] * uL;
-      s = fma(-P.liftR[j], uR, s);
-#pragma unroll
-      for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
-      const int o = Cfg::idx(jx * NN + j, c);
-      sN[o] = fma(au, s, sN[o]);
-    }
-  }
-  __syncthreads();
-  // ---------------- phase v: thread = (jx, ju, ev), line over the v nodes of element ev ----------------
-  {
-    // ju fastest: the 8 lanes of a quarter warp read 8 different rows at the same c, which the swizzle
-    // spreads over all banks
-    const int ju = v_ju, ev = v_ev, jx = v_jx;
-    double psum = 0.0;
-    if (ev < kvalid) {
-      const int row = jx * NN + ju;
-      const int cl = ev * NN;
-      double f[NN], outv[NN];
-#pragma unroll
-      for (int k = 0; k < NN; k += 2) {
-        const double2 v2 = *reinterpret_cast<const double2*>(&sF[Cfg::idx(row, cl + k)]);
-        f[k] = v2.x; f[k + 1] = v2.y;
-        const double2 a2 = *reinterpret_cast<const double2*>(&sN[Cfg::idx(row, cl + k)]);
-        outv[k] = a2.x; outv[k + 1] = a2.y;
-      }
-      double uL = f[0], uR = f[NN - 1];
-      if (av > 0.0) uL = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
-      if (av < 0.0) uR = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
+    // upwind states, Eq. 23
+    if (ax > 0.0) { const double2 v = *reinterpret_cast<const double2*>(&sXL[ju * R + c]); uL[0] = v.x; uL[1] = v.y; }
+    else { uL[0] = f[0][0]; uL[1] = f[1][0]; }
+    if (ax < 0.0) { const double2 v = *reinterpret_cast<const double2*>(&sXR[ju * R + c]); uR[0] = v.x; uR[1] = v.y; }
+    else { uR[0] = f[0][NN - 1]; uR[1] = f[1][NN - 1]; }
+    apply_lines2<NN>(P, f, uL, uR, s);
+    if (P.has_fn) {
 #pragma unroll
       for (int j = 0; j < NN; ++j) {
-        double s = P.liftL[j] * uL;
-        s = fma(-P.liftR[j], uR, s);
-#pragma unroll
-        for (int k = 0; k < NN; ++k) s = fma(P.ups[j * NN + k], f[k], s);
-        outv[j] = fma(cf, f[j], fma(av, s, outv[j]));
+        double2* q = reinterpret_cast<double2*>(&sN[Cfg::idx(j * NN + ju, c)]);
+        const double2 n2 = *q;
+        *q = make_double2(fma(P.c0, n2.x, ax * s[0][j]), fma(P.c0, n2.y, ax * s[1][j]));
       }
+    } else {
 #pragma unroll
-      for (int k = 0; k < NN; k += 2) *reinterpret_cast<double2*>(&sN[Cfg::idx(row, cl + k)]) = make_double2(outv[k], outv[k + 1]);
+      for (int j = 0; j < NN; ++j)
+        *reinterpret_cast<double2*>(&sN[Cfg::idx(j * NN + ju, c)]) = make_double2(ax * s[0][j], ax * s[1][j]);
+    }
+  }
+  __syncthreads();
+  // ---------------- phase u: thread = (jx, c..c+1), lines over ju ----------------
+  {
+    const int jx = xu_hi, c = xu_c;
+    double f[2][NN], s[2][NN], uL[2], uR[2];
+#pragma unroll
+    for (int k = 0; k < NN; ++k) {
+      const double2 v = *reinterpret_cast<const double2*>(&sF[Cfg::idx(jx * NN + k, c)]);
+      f[0][k] = v.x; f[1][k] = v.y;
+    }
+    const double2 hl = *reinterpret_cast<const double2*>(&sUL[jx * R + c]);
+    const double2 hr = *reinterpret_cast<const double2*>(&sUR[jx * R + c]);
+    uL[0] = (au[0] > 0.0) ? hl.x : f[0][0];
+    uL[1] = (au[1] > 0.0) ? hl.y : f[1][0];
+    uR[0] = (au[0] < 0.0) ? hr.x : f[0][NN - 1];
+    uR[1] = (au[1] < 0.0) ? hr.y : f[1][NN - 1];
+    apply_lines2<NN>(P, f, uL, uR, s);
+#pragma unroll
+    for (int j = 0; j < NN; ++j) {
+      double2* q = reinterpret_cast<double2*>(&sN[Cfg::idx(jx * NN + j, c)]);
+      const double2 n2 = *q;
+      *q = make_double2(fma(au[0], s[0][j], n2.x), fma(au[1], s[1][j], n2.y));
+    }
+  }
+  __syncthreads();
+  // ---------------- phase v: thread = (jx, ev, ju and ju + H), lines over the v nodes of element ev ----------------
+  {
+    // ju fastest: the 8 lanes of a quarter warp read rows that the swizzle spreads over all banks
+    const int ev = v_ev, jx = v_jx;
+    double psum = 0.0;
+    if (ev < kvalid) {
+      const int cl = ev * NN;
+      double f[2][NN], s[2][NN], acc[2][NN], uL[2], uR[2];
+#pragma unroll
+      for (int l = 0; l < 2; ++l) {
+        const int row = jx * NN + v_ju + l * H;
+#pragma unroll
+        for (int k = 0; k < NN; k += 2) {
+          const double2 v2 = *reinterpret_cast<const double2*>(&sF[Cfg::idx(row, cl + k)]);
+          f[l][k] = v2.x; f[l][k + 1] = v2.y;
+          const double2 a2 = *reinterpret_cast<const double2*>(&sN[Cfg::idx(row, cl + k)]);
+          acc[l][k] = a2.x; acc[l][k + 1] = a2.y;
+        }
+        uL[l] = f[l][0]; uR[l] = f[l][NN - 1];
+        if (av[l] > 0.0) uL[l] = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
+        if (av[l] < 0.0) uR[l] = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
+      }
+      apply_lines2<NN>(P, f, uL, uR, s);
+#pragma unroll
+      for (int l = 0; l < 2; ++l) {
+        const int row = jx * NN + v_ju + l * H;
+#pragma unroll
+        for (int j = 0; j < NN; ++j) acc[l][j] = fma(cf, f[l][j], fma(av[l], s[l][j], acc[l][j]));
+#pragma unroll
+        for (int k = 0; k < NN; k += 2)
+          *reinterpret_cast<double2*>(&sN[Cfg::idx(row, cl + k)]) = make_double2(acc[l][k], acc[l][k + 1]);
+      }
       if (P.want_partials) {
-        // Eq. 27: LGL quadrature of the stage output over this thread's v line, w_b/J_d weights
+        // Eq. 27: LGL quadrature of the stage output over this thread's two v lines
+        double p0 = 0.0, p1 = 0.0;
 #pragma unroll
-        for (int k = 0; k < NN; ++k) psum = fma(P.wref[k], outv[k], psum);
-        psum *= P.wref[ju] * P.wscale;
+        for (int k = 0; k < NN; ++k) { p0 = fma(P.wref[k], acc[0][k], p0); p1 = fma(P.wref[k], acc[1][k], p1); }
+        psum = (P.wref[v_ju] * p0 + P.wref[v_ju + H] * p1) * P.wscale;
       }
     }
     if (P.want_partials) sRed[t] = psum;
@@ -287,9 +351,9 @@ __global__ void __launch_bounds__(NN * NN * KV) rhs_tiled_kernel(const __grid_co
   if (P.want_partials && t >= 32 && t < 32 + NN) {
     // fixed-order sum over the (ev, ju) threads of x node jx: deterministic
     const int jx = t - 32;
-    double s = 0.0;
-    for (int i = 0; i < NN * KV; ++i) s += sRed[jx * NN * KV + i];
-    P.partials[(size_t)(gx0 + jx) * (P.N1 * P.tiles_v) + (eu * P.tiles_v + tv)] = s;
+    double sum = 0.0;
+    for (int i = 0; i < H * KV; ++i) sum += sRed[jx * H * KV + i];
+    P.partials[(size_t)(gx0 + jx) * (P.N1 * P.tiles_v) + (eu * P.tiles_v + tv)] = sum;
   }
 }
 
@@ -355,12 +419,16 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
       !make_map(&P.m_fn, fn ? fn : f, ctx, RB, NN, NN, Cfg::SWZ) || !make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ))
     return DG_ERR_CUDA;
   const dgsetup::Basis1D& b = ctx->basis[0];
-  for (int j = 0; j < NN; ++j) {
-    for (int k = 0; k < NN; ++k) P.ups[j * NN + k] = b.ups[j * NN + k];
-    P.liftL[j] = b.lift[2 * j];
-    P.liftR[j] = b.lift[2 * j + 1];
-    P.wref[j] = b.w[j];
+  constexpr int H = NN / 2;
+  for (int j = 0; j < H; ++j) {
+    for (int k = 0; k < H; ++k) {
+      P.pe[j * H + k] = 0.5 * (b.ups[j * NN + k] + b.ups[j * NN + NN - 1 - k]);
+      P.qo[j * H + k] = 0.5 * (b.ups[j * NN + k] - b.ups[j * NN + NN - 1 - k]);
+    }
+    P.la[j] = 0.5 * (b.lift[2 * j] - b.lift[2 * j + 1]);
+    P.lb[j] = 0.5 * (b.lift[2 * j] + b.lift[2 * j + 1]);
   }
+  for (int j = 0; j < NN; ++j) P.wref[j] = b.w[j];
   P.vx = ctx->d_coord[1]; P.vy = ctx->d_coord[2]; P.E = E;
   P.partials = ctx->partials;
   P.Jx = ctx->J[0]; P.Ju = ctx->J[1]; P.Jv = ctx->J[2]; P.omega_c = ctx->desc.omega_c;
