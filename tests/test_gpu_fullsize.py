@@ -1,0 +1,128 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times: sampled outputs
+against the pointwise oracle, plus whole-array properties (mass conservation, density, field)."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import vlasov as ov, pointwise as opw, fourier as ofr   # noqa: E402
+import workloads as wl                                               # noqa: E402
+
+K = 0.1
+
+
+def api():
+    from paper_2202_13532_b200 import api as _api
+    return _api
+
+
+def relerr(a, b):
+    return float(np.max(np.abs(np.asarray(a) - np.asarray(b))) / max(np.max(np.abs(b)), 1e-300))
+
+
+def sample_nodes(shape, count, seed):
+    """Random nodes plus every kind of boundary node (first/last element and node of each dimension)."""
+    rng = np.random.default_rng(seed)
+    pts = [tuple(int(rng.integers(0, s)) for s in shape) for _ in range(count)]
+    edge = [0, 1, 7, 8]
+    for d in range(len(shape)):
+        for e in edge + [shape[d] - 1 - q for q in edge]:
+            p = [int(rng.integers(0, s)) for s in shape]
+            p[d] = e % shape[d]
+            pts.append(tuple(p))
+    return pts
+
+
+def test_config3_full_grid_rhs_density_field():
+    """512^3 production grid (config 3): tiled kernel, one RHS with the self-consistent E."""
+    nelem, order = (64, 64, 64), (8, 8, 8)
+    lo, hi = (0.0, -8.5, -8.5), (2 * math.pi / K, 8.5, 8.5)
+    ctx = api().DGContext(nelem, order, lo, hi, bc=(0, 1, 1), omega_c=1.0, pmax=64)
+    g = ov.Grid(nelem=nelem, order=order, lo=lo, hi=hi, bc=(0, 1, 1), omega_c=1.0, pmax=64)
+    f0 = wl.add_uniform_noise(wl.ring_f0(ctx.nodes(0), ctx.nodes(1), ctx.nodes(2), K), wl.SEED_CFG3_NOISE, 1e-4)
+    fd = torch.from_numpy(f0).cuda()
+    # density: whole array against the oracle
+    rho = ctx.density(fd).cpu().numpy()
+    rho_o = ov.density(g, f0)
+    assert relerr(rho, rho_o) <= 1e-13
+    E = ctx.poisson_E(torch.from_numpy(rho_o).cuda()).cpu().numpy()
+    E_o = ofr.poisson_E(lo[0], hi[0], g.x_nodes(), ofr.fourier_project(g.T, rho_o))
+    assert relerr(E, E_o) <= 1e-12
+    out = ctx.rhs(fd, torch.from_numpy(E_o).cuda())
+    assert ctx.last_kernel.startswith("rhs_tiled<8,")
+    out_h = out.cpu().numpy()
+    scale = np.max(np.abs(out_h))
+    for p in sample_nodes(g.flat_shape, 150, 3):
+        ref = opw.rhs_at(g, f0, E_o, p)
+        assert abs(out_h[p] - ref) <= 1e-12 * scale, (p, out_h[p], ref)
+    # property that holds at any size: d(mass)/dt = - outflow through the zero-inflow velocity boundaries
+    W = [np.tile(g.w[d] / g.J[d], g.nelem[d]) for d in range(3)]
+    dm = np.einsum("i,j,k,ijk->", W[0], W[1], W[2], out_h)
+    u, v = g.coords[1].reshape(-1), g.coords[2].reshape(-1)
+    au = -E_o[:, None] - g.omega_c * v[None, :]          # [gx, gv]
+    av = g.omega_c * u                                    # [gu]
+    outflow = (np.einsum("i,k,ik,ik->", W[0], W[2], np.maximum(au, 0), f0[:, -1, :])
+               + np.einsum("i,k,ik,ik->", W[0], W[2], np.maximum(-au, 0), f0[:, 0, :])
+               + np.einsum("i,j,ij->", W[0], W[1] * np.maximum(av, 0), f0[:, :, -1])
+               + np.einsum("i,j,ij->", W[0], W[1] * np.maximum(-av, 0), f0[:, :, 0]))
+    assert abs(dm + outflow) < 1e-9 * max(abs(outflow), 1e-12), (dm, outflow)
+    ctx.close()
+
+
+@pytest.mark.parametrize("n,N", [(8, 50), (4, 100), (6, 67), (10, 40)])
+def test_config4_full_size_rhs_sampled(n, N):
+    """GL-order sweep (config 4) at ~64M DOF: U(0,1) f, N(0,0.1^2) E, sampled against the pointwise oracle."""
+    nelem, order = (N, N, N), (n, n, n)
+    lo, hi = (0.0, -8.5, -8.5), (2 * math.pi / K, 8.5, 8.5)
+    ctx = api().DGContext(nelem, order, lo, hi, bc=(0, 1, 1), omega_c=1.0, workspace=False)
+    g = ov.Grid(nelem=nelem, order=order, lo=lo, hi=hi, bc=(0, 1, 1), omega_c=1.0, pmax=2)
+    f = wl.uniform_field(g.flat_shape, wl.SEED_CFG4_F)
+    E = wl.normal_E(g.flat_shape[0], wl.SEED_CFG4_E)
+    out = ctx.rhs(torch.from_numpy(f).cuda(), torch.from_numpy(E).cuda())
+    assert ctx.last_kernel.startswith("rhs_tiled<%d," % n)
+    out_h = out.cpu().numpy()
+    scale = np.max(np.abs(out_h))
+    for p in sample_nodes(g.flat_shape, 80, n):
+        ref = opw.rhs_at(g, f, E, p)
+        assert abs(out_h[p] - ref) <= 1e-12 * scale, (p, out_h[p], ref)
+    ctx.close()
+
+
+def test_config2_grid_one_full_step():
+    """256^3 (config 2 grid): one self-consistent SSP-RK3 step, whole array against the oracle."""
+    nelem, order = (32, 32, 32), (8, 8, 8)
+    lo, hi = (0.0, -8.5, -8.5), (2 * math.pi / K, 8.5, 8.5)
+    ctx = api().DGContext(nelem, order, lo, hi, bc=(0, 1, 1), omega_c=1.0, pmax=32)
+    g = ov.Grid(nelem=nelem, order=order, lo=lo, hi=hi, bc=(0, 1, 1), omega_c=1.0, pmax=32)
+    f0 = wl.ring_f0(ctx.nodes(0), ctx.nodes(1), ctx.nodes(2), K)
+    fd = torch.from_numpy(f0).cuda()
+    ctx.ssprk3_run(fd, 1e-3, 1, True)
+    fo = ov.ssprk3_step(g, f0, 1e-3)
+    assert relerr(fd.cpu().numpy(), fo) <= 1e-12
+    # literal config-2 time step (dt = 0.005, unstable over 100 steps, C22): 1 step is still a parity case
+    fd = torch.from_numpy(f0).cuda()
+    ctx.ssprk3_run(fd, 5e-3, 1, True)
+    assert relerr(fd.cpu().numpy(), ov.ssprk3_step(g, f0, 5e-3)) <= 1e-12
+    ctx.close()
+
+
+def test_config2_replica_100_steps():
+    """north_star: <= 1e-10 after 100 RK steps. Config-2 physics on a 16^3-element (128^3 DOF) replica."""
+    nelem, order = (16, 16, 16), (8, 8, 8)
+    lo, hi = (0.0, -8.5, -8.5), (2 * math.pi / K, 8.5, 8.5)
+    ctx = api().DGContext(nelem, order, lo, hi, bc=(0, 1, 1), omega_c=1.0, pmax=16)
+    g = ov.Grid(nelem=nelem, order=order, lo=lo, hi=hi, bc=(0, 1, 1), omega_c=1.0, pmax=16)
+    f0 = wl.ring_f0(ctx.nodes(0), ctx.nodes(1), ctx.nodes(2), K)
+    dt = 2e-3
+    assert dt < ctx.max_stable_dt(0.2)
+    fd = torch.from_numpy(f0).cuda()
+    ctx.ssprk3_run(fd, dt, 100, True)
+    fo = f0.copy()
+    for _ in range(100):
+        fo = ov.ssprk3_step(g, fo, dt)
+    assert np.isfinite(fo).all()
+    assert relerr(fd.cpu().numpy(), fo) <= 1e-10
+    ctx.close()
