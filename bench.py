@@ -53,7 +53,7 @@ def make_f0(x, vx, vy, w):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -63,7 +63,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._pump, daemon=True).start()
         except Exception:
@@ -158,30 +158,20 @@ def run_reference(args, w, name):
 # -----------------------------------------------------------------------------------------------
 def run_ours(args, w, name):
     import torch
-    import torch.distributed as dist
-    from paper_2202_13532_b200 import api
+    from paper_2202_13532_b200 import api, dist_util as du
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    _, _, local = du.env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the DG kernels have no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    world, rank = du.init("nccl", dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        du.barrier(dev)
 
     def max_over_ranks(v):
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return du.max_over_ranks(v, dev)
 
     ga = grid_args(w)
     ctx = api.DGContext(device=local, **ga)
@@ -206,8 +196,8 @@ def run_ours(args, w, name):
     ms = max_over_ranks(e0.elapsed_time(e1))
     clocks = sampler.stop() if rank == 0 else None
     launches = ctx.launch_count - l0
-    finite = bool(torch.isfinite(f).all().item())
-    value = world * dof * 3.0 * args.steps / (ms * 1e-3)
+    finite = du.all_ranks_true(bool(torch.isfinite(f).all().item()), dev)
+    value = du.replica_throughput(dof, 3, args.steps, ms, world)
 
     # roofline of the dominant kernel (fused RHS + stage): per-launch events inside the library
     ctx.set_option(api.OPT_PROFILE, 1)
@@ -257,8 +247,7 @@ def run_ours(args, w, name):
         }
         print(json.dumps(line), flush=True)
     ctx.close()
-    if world > 1:
-        dist.destroy_process_group()
+    du.finalize()
 
 
 def main():
