@@ -250,16 +250,109 @@ def run_ours(args, w, name):
     du.finalize()
 
 
+# -----------------------------------------------------------------------------------------------
+# secondary workloads (BASELINE.json configs[3], configs[4]); not the driver's default line
+# -----------------------------------------------------------------------------------------------
+CONFIG4 = {"config4_rhs_n4": (4, 100), "config4_rhs_n6": (6, 67), "config4_rhs_n8": (8, 50), "config4_rhs_n10": (10, 40)}
+FP64_ALU_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # DESIGN.md K3: SMs x DFMA/clk/SM x 2 flop x max SM clock
+
+
+def run_config4(args, name):
+    """RHS kernel alone (dg_rhs), seeded U(0,1) f and N(0,0.1^2) E, ~64 M DOF; a 'step' is one evaluation."""
+    import torch
+    import workloads as wl
+    from paper_2202_13532_b200 import api
+    n, N = CONFIG4[name]
+    ctx = api.DGContext((N, N, N), (n, n, n), (0.0, -8.5, -8.5), (2 * math.pi / K_WAVE, 8.5, 8.5), bc=(0, 1, 1), omega_c=1.0,
+                        workspace=False)
+    G = n * N
+    f = torch.from_numpy(wl.uniform_field((G, G, G), wl.SEED_CFG4_F)).cuda()
+    E = torch.from_numpy(wl.normal_E(G, wl.SEED_CFG4_E)).cuda()
+    out = torch.empty_like(f)
+    for _ in range(max(args.warmup, 3)):
+        ctx.rhs(f, E, out)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0); sampler.start()
+    l0 = ctx.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ctx.rhs(f, E, out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    dof = G ** 3
+    peak, peak_src = measured_peak_hbm()
+    achieved = 16.0 * dof * args.steps / (ms * 1e-3) / 1e9
+    print(json.dumps({
+        "metric": "FP64 phase-space DOF-updates/s per RHS evaluation", "value": dof * args.steps / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "order": n, "elements": N, "dof": dof, "l2": "arrays (2 x %.2f GB) larger than L2" % (dof * 8 / 1e9)},
+        "clocks": clocks, "gpu_launches": ctx.launch_count - l0,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "kernel": ctx.last_kernel, "algorithmic_bytes_per_launch": 16.0 * dof, "peak_source": peak_src}}), flush=True)
+    ctx.close()
+
+
+def run_config5(args, name):
+    """DG->Fourier projection + spectral Poisson solve alone: 2048 x 8 x-nodes, batch 4096, modes <= 8192."""
+    import torch
+    import workloads as wl
+    from paper_2202_13532_b200 import api
+    N, n, pmax, batch = 2048, 8, 8192, args.batch
+    t0 = time.perf_counter()
+    ctx = api.DGContext((N,), (n,), (0.0,), (2 * math.pi,), pmax=pmax, field_batch=batch)
+    t_create = time.perf_counter() - t0
+    x = ctx.nodes(0)
+    rho_h, _, _, _ = wl.cosine_sum_density(x, batch, wl.SEED_CFG5)
+    rho = torch.from_numpy(rho_h).cuda()
+    E = torch.empty_like(rho)
+    for _ in range(max(args.warmup, 3)):
+        ctx.poisson_E(rho, E)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0); sampler.start()
+    l0 = ctx.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ctx.poisson_E(rho, E)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    G, Q = N * n, 2 * (pmax + 1)
+    flops = 2.0 * 2.0 * batch * G * Q            # projection + synthesis, 2 flop per multiply-add
+    tf = flops * args.steps / (ms * 1e-3) / 1e12
+    print(json.dumps({
+        "metric": "FP64 TFLOP/s of projection + Poisson synthesis (dense contraction)", "value": tf, "unit": "TFLOP/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "x_nodes": G, "batch": batch, "modes": pmax, "dg_create_s": t_create,
+                   "l2": "T and S (2 x %.2f GB) larger than L2" % (G * Q * 8 / 1e9)},
+        "clocks": clocks, "gpu_launches": ctx.launch_count - l0,
+        "roofline": {"bound": "alu", "achieved": tf, "peak": FP64_ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_ALU_PEAK_TFLOPS,
+                     "traffic": None, "kernel": "field_gemm_tn_kernel",
+                     "peak_source": "148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md K3)"}}), flush=True)
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config3_1d2v_512^3", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="config3_1d2v_512^3", choices=sorted(WORKLOADS) + sorted(CONFIG4) + ["config5_field"])
+    ap.add_argument("--batch", type=int, default=4096, help="config5_field only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.workload in CONFIG4:
+        return run_config4(args, args.workload)
+    if args.workload == "config5_field":
+        return run_config5(args, args.workload)
     w = WORKLOADS[args.workload]
     if args.impl == "reference":
         run_reference(args, w, args.workload)
