@@ -16,6 +16,7 @@ _L = _lib.load()
 OPT_RHS_KERNEL = 1
 OPT_FIELD_KERNEL = 2
 OPT_PROFILE = 3
+OPT_PDL = 4
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 
 

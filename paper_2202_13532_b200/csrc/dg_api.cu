@@ -104,6 +104,12 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   }
   const size_t o_T = off; off = align_up(off + sizeof(double) * T.size(), 256);
   const size_t o_S = off; off = align_up(off + sizeof(double) * S.size(), 256);
+  size_t o_cpart = 0, o_sync = 0;
+  if (desc->ndim >= 2 && dgf::field_fused_supported(ctx->G[0], 2 * ctx->P1)) {
+    dgf::field_fused_shape(ctx->G[0], &ctx->fused_rows, &ctx->fused_grid);
+    o_cpart = off; off = align_up(off + sizeof(double) * (size_t)ctx->fused_grid * 2 * ctx->P1, 256);
+    o_sync = off;  off = align_up(off + 2 * sizeof(unsigned int), 256);
+  }
   cudaError_t e = cudaMalloc(&ctx->dev_block, off);
   if (e != cudaSuccess) { delete ctx; return fail(DG_ERR_CUDA, std::string("dg_create: cudaMalloc: ") + cudaGetErrorString(e)); }
   char* base = (char*)ctx->dev_block;
@@ -122,6 +128,11 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   ctx->d_S = (double*)(base + o_S);
   ok = ok && cudaMemcpy(ctx->d_T, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice) == cudaSuccess;
   ok = ok && cudaMemcpy(ctx->d_S, S.data(), sizeof(double) * S.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+  if (ctx->fused_grid > 0) {
+    ctx->d_cpart = (double*)(base + o_cpart);
+    ctx->d_sync = (unsigned int*)(base + o_sync);
+    ok = ok && cudaMemset(ctx->d_sync, 0, 2 * sizeof(unsigned int)) == cudaSuccess;
+  }
   if (!ok) {
     cudaFree(ctx->dev_block);
     delete ctx;
@@ -240,7 +251,8 @@ static int launch_rhs_inner(dg_ctx* ctx, const double* f, const double* fn, cons
   return launch_rhs_generic(ctx, f, fn, E, out, mode, c0, c1, dt, st);
 }
 
-static int launch_density(dg_ctx* ctx, const double* f, double* rho, double* partial, size_t partial_cap, cudaStream_t st) {
+// Density partials of f: partial[gx][chunk]; returns the chunk count through *nchunks_out.
+static int launch_density_partials(dg_ctx* ctx, const double* f, double* partial, size_t partial_cap, int* nchunks_out, cudaStream_t st) {
   const int G0 = ctx->G[0], G1 = ctx->G[1], G2 = ctx->ndim == 3 ? ctx->G[2] : 1;
   // chunking of the G1 rows of each velocity plane
   int nchunks, rows;
@@ -255,9 +267,15 @@ static int launch_density(dg_ctx* ctx, const double* f, double* rho, double* par
   if ((size_t)nchunks * G0 > partial_cap) return fail(DG_ERR_WORKSPACE, "density partial buffer too small");
   dim3 grid(nchunks, G0);
   dgk::density_partial_kernel<<<grid, 256, 0, st>>>(f, ctx->d_wq[1], ctx->ndim == 3 ? ctx->d_wq[2] : nullptr, G1, G2, rows, partial);
-  int rc = check_launch(ctx, "density_partial_kernel");
+  *nchunks_out = nchunks;
+  return check_launch(ctx, "density_partial_kernel");
+}
+
+static int launch_density(dg_ctx* ctx, const double* f, double* rho, double* partial, size_t partial_cap, cudaStream_t st) {
+  int nchunks = 0;
+  int rc = launch_density_partials(ctx, f, partial, partial_cap, &nchunks, st);
   if (rc) return rc;
-  dgk::density_finish_kernel<<<(G0 + 3) / 4, 128, 0, st>>>(partial, nchunks, G0, rho);
+  dgk::density_finish_kernel<<<(ctx->G[0] + 3) / 4, 128, 0, st>>>(partial, nchunks, ctx->G[0], rho);
   return check_launch(ctx, "density_finish_kernel");
 }
 
@@ -331,6 +349,22 @@ extern "C" int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, d
 
 static int field_from_partials_or_f(dg_ctx* ctx, const double* f, int partial_chunks, cudaStream_t st) {
   int rc;
+  if (ctx->fused_grid > 0 && ctx->opt_field_kernel != 1) {
+    // one launch: finish the density, project, synthesise (field_fused_kernel)
+    bool pdl = ctx->opt_pdl != 0 && !ctx->opt_profile;
+    if (partial_chunks <= 0) {
+      rc = launch_density_partials(ctx, f, ctx->partials, ctx->partials_doubles, &partial_chunks, st);
+      if (rc) return rc;
+      pdl = false;                     // density_partial_kernel does not take part in programmatic launches
+    }
+    dgf::FieldFusedParams P;
+    P.partials = ctx->partials; P.T = ctx->d_T; P.S = ctx->d_S; P.rho = ctx->rho; P.cpart = ctx->d_cpart;
+    P.c = ctx->cbuf; P.E = ctx->E; P.sync = ctx->d_sync;
+    P.nchunks = partial_chunks; P.G0 = ctx->G[0]; P.Q = 2 * ctx->P1; P.rows = ctx->fused_rows;
+    rc = dgf::launch_field_fused(P, ctx->fused_grid, pdl, st);
+    if (rc != DG_OK) return fail(rc, std::string("field_fused_kernel launch failed: ") + cudaGetErrorString(cudaGetLastError()));
+    return check_launch(ctx, "field_fused_kernel");
+  }
   if (partial_chunks > 0) rc = launch_density_finish(ctx, ctx->partials, partial_chunks, ctx->rho, st);
   else rc = launch_density(ctx, f, ctx->rho, ctx->partials, ctx->partials_doubles, st);
   if (rc) return rc;
@@ -456,6 +490,7 @@ extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
   if (key == DG_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
   if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 2) { ctx->opt_field_kernel = (int)value; return DG_OK; }
+  if (key == DG_OPT_PDL && (value == 0 || value == 1)) { ctx->opt_pdl = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg_set_option: unknown key or value");
 }
 

@@ -29,6 +29,10 @@ struct dg_ctx {
   double* d_wq[3] = {nullptr, nullptr, nullptr};     // quadrature weight w_b / J_d per flat node [G_d]
   double* d_T = nullptr;      // [2*P1][G0]   rows 2p / 2p+1 = Re / Im of T_p (Eq. 63)
   double* d_S = nullptr;      // [G0][2*P1]   synthesis rows of Eq. 71 with -1/(i k_p) folded in
+  // one-launch field solve (field_fused_kernel): per-CTA shares of c_q and the rendezvous words
+  double* d_cpart = nullptr;  // [fused_grid][2*P1]
+  unsigned int* d_sync = nullptr;
+  int fused_rows = 0, fused_grid = 0;
 
   // caller-provided workspace
   void* ws = nullptr;
@@ -40,7 +44,7 @@ struct dg_ctx {
   double* f_stage = nullptr;
 
   int64_t launches = 0;
-  int opt_rhs_kernel = 0, opt_field_kernel = 0, opt_profile = 0;
+  int opt_rhs_kernel = 0, opt_field_kernel = 0, opt_profile = 0, opt_pdl = 1;
   std::vector<cudaEvent_t> prof_events;   // (start, stop) pairs around RHS launches in profile mode
   double prof_rhs_ms = 0.0;
   int64_t prof_rhs_launches = 0;

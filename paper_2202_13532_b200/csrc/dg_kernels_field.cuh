@@ -112,4 +112,130 @@ inline int launch_gemm_tn(const double* A, const double* B, double* C, int M, in
   return DG_OK;
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// One-launch field solve of a single density vector (the per-stage solve inside dg_ssprk3_*):
+//   rho[gx] = sum_c partial[gx][c]                    (finish of Eq. 27)
+//   c_q     = sum_gx T[q][gx] rho[gx]                 (Eq. 63)
+//   E[gx]   = sum_q S[gx][q] c_q                      (Eq. 71; Poisson factor folded into S)
+// CTA b owns the x nodes [b*rows, (b+1)*rows): it finishes their densities, forms its share of every
+// c_q, and after a grid-wide rendezvous sums all shares in CTA order (deterministic) and synthesises
+// E at its own nodes.  The grid never exceeds the SM count and each CTA needs few resources, so all
+// CTAs are co-resident and the sense-reversing rendezvous (count, generation) cannot deadlock; it
+// resets itself, so the launch may be replayed.
+// ------------------------------------------------------------------------------------------------
+struct FieldFusedParams {
+  const double* partials;   // [G0][nchunks]
+  const double* T;          // [Q][G0]
+  const double* S;          // [G0][Q]
+  double* rho;              // [G0]
+  double* cpart;            // [grid][Q] scratch
+  double* c;                // [Q]
+  double* E;                // [G0]
+  unsigned int* sync;       // {count, generation}
+  int nchunks, G0, Q, rows;
+};
+
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+__global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams P) {
+  extern __shared__ double fsm[];
+  double* rho_s = fsm;              // [rows]
+  double* c_s = fsm + P.rows;       // [Q]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g0 = blockIdx.x * P.rows;
+  const int nrows = max(0, min(P.rows, P.G0 - g0));
+#if __CUDA_ARCH__ >= 900
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+  // A: densities of the own nodes, one warp per node, fixed order
+  for (int i = warp; i < nrows; i += 8) {
+    const double* pr = P.partials + (size_t)(g0 + i) * P.nchunks;
+    double acc = 0.0;
+#pragma unroll 8
+    for (int cidx = lane; cidx < P.nchunks; cidx += 32) acc += pr[cidx];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
+    if (lane == 0) { rho_s[i] = acc; P.rho[g0 + i] = acc; }
+  }
+  __syncthreads();
+  // B: this CTA's share of c_q
+  for (int q = tid; q < P.Q; q += 256) {
+    const double* tr = P.T + (size_t)q * P.G0 + g0;
+    double acc = 0.0;
+    for (int i = 0; i < nrows; ++i) acc = fma(tr[i], rho_s[i], acc);
+    P.cpart[(size_t)blockIdx.x * P.Q + q] = acc;
+  }
+  // C: grid-wide rendezvous
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) {
+    const unsigned int gen = ld_acquire_u32(P.sync + 1);
+    const unsigned int old = atomicAdd(P.sync, 1u);
+    if (old == gridDim.x - 1) {
+      P.sync[0] = 0u;
+      __threadfence();
+      atomicAdd(P.sync + 1, 1u);
+    } else {
+      const long long t0 = clock64();
+      while (ld_acquire_u32(P.sync + 1) == gen) {
+        if (clock64() - t0 > (1LL << 32)) __trap();      // ~2 s: a lost CTA must not hang the device
+      }
+    }
+    __threadfence();
+  }
+  __syncthreads();
+  // D: c_q = sum of the shares in CTA order
+  for (int q = tid; q < P.Q; q += 256) {
+    double acc = 0.0;
+    for (unsigned int b = 0; b < gridDim.x; ++b) acc += __ldcg(P.cpart + (size_t)b * P.Q + q);
+    c_s[q] = acc;
+    if (blockIdx.x == 0) P.c[q] = acc;
+  }
+  __syncthreads();
+  // E: synthesis at the own nodes, one warp per node
+  for (int i = warp; i < nrows; i += 8) {
+    const double* sr = P.S + (size_t)(g0 + i) * P.Q;
+    double acc = 0.0;
+    for (int q = lane; q < P.Q; q += 32) acc = fma(sr[q], c_s[q], acc);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
+    if (lane == 0) P.E[g0 + i] = acc;
+  }
+}
+
+constexpr int FIELD_FUSED_MAX_GRID = 128;
+
+// rows per CTA and grid of the fused field kernel for G0 x nodes
+inline void field_fused_shape(int G0, int* rows, int* grid) {
+  const int r = (G0 + FIELD_FUSED_MAX_GRID - 1) / FIELD_FUSED_MAX_GRID;
+  *rows = r; *grid = (G0 + r - 1) / r;
+}
+inline size_t field_fused_smem(int rows, int Q) { return sizeof(double) * ((size_t)rows + Q); }
+inline bool field_fused_supported(int G0, int Q) {
+  int rows, grid; field_fused_shape(G0, &rows, &grid);
+  return field_fused_smem(rows, Q) <= 160 * 1024;
+}
+
+inline int launch_field_fused(const FieldFusedParams& P, int grid, bool pdl, cudaStream_t st) {
+  const size_t smem = field_fused_smem(P.rows, P.Q);
+  static size_t smem_set = 0;
+  if (smem > 48 * 1024 && smem > smem_set) {
+    if (cudaFuncSetAttribute(field_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return DG_ERR_CUDA;
+    smem_set = smem;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, field_fused_kernel, P) == cudaSuccess ? DG_OK : DG_ERR_CUDA;
+}
+
 }  // namespace dgf

@@ -100,6 +100,7 @@ struct TileCfg {
   // 256-byte rows are held as two 128-byte half-rows in TMA SWIZZLE_128B layout (16-byte chunk index
   // XOR row mod 8), which makes the per-line 128-bit accesses of the v phase bank-conflict free.
   static constexpr bool SWZ = (R == 32);
+  static constexpr bool SHFL_RED = (NN / 2 * KV == 16);   // density partials by a half-warp butterfly
   static constexpr int a1k(int b) { return (b + 1023) / 1024 * 1024; }
   static constexpr int SZ_MAIN = a1k(NN * NN * R * 8);
   // offset (in doubles) of node (row = jx*NN + ju, c) inside a main-tile buffer
@@ -186,6 +187,27 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
     if (smem_u32(smem) & 1023u) __trap();             // the swizzled layout needs the 1024-byte alignment
     mbar_init(bar, 1);
     fence_mbar_init();
+  }
+  // Thread <-> line maps of the three phases and the E-independent speeds (Eq. 28), scaled by the Jacobian
+  // J_d = 2/Delta_d (Eq. 61) and by cr.  out = c0*fn + cf*f + cr*rhs:  plain RHS (mode 0): cf = 0, cr = 1;
+  // RK stage: cf = c1, cr = c1*dt.  None of this reads what the previous kernel in the stream wrote.
+  const double cf = (P.mode != 0) ? P.c1 : 0.0;
+  const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
+  const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
+  const int v_ju = t % H, v_ev = (t / H) % KV, v_jx = t / (KV * H);  // phase v: rows ju and ju + H of (jx, ev)
+  const double ax = cr * P.Jx * P.vx[gu0 + xu_hi];                                         // a_x = u
+  double au[2], av[2];
+#pragma unroll
+  for (int l = 0; l < 2; ++l) {
+    au[l] = P.omega_c * P.vy[min(c0 + xu_c + l, P.G2 - 1)];
+    av[l] = cr * P.Jv * (P.omega_c * P.vx[gu0 + v_ju + l * H]);                            // a_v = omega_c u
+  }
+  // Programmatic dependent launch: let the next kernel of the stream start its prologue, then wait until the
+  // previous kernel (the field solve that wrote E, and through it the stage that wrote f_s) has completed.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+
+  if (t == 0) {
     // which upwind halos can be needed at all (signs of the speeds over the tile, Eq. 28)
     const double vx_lo = P.vx[gu0], vx_hi = P.vx[gu0 + NN - 1];
     const bool ax_pos = vx_hi > 0.0, ax_neg = vx_lo < 0.0;
@@ -226,22 +248,10 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
       if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
     }
   }
-
-  // Per-thread advection speeds of the three phases (Eq. 28; E = -Phi', reading C15), scaled by the
-  // Jacobian J_d = 2/Delta_d (Eq. 61) and by cr, fetched while the TMA loads are in flight.
-  // out = c0*fn + cf*f + cr*rhs:  plain RHS (mode 0): cf = 0, cr = 1;  RK stage: cf = c1, cr = c1*dt.
-  const double cf = (P.mode != 0) ? P.c1 : 0.0;
-  const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
-  const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
-  const int v_ju = t % H, v_ev = (t / H) % KV, v_jx = t / (KV * H);  // phase v: rows ju and ju + H of (jx, ev)
-  const double ax = cr * P.Jx * P.vx[gu0 + xu_hi];                                         // a_x = u
+  // a_u = -E - omega_c v  (E = -Phi', reading C15), fetched while the TMA loads are in flight
   const double Ex = P.E ? P.E[gx0 + xu_hi] : 0.0;
-  double au[2], av[2];
 #pragma unroll
-  for (int l = 0; l < 2; ++l) {
-    au[l] = cr * P.Ju * (-Ex - P.omega_c * P.vy[min(c0 + xu_c + l, P.G2 - 1)]);          // a_u = -E - omega_c v
-    av[l] = cr * P.Jv * (P.omega_c * P.vx[gu0 + v_ju + l * H]);                            // a_v = omega_c u
-  }
+  for (int l = 0; l < 2; ++l) au[l] = cr * P.Ju * (-Ex - au[l]);
 
   __syncthreads();           // barrier init visible to all waiters
   mbar_wait(bar, 0);
@@ -339,7 +349,16 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
         psum = (P.wref[v_ju] * p0 + P.wref[v_ju + H] * p1) * P.wscale;
       }
     }
-    if (P.want_partials) sRed[t] = psum;
+    if (P.want_partials) {
+      if (Cfg::SHFL_RED) {
+        // the H*KV = 16 threads of x node jx are one aligned half-warp: fixed butterfly, deterministic
+#pragma unroll
+        for (int off = 8; off > 0; off >>= 1) psum += __shfl_xor_sync(0xffffffffu, psum, off);
+        if ((t & 15) == 0) P.partials[(size_t)(gx0 + v_jx) * (P.N1 * P.tiles_v) + (eu * P.tiles_v + tv)] = psum;
+      } else {
+        sRed[t] = psum;
+      }
+    }
   }
   fence_proxy_async();       // generic-proxy writes to sN must be visible to the TMA store
   __syncthreads();
@@ -348,7 +367,7 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
     if (Cfg::SWZ) tma_store_3d(&P.m_out, smem_u32(sN + Cfg::ROWS * 16), c0 + 16, gu0, gx0);
     tma_store_commit_and_wait_read();
   }
-  if (P.want_partials && t >= 32 && t < 32 + NN) {
+  if (!Cfg::SHFL_RED && P.want_partials && t >= 32 && t < 32 + NN) {
     // fixed-order sum over the (ev, ju) threads of x node jx: deterministic
     const int jx = t - 32;
     double sum = 0.0;
@@ -450,7 +469,13 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   }
   const long long tiles = (long long)P.N0 * P.N1 * P.tiles_v;
   if (tiles > 0x7fffffffLL) { g_tiled_err = "too many tiles"; return DG_ERR_UNSUPPORTED; }
-  rhs_tiled_kernel<NN, KV><<<(unsigned)tiles, Cfg::NT, Cfg::SMEM_BYTES, st>>>(P);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)tiles); cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = Cfg::SMEM_BYTES; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = (ctx->opt_pdl && !ctx->opt_profile) ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, rhs_tiled_kernel<NN, KV>, P);
   ctx->last_kernel = "rhs_tiled<" + std::to_string(NN) + "," + std::to_string(KV) + ">";
   return DG_OK;
 }
