@@ -31,6 +31,9 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_expect_tx_noarrive(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
@@ -208,6 +211,15 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
   if (t == 0) {
+    // The tile itself (and f_n) first: their byte count is known, so the transaction count is raised without
+    // arriving, and the loads are in flight while the halo decision below fetches the speeds.
+    mbar_expect_tx_noarrive(bar, (P.has_fn ? 2u : 1u) * (NN * NN * R * 8));
+    tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
+    if (Cfg::SWZ) tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
+    if (P.has_fn) {
+      tma_load_3d(smem_u32(sN), &P.m_fn, bar, c0, gu0, gx0);
+      if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
+    }
     // which upwind halos can be needed at all (signs of the speeds over the tile, Eq. 28)
     const double vx_lo = P.vx[gu0], vx_hi = P.vx[gu0 + NN - 1];
     const bool ax_pos = vx_hi > 0.0, ax_neg = vx_lo < 0.0;
@@ -221,17 +233,14 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
     const double y_lo = -P.omega_c * P.vy[c0], y_hi = -P.omega_c * P.vy[c0 + kvalid * NN - 1];
     const bool au_pos = (-e_min + fmax(y_lo, y_hi)) > 0.0, au_neg = (-e_max + fmin(y_lo, y_hi)) < 0.0;
 
-    uint32_t bytes = NN * NN * R * 8;
-    if (P.has_fn) bytes += NN * NN * R * 8;
+    uint32_t bytes = 0;
     if (ax_pos) bytes += NN * R * 8;
     if (ax_neg) bytes += NN * R * 8;
     if (au_pos) bytes += NN * R * 8;
     if (au_neg) bytes += NN * R * 8;
     if (av_pos) bytes += NN * NN * 2 * 8;
     if (av_neg) bytes += NN * NN * 2 * 8;
-    mbar_expect_tx(bar, bytes);
-    tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
-    if (Cfg::SWZ) tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
+    mbar_expect_tx(bar, bytes);          // the one arrival of this phase, with the halo bytes
     // Periodic wrap (the paper's roll) by coordinate; zero inflow by letting the box fall
     // outside the tensor, where TMA fills zeros (exterior state 0, reading C2).
     if (ax_pos) tma_load_3d(smem_u32(sXL), &P.m_xface, bar, c0, gu0, (ex > 0) ? gx0 - 1 : (P.bc0 == 0 ? P.G0 - 1 : -1));
@@ -242,10 +251,6 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
     if (av_neg) {
       const int cend = c0 + kvalid * NN;
       tma_load_3d(smem_u32(sVR), &P.m_vface, bar, (cend < P.G2) ? cend : (P.bc2 == 0 ? 0 : P.G2), gu0, gx0);
-    }
-    if (P.has_fn) {
-      tma_load_3d(smem_u32(sN), &P.m_fn, bar, c0, gu0, gx0);
-      if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
     }
   }
   // a_u = -E - omega_c v  (E = -Phi', reading C15), fetched while the TMA loads are in flight
