@@ -30,7 +30,7 @@ struct dg_ctx {
   double* d_T = nullptr;      // [2*P1][G0]   rows 2p / 2p+1 = Re / Im of T_p (Eq. 63)
   double* d_S = nullptr;      // [G0][2*P1]   synthesis rows of Eq. 71 with -1/(i k_p) folded in
   // one-launch field solve (field_fused_kernel): per-CTA shares of c_q and the rendezvous words
-  double* d_cpart = nullptr;  // [fused_grid][2*P1]
+  double* d_cpart = nullptr;  // [2*P1][fused_grid]
   unsigned int* d_sync = nullptr;
   int fused_rows = 0, fused_grid = 0;
 

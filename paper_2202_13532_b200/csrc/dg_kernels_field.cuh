@@ -129,7 +129,7 @@ struct FieldFusedParams {
   const double* T;          // [Q][G0]
   const double* S;          // [G0][Q]
   double* rho;              // [G0]
-  double* cpart;            // [grid][Q] scratch
+  double* cpart;            // [Q][grid] scratch (q-major)
   double* c;                // [Q]
   double* E;                // [G0]
   unsigned int* sync;       // {count, generation}
@@ -144,8 +144,9 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
 
 __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams P) {
   extern __shared__ double fsm[];
-  double* rho_s = fsm;              // [rows]
-  double* c_s = fsm + P.rows;       // [Q]
+  double* rho_s = fsm;                  // [rows]
+  double* c_s = fsm + P.rows;           // [Q]
+  double* half_s = c_s + P.Q;           // [2*rows] half-row sums of phase A
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g0 = blockIdx.x * P.rows;
   const int nrows = max(0, min(P.rows, P.G0 - g0));
@@ -153,23 +154,33 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
 #endif
-  // A: densities of the own nodes, one warp per node, fixed order
-  for (int i = warp; i < nrows; i += 8) {
+  // A: densities of the own nodes.  One warp per half row of partials (fixed split, fixed lane stride, fixed
+  // butterfly), sixteen loads in flight per lane; the two halves are added in order: deterministic.
+  const int hsplit = ((P.nchunks + 1) / 2 + 31) / 32 * 32;
+  for (int item = warp; item < 2 * nrows; item += 8) {
+    const int i = item >> 1, h = item & 1;
     const double* pr = P.partials + (size_t)(g0 + i) * P.nchunks;
+    const int c_lo = h ? hsplit : 0, c_hi = h ? P.nchunks : min(hsplit, P.nchunks);
     double acc = 0.0;
-#pragma unroll 8
-    for (int cidx = lane; cidx < P.nchunks; cidx += 32) acc += pr[cidx];
+#pragma unroll 16
+    for (int cidx = c_lo + lane; cidx < c_hi; cidx += 32) acc += __ldcg(pr + cidx);
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
-    if (lane == 0) { rho_s[i] = acc; P.rho[g0 + i] = acc; }
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    if (lane == 0) half_s[item] = acc;
   }
   __syncthreads();
-  // B: this CTA's share of c_q
+  if (tid < nrows) {
+    const double r = half_s[2 * tid] + half_s[2 * tid + 1];
+    rho_s[tid] = r;
+    P.rho[g0 + tid] = r;
+  }
+  __syncthreads();
+  // B: this CTA's share of c_q, stored q-major so that phase D reads along the CTA index
   for (int q = tid; q < P.Q; q += 256) {
     const double* tr = P.T + (size_t)q * P.G0 + g0;
     double acc = 0.0;
     for (int i = 0; i < nrows; ++i) acc = fma(tr[i], rho_s[i], acc);
-    P.cpart[(size_t)blockIdx.x * P.Q + q] = acc;
+    P.cpart[(size_t)q * gridDim.x + blockIdx.x] = acc;
   }
   // C: grid-wide rendezvous
   __threadfence();
@@ -190,21 +201,41 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
     __threadfence();
   }
   __syncthreads();
-  // D: c_q = sum of the shares in CTA order
-  for (int q = tid; q < P.Q; q += 256) {
-    double acc = 0.0;
-    for (unsigned int b = 0; b < gridDim.x; ++b) acc += __ldcg(P.cpart + (size_t)b * P.Q + q);
-    c_s[q] = acc;
-    if (blockIdx.x == 0) P.c[q] = acc;
+  // D: c_q = sum of the shares.  One warp per q, lanes along the CTA index (grid <= 128: at most four loads per
+  // lane, added in order), then a fixed butterfly: the same association in every CTA and every run.
+  const int nb = (int)gridDim.x;
+  for (int q0 = warp * 4; q0 < P.Q; q0 += 32) {
+    double v[4][4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int q = q0 + u;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int b = lane + 32 * j;
+        v[u][j] = (q < P.Q && b < nb) ? __ldcg(P.cpart + (size_t)q * nb + b) : 0.0;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      double acc = ((v[u][0] + v[u][1]) + v[u][2]) + v[u][3];
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+      const int q = q0 + u;
+      if (lane == 0 && q < P.Q) {
+        c_s[q] = acc;
+        if (blockIdx.x == 0) P.c[q] = acc;
+      }
+    }
   }
   __syncthreads();
   // E: synthesis at the own nodes, one warp per node
   for (int i = warp; i < nrows; i += 8) {
     const double* sr = P.S + (size_t)(g0 + i) * P.Q;
     double acc = 0.0;
+#pragma unroll 8
     for (int q = lane; q < P.Q; q += 32) acc = fma(sr[q], c_s[q], acc);
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
     if (lane == 0) P.E[g0 + i] = acc;
   }
 }
@@ -216,7 +247,7 @@ inline void field_fused_shape(int G0, int* rows, int* grid) {
   const int r = (G0 + FIELD_FUSED_MAX_GRID - 1) / FIELD_FUSED_MAX_GRID;
   *rows = r; *grid = (G0 + r - 1) / r;
 }
-inline size_t field_fused_smem(int rows, int Q) { return sizeof(double) * ((size_t)rows + Q); }
+inline size_t field_fused_smem(int rows, int Q) { return sizeof(double) * ((size_t)3 * rows + Q); }
 inline bool field_fused_supported(int G0, int Q) {
   int rows, grid; field_fused_shape(G0, &rows, &grid);
   return field_fused_smem(rows, Q) <= 160 * 1024;
