@@ -256,6 +256,21 @@ static int launch_density_partials(dg_ctx* ctx, const double* f, double* partial
   const int G0 = ctx->G[0], G1 = ctx->G[1], G2 = ctx->ndim == 3 ? ctx->G[2] : 1;
   // chunking of the G1 rows of each velocity plane
   int nchunks, rows;
+  if (G2 > 1 && G2 % 2 == 0 && ((uintptr_t)f & 15) == 0) {
+    // bandwidth-shaped kernel: 256 threads = (256/CP row lanes) x (CP column pairs), 8 rows in flight per thread
+    int CP = 1;
+    while (CP < G2 / 2 && CP < 256) CP *= 2;
+    const int RL = 256 / CP;
+    rows = 32 * RL;
+    while (rows > 8 * RL && (long long)((G1 + rows - 1) / rows) * G0 < 148LL * 16) rows /= 2;
+    nchunks = (G1 + rows - 1) / rows;
+    if ((size_t)nchunks * G0 <= partial_cap) {
+      dim3 grid(nchunks, G0);
+      dgk::density_partial_vec_kernel<8><<<grid, 256, 0, st>>>(f, ctx->d_wq[1], ctx->d_wq[2], G1, G2, rows, CP, partial);
+      *nchunks_out = nchunks;
+      return check_launch(ctx, "density_partial_vec_kernel");
+    }
+  }
   if (G2 == 1) { rows = 4096; nchunks = (G1 + rows - 1) / rows; }
   else {
     int target = (int)((148LL * 8 + G0 - 1) / G0);         // enough CTAs to fill the chip

@@ -118,6 +118,45 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const double* __re
   if (threadIdx.x == 0) partial[(size_t)gx * nchunks + chunk] = tot;
 }
 
+// Same sum for even G2 and a 16-byte aligned f, shaped for HBM bandwidth: thread = (row lane, column pair),
+// 128-bit loads, UNR rows in flight per thread; the weight of the column pair is applied once at the end.
+// CP = column pairs covered per pass (power of two <= 256), 256 / CP row lanes.  Fixed association: deterministic.
+template <int UNR>
+__global__ void __launch_bounds__(256) density_partial_vec_kernel(const double* __restrict__ f, const double* __restrict__ wq1,
+                                                                  const double* __restrict__ wq2, int G1, int G2, int rows_per_chunk,
+                                                                  int CP, double* __restrict__ partial) {
+  __shared__ double red[8];
+  const int gx = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x;
+  const int r0 = chunk * rows_per_chunk;
+  const int r1 = min(G1, r0 + rows_per_chunk);
+  const int ncol2 = G2 >> 1;
+  const int cp0 = threadIdx.x & (CP - 1), rl = threadIdx.x / CP, RL = 256 / CP;
+  const double2* plane = reinterpret_cast<const double2*>(f + (size_t)gx * G1 * G2);
+  double acc = 0.0;
+  for (int cp = cp0; cp < ncol2; cp += CP) {
+    const double2 w2 = *reinterpret_cast<const double2*>(wq2 + 2 * cp);
+    const double2* col = plane + cp;
+    double a0 = 0.0, a1 = 0.0;
+    int r = r0 + rl;
+    for (; r + (UNR - 1) * RL < r1; r += UNR * RL) {
+      double2 v[UNR];
+      double w[UNR];
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) { v[u] = __ldcs(col + (size_t)(r + u * RL) * ncol2); w[u] = wq1[r + u * RL]; }
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) { a0 = fma(w[u], v[u].x, a0); a1 = fma(w[u], v[u].y, a1); }
+    }
+    for (; r < r1; r += RL) {
+      const double2 v = __ldcs(col + (size_t)r * ncol2);
+      const double w = wq1[r];
+      a0 = fma(w, v.x, a0); a1 = fma(w, v.y, a1);
+    }
+    acc = fma(w2.x, a0, fma(w2.y, a1, acc));
+  }
+  const double tot = block_reduce_sum<256>(acc, red);
+  if (threadIdx.x == 0) partial[(size_t)gx * nchunks + chunk] = tot;
+}
+
 // rho[gx] = sum_c partial[gx][c] in index order (deterministic).  One warp per gx.
 __global__ void __launch_bounds__(128) density_finish_kernel(const double* __restrict__ partial, int nchunks, int G0,
                                                              double* __restrict__ rho) {
