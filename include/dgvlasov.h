@@ -114,7 +114,8 @@ double dg_max_stable_dt(const dg_ctx* ctx, double E_bound);
 /* Options and counters. */
 #define DG_OPT_RHS_KERNEL   1   /* 0 auto (tiled when supported), 1 generic, 2 tiled (error if unsupported) */
 #define DG_OPT_FIELD_KERNEL 2   /* 0 auto, 1 simple kernels (also inside dg_ssprk3_*: three launches per stage instead of the
-                                  one-launch field solve), 2 tiled GEMM kernels */
+                                  one-launch field solve), 2 tiled GEMM kernel (FP64 tensor cores, DMMA, when K is even and
+                                  the operands are 16-byte aligned; else the DFMA kernel), 3 tiled DFMA GEMM kernel */
 #define DG_OPT_PROFILE      3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
 #define DG_OPT_PDL          4   /* 1 (default): consecutive kernels of dg_ssprk3_* are chained by programmatic dependent
                                   launch (the next kernel's prologue overlaps the previous kernel's tail); 0: plain launches */

@@ -302,9 +302,9 @@ static int launch_density_finish(dg_ctx* ctx, const double* partial, int nchunks
 static int launch_project(dg_ctx* ctx, const double* rho, int batch, double* c, cudaStream_t st) {
   const int G = ctx->G[0], P1 = ctx->P1;
   const bool big = dgf::gemm_worthwhile(batch, 2 * P1, G);
-  if (ctx->opt_field_kernel == 2 || (ctx->opt_field_kernel == 0 && big)) {
+  if (ctx->opt_field_kernel >= 2 || (ctx->opt_field_kernel == 0 && big)) {
     // C[batch][2*P1] = rho[batch][G] * T[2*P1][G]^T
-    int rc = dgf::launch_gemm_tn(rho, ctx->d_T, c, batch, 2 * P1, G, st);
+    int rc = dgf::launch_gemm_tn(rho, ctx->d_T, c, batch, 2 * P1, G, st, ctx->opt_field_kernel == 3 ? 1 : 0);
     if (rc != DG_OK) return fail(rc, "projection GEMM launch failed");
     return check_launch(ctx, "field_gemm_kernel");
   }
@@ -316,9 +316,9 @@ static int launch_project(dg_ctx* ctx, const double* rho, int batch, double* c, 
 static int launch_synth(dg_ctx* ctx, const double* c, int batch, double* E, cudaStream_t st) {
   const int G = ctx->G[0], Q = 2 * ctx->P1;
   const bool big = dgf::gemm_worthwhile(batch, G, Q);
-  if (ctx->opt_field_kernel == 2 || (ctx->opt_field_kernel == 0 && big)) {
+  if (ctx->opt_field_kernel >= 2 || (ctx->opt_field_kernel == 0 && big)) {
     // E[batch][G] = c[batch][Q] * S[G][Q]^T
-    int rc = dgf::launch_gemm_tn(c, ctx->d_S, E, batch, G, Q, st);
+    int rc = dgf::launch_gemm_tn(c, ctx->d_S, E, batch, G, Q, st, ctx->opt_field_kernel == 3 ? 1 : 0);
     if (rc != DG_OK) return fail(rc, "synthesis GEMM launch failed");
     return check_launch(ctx, "field_gemm_kernel");
   }
@@ -504,7 +504,7 @@ extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_option: null context");
   if (key == DG_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
   if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
-  if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 2) { ctx->opt_field_kernel = (int)value; return DG_OK; }
+  if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 3) { ctx->opt_field_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_PDL && (value == 0 || value == 1)) { ctx->opt_pdl = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg_set_option: unknown key or value");
 }

@@ -103,7 +103,117 @@ __global__ void __launch_bounds__(256) field_gemm_tn_kernel(const double* __rest
   }
 }
 
-inline int launch_gemm_tn(const double* A, const double* B, double* C, int M, int N, int K, cudaStream_t st) {
+// ------------------------------------------------------------------------------------------------
+// Tensor-core form of the same contraction: DMMA (mma.sync m8n8k4 f64, SASS DMMA.8x8x4).  On B200 DMMA has the
+// DFMA peak (37 TFLOP/s measured for both), but one warp instruction carries 256 multiply-adds instead of 32,
+// so operand fetch and issue no longer compete with the arithmetic.  128x128 CTA tile, 8 warps of 64x32,
+// BK = 16, three cp.async stages, rows padded to 20 doubles (fragment loads are bank-conflict free).
+// Needs K even and 16-byte aligned A, B.  The accumulation order over k is fixed: deterministic.
+// ------------------------------------------------------------------------------------------------
+constexpr int TK = 16, TPITCH = 20, TSTAGES = 3;
+constexpr int DMMA_SMEM_BYTES = TSTAGES * 2 * 128 * TPITCH * 8;
+
+__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+
+__global__ void __launch_bounds__(256, 1) field_gemm_dmma_kernel(const double* __restrict__ A, const double* __restrict__ B,
+                                                                 double* __restrict__ C, int M, int N, int K) {
+  extern __shared__ __align__(16) double gsm[];
+  double* As = gsm;                                   // [TSTAGES][128][TPITCH]
+  double* Bs = gsm + TSTAGES * 128 * TPITCH;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g = lane >> 2, tig = lane & 3;
+  const int wm = (warp & 1) * 64, wn = (warp >> 1) * 32;
+  const int tiles_m = (M + 127) / 128;
+  const int bm = (blockIdx.x % tiles_m) * 128, bn = (blockIdx.x / tiles_m) * 128;
+  const uint32_t as_u = (uint32_t)__cvta_generic_to_shared(As), bs_u = (uint32_t)__cvta_generic_to_shared(Bs);
+
+  auto load_stage = [&](int stage, int k0) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int c = tid + i * 256, row = c >> 3, kc = (c & 7) * 2;
+      const int k = k0 + kc;
+      const int kb = (k < K) ? 16 : 0;                // K is even: a 16-byte chunk is inside or outside
+      const int ra = bm + row, rb = bn + row;
+      const double* sa = A + (size_t)min(ra, M - 1) * K + min(k, K - 2);
+      const double* sb = B + (size_t)min(rb, N - 1) * K + min(k, K - 2);
+      const uint32_t off = (uint32_t)((stage * 128 + row) * TPITCH + kc) * 8u;
+      cp_async16_zfill(as_u + off, sa, ra < M ? kb : 0);
+      cp_async16_zfill(bs_u + off, sb, rb < N ? kb : 0);
+    }
+  };
+
+  double acc[8][4][2];
+#pragma unroll
+  for (int i = 0; i < 8; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  const int ktiles = (K + TK - 1) / TK;
+  load_stage(0, 0);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  if (ktiles > 1) load_stage(1, TK);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+
+  for (int kt = 0; kt < ktiles; ++kt) {
+    asm volatile("cp.async.wait_group 1;" ::: "memory");
+    __syncthreads();                                  // stage kt landed; everyone is done with stage kt-1
+    if (kt + 2 < ktiles) load_stage((kt + 2) % TSTAGES, (kt + 2) * TK);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    const double* as = As + (size_t)(kt % TSTAGES) * 128 * TPITCH;
+    const double* bs = Bs + (size_t)(kt % TSTAGES) * 128 * TPITCH;
+#pragma unroll
+    for (int k4 = 0; k4 < TK; k4 += 4) {
+      double a[8], b[4];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) a[i] = as[(wm + i * 8 + g) * TPITCH + k4 + tig];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) b[j] = bs[(wn + j * 8 + g) * TPITCH + k4 + tig];
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                       : "+d"(acc[i][j][0]), "+d"(acc[i][j][1]) : "d"(a[i]), "d"(b[j]));
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+
+  const bool cvec = (N % 2 == 0) && ((reinterpret_cast<uintptr_t>(C) & 15) == 0);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int m = bm + wm + i * 8 + g;
+    if (m >= M) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int nn = bn + wn + j * 8 + 2 * tig;
+      double* dst = C + (size_t)m * N + nn;
+      if (cvec && nn + 1 < N) *reinterpret_cast<double2*>(dst) = make_double2(acc[i][j][0], acc[i][j][1]);
+      else {
+        if (nn < N) dst[0] = acc[i][j][0];
+        if (nn + 1 < N) dst[1] = acc[i][j][1];
+      }
+    }
+  }
+}
+
+// variant: 0 auto (DMMA when the operands allow it), 1 DFMA register-tiled kernel, 2 DMMA (error if not allowed)
+inline int launch_gemm_tn(const double* A, const double* B, double* C, int M, int N, int K, cudaStream_t st, int variant = 0) {
+  const bool dmma_ok = (K % 2 == 0) && K >= 2 && ((reinterpret_cast<uintptr_t>(A) & 15) == 0) && ((reinterpret_cast<uintptr_t>(B) & 15) == 0);
+  if (variant == 2 && !dmma_ok) return DG_ERR_UNSUPPORTED;
+  if (variant != 1 && dmma_ok) {
+    const long long tiles = (long long)((M + 127) / 128) * ((N + 127) / 128);
+    if (tiles <= 0 || tiles > 0x7fffffffLL) return DG_ERR_INVALID_ARG;
+    static bool attr_set = false;
+    if (!attr_set) {
+      if (cudaFuncSetAttribute(field_gemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM_BYTES) != cudaSuccess) return DG_ERR_CUDA;
+      attr_set = true;
+    }
+    field_gemm_dmma_kernel<<<(unsigned)tiles, 256, DMMA_SMEM_BYTES, st>>>(A, B, C, M, N, K);
+    return DG_OK;
+  }
+
   const int tiles_m = (M + BM - 1) / BM, tiles_n = (N + BN - 1) / BN;
   const long long tiles = (long long)tiles_m * tiles_n;
   if (tiles <= 0 || tiles > 0x7fffffffLL) return DG_ERR_INVALID_ARG;

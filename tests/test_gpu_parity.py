@@ -133,7 +133,9 @@ def test_density_matches_oracle(case):
 
 
 @pytest.mark.parametrize("N,n,pmax,batch,kernel", [(16, 4, 16, 1, 0), (32, 8, 32, 3, 1), (64, 8, 100, 40, 2),
-                                                  (37, 6, 51, 33, 2), (64, 8, 64, 1, 2), (9, 5, 7, 130, 0)])
+                                                  (37, 6, 51, 33, 2), (64, 8, 64, 1, 2), (9, 5, 7, 130, 0),
+                                                  (64, 8, 100, 40, 3), (9, 5, 7, 130, 2), (40, 8, 150, 200, 2),
+                                                  (41, 6, 163, 300, 2), (40, 8, 150, 200, 3)])
 def test_project_and_poisson_match_oracle(N, n, pmax, batch, kernel):
     lo, hi = 0.0, 2 * math.pi
     ctx = api().DGContext((N,), (n,), (lo,), (hi,), pmax=pmax, field_batch=batch)
