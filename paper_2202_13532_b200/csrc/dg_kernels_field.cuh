@@ -257,9 +257,19 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
   double* rho_s = fsm;                  // [rows]
   double* c_s = fsm + P.rows;           // [Q]
   double* half_s = c_s + P.Q;           // [2*rows] half-row sums of phase A
+  double* T_s = half_s + 2 * P.rows;    // [Q][rows]  this CTA's columns of T
+  double* S_s = T_s + P.Q * P.rows;     // [rows][Q]  this CTA's rows of S
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g0 = blockIdx.x * P.rows;
   const int nrows = max(0, min(P.rows, P.G0 - g0));
+  // T and S are constants of the context: fetch this CTA's slices before waiting for the previous kernel, so their
+  // DRAM latency (the f arrays streamed through L2 since the last stage) overlaps its tail.
+  for (int e = tid; e < P.Q * nrows; e += 256) {
+    const int q = e / nrows, i = e - q * nrows;
+    T_s[q * P.rows + i] = P.T[(size_t)q * P.G0 + g0 + i];
+    const int i2 = e / P.Q, q2 = e - i2 * P.Q;
+    S_s[i2 * P.Q + q2] = P.S[(size_t)(g0 + i2) * P.Q + q2];
+  }
 #if __CUDA_ARCH__ >= 900
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -287,7 +297,7 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
   __syncthreads();
   // B: this CTA's share of c_q, stored q-major so that phase D reads along the CTA index
   for (int q = tid; q < P.Q; q += 256) {
-    const double* tr = P.T + (size_t)q * P.G0 + g0;
+    const double* tr = T_s + q * P.rows;
     double acc = 0.0;
     for (int i = 0; i < nrows; ++i) acc = fma(tr[i], rho_s[i], acc);
     P.cpart[(size_t)q * gridDim.x + blockIdx.x] = acc;
@@ -311,14 +321,15 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
     __threadfence();
   }
   __syncthreads();
-  // D: c_q = sum of the shares.  One warp per q, lanes along the CTA index (grid <= 128: at most four loads per
-  // lane, added in order), then a fixed butterfly: the same association in every CTA and every run.
+  // D: c_q = sum of the shares.  One warp per q (q = warp, warp + 8, ...), lanes along the CTA index (grid <= 128: at
+  // most four loads per lane, added in order), then a fixed butterfly: the same association in every CTA and every
+  // run.  Eight q per pass: 32 loads in flight per lane.
   const int nb = (int)gridDim.x;
-  for (int q0 = warp * 4; q0 < P.Q; q0 += 32) {
-    double v[4][4];
+  for (int qb = warp; qb < P.Q; qb += 64) {
+    double v[8][4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int q = q0 + u;
+    for (int u = 0; u < 8; ++u) {
+      const int q = qb + 8 * u;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const int b = lane + 32 * j;
@@ -326,11 +337,11 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
       }
     }
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < 8; ++u) {
       double acc = ((v[u][0] + v[u][1]) + v[u][2]) + v[u][3];
 #pragma unroll
       for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-      const int q = q0 + u;
+      const int q = qb + 8 * u;
       if (lane == 0 && q < P.Q) {
         c_s[q] = acc;
         if (blockIdx.x == 0) P.c[q] = acc;
@@ -340,7 +351,7 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
   __syncthreads();
   // E: synthesis at the own nodes, one warp per node
   for (int i = warp; i < nrows; i += 8) {
-    const double* sr = P.S + (size_t)(g0 + i) * P.Q;
+    const double* sr = S_s + i * P.Q;
     double acc = 0.0;
 #pragma unroll 8
     for (int q = lane; q < P.Q; q += 32) acc = fma(sr[q], c_s[q], acc);
@@ -357,7 +368,7 @@ inline void field_fused_shape(int G0, int* rows, int* grid) {
   const int r = (G0 + FIELD_FUSED_MAX_GRID - 1) / FIELD_FUSED_MAX_GRID;
   *rows = r; *grid = (G0 + r - 1) / r;
 }
-inline size_t field_fused_smem(int rows, int Q) { return sizeof(double) * ((size_t)3 * rows + Q); }
+inline size_t field_fused_smem(int rows, int Q) { return sizeof(double) * ((size_t)3 * rows + Q + (size_t)2 * rows * Q); }
 inline bool field_fused_supported(int G0, int Q) {
   int rows, grid; field_fused_shape(G0, &rows, &grid);
   return field_fused_smem(rows, Q) <= 160 * 1024;
