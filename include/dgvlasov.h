@@ -47,7 +47,9 @@ typedef struct {
   double  lo[3];       /* lower bounds; x is [lo,hi) periodic */
   double  hi[3];       /* upper bounds */
   int32_t bc[3];       /* 0 periodic (the paper's roll), 1 zero-inflow
-                          (exterior state 0); bc[0] must be 0 when the Poisson solve is used */
+                          (exterior state 0); bc[0] must be 0 when the Poisson solve is used.
+                          bc[0] = 2 (DG_BC_HALO): this context is an x-slab of a larger grid; the
+                          exterior states at its two x faces come from dg_set_xhalo */
   double  omega_c;     /* = B_ext of Eq. 28; ignored for ndim < 3 */
   int32_t pmax;        /* Fourier modes kept, p = 0..pmax; 0 -> nelem[0] */
   int32_t mass_mode;   /* 0 = the paper's exact LGL mass matrix (Eq. 51/53/54);
@@ -74,6 +76,21 @@ int dg_set_workspace(dg_ctx* ctx, void* ws_dev, size_t bytes);
  *   E_dev    [in]  electric field at the x nodes, [N_x*n_x]; NULL means E = 0
  *   dfdt_dev [out] same shape as f; must not alias f_dev */
 int dg_rhs(dg_ctx* ctx, const double* f_dev, const double* E_dev, double* dfdt_dev, void* stream);
+
+/* x-slab decomposition (one slab of x-elements per GPU, velocity axes whole).  With bc[0] = DG_BC_HALO
+ * the upwind flux of Eq. 23 at the slab's first / last x face takes its exterior
+ * state from halo_dev instead of the paper's roll:
+ *   halo_dev [in] [2][N_u*n_u][N_v*n_v] (ndim = 3) or [2][N_v*n_v] (ndim = 2):
+ *            plane 0 = the left neighbour's LAST x-node plane, plane 1 = the right neighbour's FIRST.
+ * The pointer is kept (caller-owned) and read by every later dg_rhs / dg_rk_stage call. */
+#define DG_BC_HALO 2
+int dg_set_xhalo(dg_ctx* ctx, const double* halo_dev);
+
+/* One Runge-Kutta stage in Shu-Osher form: out = c0 f_n + c1 (f_s + dt L(f_s; E)).
+ *   f_s_dev [in] stage input   f_n_dev [in] step input (NULL when c0 = 0)   E_dev [in] field or NULL
+ *   out_dev [out] may alias f_n_dev (each node is read and written by one thread), not f_s_dev */
+int dg_rk_stage(dg_ctx* ctx, const double* f_s_dev, const double* f_n_dev, const double* E_dev, double* out_dev,
+                double c0, double c1, double dt, void* stream);
 
 /* Shu-Osher SSP-RK3: u1 = u + dt L(u); u2 = 3/4 u + 1/4 (u1 + dt L(u1));
  * u+ = 1/3 u + 2/3 (u2 + dt L(u2)), in place on f_dev.  self_consistent = 1: E is solved from

@@ -18,6 +18,7 @@ OPT_FIELD_KERNEL = 2
 OPT_PROFILE = 3
 OPT_PDL = 4
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
+BC_PERIODIC, BC_ZERO_INFLOW, BC_HALO = 0, 1, 2
 
 
 class DGError(RuntimeError):
@@ -91,6 +92,16 @@ class DGContext:
     def rhs(self, f, E=None, out=None):
         out = torch.empty_like(f) if out is None else out
         _check(_L.dg_rhs(self._h, _ptr(f), _ptr(E), _ptr(out), _stream(self.device)), "dg_rhs")
+        return out
+
+    def set_xhalo(self, halo):
+        """halo: [2][G_u][G_v] exterior x-face planes of an x-slab context (bc[0] = BC_HALO); kept alive here."""
+        self._xhalo = halo
+        _check(_L.dg_set_xhalo(self._h, _ptr(halo)), "dg_set_xhalo")
+
+    def rk_stage(self, f_s, f_n, E, out, c0, c1, dt):
+        _check(_L.dg_rk_stage(self._h, _ptr(f_s), _ptr(f_n), _ptr(E), _ptr(out), float(c0), float(c1), float(dt),
+                              _stream(self.device)), "dg_rk_stage")
         return out
 
     def ssprk3_step(self, f, dt, self_consistent=True):

@@ -48,7 +48,8 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
     if (desc->order[d] < 2 || desc->order[d] > DG_MAX_ORDER)
       return fail(DG_ERR_UNSUPPORTED, "dg_create: order must be 2..10");
     if (!(desc->hi[d] > desc->lo[d])) return fail(DG_ERR_INVALID_ARG, "dg_create: hi must exceed lo");
-    if (desc->bc[d] != 0 && desc->bc[d] != 1) return fail(DG_ERR_INVALID_ARG, "dg_create: bc must be 0 or 1");
+    if (desc->bc[d] != 0 && desc->bc[d] != 1 && !(d == 0 && desc->bc[d] == DG_BC_HALO))
+      return fail(DG_ERR_INVALID_ARG, "dg_create: bc must be 0 or 1 (or DG_BC_HALO for x)");
   }
   if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dg_create: mass_mode must be 0 or 1");
   if (desc->pmax < 0) return fail(DG_ERR_INVALID_ARG, "dg_create: pmax must be >= 0");
@@ -208,6 +209,7 @@ static int launch_rhs_generic(dg_ctx* ctx, const double* f, const double* fn, co
     p.ups[d] = ctx->d_ups[d]; p.lift[d] = ctx->d_lift[d]; p.coord[d] = ctx->d_coord[d]; p.J[d] = ctx->J[d];
   }
   p.omega_c = ctx->desc.omega_c;
+  p.xhalo = ctx->xhalo;
   p.E = E; p.f = f; p.fn = fn; p.out = out; p.c0 = c0; p.c1 = c1; p.dt = dt; p.mode = mode;
   p.dof = (long long)ctx->dof;
   long long blocks = ((long long)ctx->dof + 255) / 256;
@@ -241,6 +243,7 @@ static int launch_rhs(dg_ctx* ctx, const double* f, const double* fn, const doub
 static int launch_rhs_inner(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                             double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
   if (partial_chunks) *partial_chunks = 0;
+  if (ctx->desc.bc[0] == DG_BC_HALO && !ctx->xhalo) return fail(DG_ERR_INVALID_ARG, "bc[0] = DG_BC_HALO needs dg_set_xhalo first");
   const bool tiled_ok = dgt::tiled_supported(ctx);
   if (ctx->opt_rhs_kernel == 2 && !tiled_ok) return fail(DG_ERR_UNSUPPORTED, "tiled RHS kernel does not support this grid");
   if (tiled_ok && ctx->opt_rhs_kernel != 1) {
@@ -335,6 +338,23 @@ extern "C" int dg_rhs(dg_ctx* ctx, const double* f_dev, const double* E_dev, dou
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_rhs: field-only context (ndim = 1)");
   if (f_dev == dfdt_dev) return fail(DG_ERR_INVALID_ARG, "dg_rhs: dfdt must not alias f");
   return launch_rhs(ctx, f_dev, nullptr, E_dev, dfdt_dev, 0, 0.0, 1.0, 0.0, false, nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int dg_set_xhalo(dg_ctx* ctx, const double* halo_dev) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_xhalo: null context");
+  if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_set_xhalo: field-only context (ndim = 1)");
+  if (halo_dev && ((uintptr_t)halo_dev & 15)) return fail(DG_ERR_INVALID_ARG, "dg_set_xhalo: pointer must be 16-byte aligned");
+  ctx->xhalo = halo_dev;
+  return DG_OK;
+}
+
+extern "C" int dg_rk_stage(dg_ctx* ctx, const double* f_s_dev, const double* f_n_dev, const double* E_dev, double* out_dev,
+                           double c0, double c1, double dt, void* stream) {
+  if (!ctx || !f_s_dev || !out_dev) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: null argument");
+  if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_rk_stage: field-only context (ndim = 1)");
+  if (f_s_dev == out_dev) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: out must not alias f_s");
+  if (!f_n_dev && c0 != 0.0) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: f_n is needed when c0 != 0");
+  return launch_rhs(ctx, f_s_dev, c0 != 0.0 ? f_n_dev : nullptr, E_dev, out_dev, 1, c0, c1, dt, false, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" int dg_density(dg_ctx* ctx, const double* f_dev, double* rho_dev, void* stream) {

@@ -40,6 +40,8 @@ struct dg_ctx {
   double *u1 = nullptr, *u2 = nullptr, *partials = nullptr, *rho = nullptr, *E = nullptr, *cbuf = nullptr;
   size_t cbuf_doubles = 0, partials_doubles = 0;
 
+  const double* xhalo = nullptr;   // caller-owned exterior x-face planes (bc[0] = DG_BC_HALO)
+
   // library-owned staging for the host entry point
   double* f_stage = nullptr;
 

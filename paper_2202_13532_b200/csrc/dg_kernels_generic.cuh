@@ -16,6 +16,7 @@ struct GenericParams {
   double J[3];
   double omega_c;
   const double* E;          // [G0] or nullptr
+  const double* xhalo;      // exterior x-face planes [2][G1*G2] (bc[0] = 2) or nullptr
   const double* f;          // stage input
   const double* fn;         // f_n for the stage combination (mode 1) or nullptr
   double* out;
@@ -59,10 +60,12 @@ __global__ void __launch_bounds__(256) rhs_generic_kernel(const GenericParams p)
         uR = own1;
         if (e > 0) uL = p.f[base - strd[d]];
         else if (p.bc[d] == 0) uL = p.f[base + ((long long)(N - 1) * n + (n - 1)) * strd[d]];
+        else if (p.bc[d] == 2) uL = p.xhalo[idx % strd[0]];                       // left neighbour's last x plane
       } else if (a[d] < 0.0) {
         uL = own0;
         if (e < N - 1) uR = p.f[base + (long long)n * strd[d]];
         else if (p.bc[d] == 0) uR = p.f[base - (long long)e * n * strd[d]];
+        else if (p.bc[d] == 2) uR = p.xhalo[strd[0] + idx % strd[0]];             // right neighbour's first x plane
       }
       const double xl = p.lift[d][2 * j], xr = p.lift[d][2 * j + 1];
       rhs += (p.J[d] * a[d]) * (vol - xr * uR + xl * uL);

@@ -77,6 +77,7 @@ struct alignas(64) TiledParams {
   CUtensorMap m_vface;   // f_s, box (2, NN, NN)
   CUtensorMap m_fn;      // f_n, box as m_main
   CUtensorMap m_out;     // output, box as m_main
+  CUtensorMap m_xhalo;   // exterior x-face planes [2][G1][G2] of an x-slab (bc0 = 2), box (R, NN, 1)
   double pe[NN * NN / 4];
   double qo[NN * NN / 4];
   double la[NN / 2];
@@ -243,8 +244,15 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
     mbar_expect_tx(bar, bytes);          // the one arrival of this phase, with the halo bytes
     // Periodic wrap (the paper's roll) by coordinate; zero inflow by letting the box fall
     // outside the tensor, where TMA fills zeros (exterior state 0, reading C2).
-    if (ax_pos) tma_load_3d(smem_u32(sXL), &P.m_xface, bar, c0, gu0, (ex > 0) ? gx0 - 1 : (P.bc0 == 0 ? P.G0 - 1 : -1));
-    if (ax_neg) tma_load_3d(smem_u32(sXR), &P.m_xface, bar, c0, gu0, (ex < P.N0 - 1) ? gx0 + NN : (P.bc0 == 0 ? 0 : P.G0));
+    // x-slab of a larger grid (bc0 = 2): the exterior planes at the slab's two x faces come from the halo buffer.
+    if (ax_pos) {
+      if (P.bc0 == 2 && ex == 0) tma_load_3d(smem_u32(sXL), &P.m_xhalo, bar, c0, gu0, 0);
+      else tma_load_3d(smem_u32(sXL), &P.m_xface, bar, c0, gu0, (ex > 0) ? gx0 - 1 : (P.bc0 == 0 ? P.G0 - 1 : -1));
+    }
+    if (ax_neg) {
+      if (P.bc0 == 2 && ex == P.N0 - 1) tma_load_3d(smem_u32(sXR), &P.m_xhalo, bar, c0, gu0, 1);
+      else tma_load_3d(smem_u32(sXR), &P.m_xface, bar, c0, gu0, (ex < P.N0 - 1) ? gx0 + NN : (P.bc0 == 0 ? 0 : P.G0));
+    }
     if (au_pos) tma_load_3d(smem_u32(sUL), &P.m_uface, bar, c0, (eu > 0) ? gu0 - 1 : (P.bc1 == 0 ? P.G1 - 1 : -1), gx0);
     if (au_neg) tma_load_3d(smem_u32(sUR), &P.m_uface, bar, c0, (eu < P.N1 - 1) ? gu0 + NN : (P.bc1 == 0 ? 0 : P.G1), gx0);
     if (av_pos) tma_load_3d(smem_u32(sVL), &P.m_vface, bar, (ev0 > 0) ? c0 - 2 : (P.bc2 == 0 ? P.G2 - 2 : -2), gu0, gx0);
@@ -416,10 +424,11 @@ inline EncodeTiledFn encode_fn() {
   return fn;
 }
 
-inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0, int b1, int b2, bool swz128 = false) {
+inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0, int b1, int b2, bool swz128 = false,
+                     int outer = 0) {
   EncodeTiledFn enc = encode_fn();
   if (!enc) { g_tiled_err = "cuTensorMapEncodeTiled not available"; return false; }
-  const cuuint64_t dims[3] = {(cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)ctx->G[0]};
+  const cuuint64_t dims[3] = {(cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)(outer > 0 ? outer : ctx->G[0])};
   const cuuint64_t strides[2] = {(cuuint64_t)ctx->G[2] * 8, (cuuint64_t)ctx->G[2] * ctx->G[1] * 8};
   const cuuint32_t box[3] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -442,6 +451,12 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
       !make_map(&P.m_uface, f, ctx, R, 1, NN) || !make_map(&P.m_vface, f, ctx, 2, NN, NN) ||
       !make_map(&P.m_fn, fn ? fn : f, ctx, RB, NN, NN, Cfg::SWZ) || !make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ))
     return DG_ERR_CUDA;
+  if (ctx->desc.bc[0] == 2) {
+    if (!ctx->xhalo) { g_tiled_err = "bc[0] = DG_BC_HALO needs dg_set_xhalo first"; return DG_ERR_INVALID_ARG; }
+    if (!make_map(&P.m_xhalo, ctx->xhalo, ctx, R, NN, 1, false, 2)) return DG_ERR_CUDA;
+  } else {
+    P.m_xhalo = P.m_xface;
+  }
   const dgsetup::Basis1D& b = ctx->basis[0];
   constexpr int H = NN / 2;
   for (int j = 0; j < H; ++j) {

@@ -33,3 +33,41 @@ def test_reference_arm_prints_contract_line():
     out = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])
     assert out["impl"] == "reference" and out["cpu_baseline"]["kind"] == "oracle" and out["value"] > 0
     assert out["e2e"]["h2d_bytes_per_step"] == 0 and out["unit"] == "DOF-updates/s"
+
+
+def test_xslab_partition():
+    sys.path.insert(0, ROOT)
+    from paper_2202_13532_b200 import sharded
+    assert sharded.slab_partition(64, 8) == [(8 * r, 8 * r + 8) for r in range(8)]
+    parts = sharded.slab_partition(5, 2)
+    assert parts == [(0, 2), (2, 5)]
+    for N, w in ((7, 3), (64, 5), (3, 3)):
+        p = sharded.slab_partition(N, w)
+        assert p[0][0] == 0 and p[-1][1] == N and all(a[1] == b[0] for a, b in zip(p, p[1:])) and all(b > a for a, b in p)
+    import pytest
+    with pytest.raises(ValueError):
+        sharded.slab_partition(2, 3)
+    lo, hi = sharded.slab_bounds(0.0, 10.0, 5, 2, 5)
+    assert (lo, hi) == (4.0, 10.0)
+
+
+def test_xslab_world1_wraps_through_the_halo_planes():
+    """world = 1: the periodic roll goes through exchange_faces -> halo planes; must equal the unsharded oracle."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import _xslab_worker as xw
+    for sc in (True, False):
+        err, part = xw.run_sharded(0, 1, self_consistent=sc)
+        assert part == (0, 5) and err <= 1e-13, (sc, err)
+    err, _ = xw.run_sharded(0, 1, self_consistent=False, bc0=1)
+    assert err <= 1e-13
+
+
+def test_xslab_two_rank_gloo_matches_unsharded_oracle():
+    """world = 2 over gloo, uneven slabs (2 + 3 x-elements): face-plane exchange + all-gather of rho."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), os.path.join(ROOT, "tests", "_xslab_worker.py")]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-3000:]
+    out = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])
+    assert out["world"] == 2 and out["parts"] == [[0, 2], [2, 5]]
+    assert out["err_sc1_bc0"] <= 1e-13 and out["err_sc0_bc0"] <= 1e-13 and out["err_sc0_bc1"] <= 1e-13, out
