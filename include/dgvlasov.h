@@ -88,9 +88,11 @@ int dg_set_xhalo(dg_ctx* ctx, const double* halo_dev);
 
 /* One Runge-Kutta stage in Shu-Osher form: out = c0 f_n + c1 (f_s + dt L(f_s; E)).
  *   f_s_dev [in] stage input   f_n_dev [in] step input (NULL when c0 = 0)   E_dev [in] field or NULL
- *   out_dev [out] may alias f_n_dev (each node is read and written by one thread), not f_s_dev */
+ *   out_dev [out] may alias f_n_dev (each node is read and written by one thread), not f_s_dev
+ *   rho_out_dev [out, optional] density (Eq. 27) of out_dev at the own x nodes, [N_x*n_x]: finished from the per-tile
+ *           partials of the kernel epilogue (tiled kernel; needs a workspace) instead of another pass over out_dev */
 int dg_rk_stage(dg_ctx* ctx, const double* f_s_dev, const double* f_n_dev, const double* E_dev, double* out_dev,
-                double c0, double c1, double dt, void* stream);
+                double c0, double c1, double dt, double* rho_out_dev, void* stream);
 
 /* Shu-Osher SSP-RK3: u1 = u + dt L(u); u2 = 3/4 u + 1/4 (u1 + dt L(u1));
  * u+ = 1/3 u + 2/3 (u2 + dt L(u2)), in place on f_dev.  self_consistent = 1: E is solved from

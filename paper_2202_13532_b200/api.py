@@ -99,9 +99,9 @@ class DGContext:
         self._xhalo = halo
         _check(_L.dg_set_xhalo(self._h, _ptr(halo)), "dg_set_xhalo")
 
-    def rk_stage(self, f_s, f_n, E, out, c0, c1, dt):
+    def rk_stage(self, f_s, f_n, E, out, c0, c1, dt, rho_out=None):
         _check(_L.dg_rk_stage(self._h, _ptr(f_s), _ptr(f_n), _ptr(E), _ptr(out), float(c0), float(c1), float(dt),
-                              _stream(self.device)), "dg_rk_stage")
+                              _ptr(rho_out), _stream(self.device)), "dg_rk_stage")
         return out
 
     def ssprk3_step(self, f, dt, self_consistent=True):

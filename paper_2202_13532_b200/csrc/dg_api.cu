@@ -349,12 +349,18 @@ extern "C" int dg_set_xhalo(dg_ctx* ctx, const double* halo_dev) {
 }
 
 extern "C" int dg_rk_stage(dg_ctx* ctx, const double* f_s_dev, const double* f_n_dev, const double* E_dev, double* out_dev,
-                           double c0, double c1, double dt, void* stream) {
+                           double c0, double c1, double dt, double* rho_out_dev, void* stream) {
   if (!ctx || !f_s_dev || !out_dev) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: null argument");
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_rk_stage: field-only context (ndim = 1)");
   if (f_s_dev == out_dev) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: out must not alias f_s");
   if (!f_n_dev && c0 != 0.0) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: f_n is needed when c0 != 0");
-  return launch_rhs(ctx, f_s_dev, c0 != 0.0 ? f_n_dev : nullptr, E_dev, out_dev, 1, c0, c1, dt, false, nullptr, (cudaStream_t)stream);
+  if (rho_out_dev && !ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_rk_stage: rho_out needs a workspace (partials live there)");
+  cudaStream_t st = (cudaStream_t)stream;
+  int chunks = 0;
+  int rc = launch_rhs(ctx, f_s_dev, c0 != 0.0 ? f_n_dev : nullptr, E_dev, out_dev, 1, c0, c1, dt, rho_out_dev != nullptr, &chunks, st);
+  if (rc || !rho_out_dev) return rc;
+  if (chunks > 0) return launch_density_finish(ctx, ctx->partials, chunks, rho_out_dev, st);
+  return launch_density(ctx, out_dev, rho_out_dev, ctx->partials, ctx->partials_doubles, st);
 }
 
 extern "C" int dg_density(dg_ctx* ctx, const double* f_dev, double* rho_dev, void* stream) {

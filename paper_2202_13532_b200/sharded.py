@@ -3,7 +3,8 @@
 The phase-space grid is cut into contiguous slabs of x-elements, one per rank; the velocity axes stay
 whole, so the density moment (Eq. 27) is local.  Per Runge-Kutta stage:
 
-  1. rho of the own x nodes                       (dg_density, local)
+  1. rho of the own x nodes                       (dg_density, local -- or, from the second stage of a run on, the
+     density the previous stage's dg_rk_stage finished from its kernel-epilogue partials: no extra pass over f)
   2. all-gather of rho (N_x n_x doubles, 4 KB at 512^3); every rank then solves the same global
      Fourier-series Poisson problem (Eq. 63 / 71) and keeps E at its own nodes --
      bit-identical to the unsharded solve, whatever the number of ranks
@@ -123,8 +124,8 @@ class CudaBackend:
     def set_halo(self, halo):
         self.slab.set_xhalo(halo)
 
-    def rk_stage(self, f_s, f_n, E_loc, out, c0, c1, dt):
-        return self.slab.rk_stage(f_s, f_n, E_loc, out, c0, c1, dt)
+    def rk_stage(self, f_s, f_n, E_loc, out, c0, c1, dt, rho_out=None):
+        return self.slab.rk_stage(f_s, f_n, E_loc, out, c0, c1, dt, rho_out)
 
     def close(self):
         self.slab.close(); self.field.close()
@@ -155,31 +156,35 @@ class XSlabStepper:
         self.E = self.be.empty((self.G0,))
         self.E_loc = self.be.empty((shp[0],))
 
-    def field(self, f_s):
-        """Steps 1-2: E at the own x nodes from the global density."""
-        self.be.density(f_s, self.rho_loc)
+    def field(self, f_s, rho_known=False):
+        """Steps 1-2: E at the own x nodes from the global density.  rho_known: self.rho_loc already holds the density
+        of f_s (written by the previous stage's rk_stage)."""
+        if not rho_known:
+            self.be.density(f_s, self.rho_loc)
         self.comm.all_gather_rho(self.rho_loc, self.counts, self.rho)
         self.be.poisson_E(self.rho, self.E)
         self.E_loc.copy_(self.E[self.g0:self.g1])
         return self.E_loc
 
-    def stage(self, f_s, f_n, out, c0, c1, dt, self_consistent=True):
-        E = self.field(f_s) if self_consistent else None
+    def stage(self, f_s, f_n, out, c0, c1, dt, self_consistent=True, rho_known=False):
+        """One stage; with self_consistent the density of `out` is left in self.rho_loc for the next stage."""
+        E = self.field(f_s, rho_known) if self_consistent else None
         self.comm.exchange_faces(f_s[0], f_s[-1], self.halo, periodic=(self.bc[0] == 0))
-        self.be.rk_stage(f_s, f_n if c0 != 0.0 else None, E, out, c0, c1, dt)
+        self.be.rk_stage(f_s, f_n if c0 != 0.0 else None, E, out, c0, c1, dt, self.rho_loc if self_consistent else None)
         return out
 
-    def step(self, f, dt, self_consistent=True):
-        """u1 = u + dt L(u); u2 = 3/4 u + 1/4 (u1 + dt L(u1)); u <- 1/3 u + 2/3 (u2 + dt L(u2)), in place."""
+    def step(self, f, dt, self_consistent=True, rho_known=False):
+        """u1 = u + dt L(u); u2 = 3/4 u + 1/4 (u1 + dt L(u1)); u <- 1/3 u + 2/3 (u2 + dt L(u2)), in place.
+        rho_known is for run(): a lone step cannot know whether the caller touched f since the last one."""
         (a0, b0), (a1, b1), (a2, b2) = SSPRK3
-        self.stage(f, f, self.u1, a0, b0, dt, self_consistent)
-        self.stage(self.u1, f, self.u2, a1, b1, dt, self_consistent)
-        self.stage(self.u2, f, f, a2, b2, dt, self_consistent)
+        self.stage(f, f, self.u1, a0, b0, dt, self_consistent, rho_known)
+        self.stage(self.u1, f, self.u2, a1, b1, dt, self_consistent, True)
+        self.stage(self.u2, f, f, a2, b2, dt, self_consistent, True)
         return f
 
     def run(self, f, dt, nsteps, self_consistent=True):
-        for _ in range(nsteps):
-            self.step(f, dt, self_consistent)
+        for i in range(nsteps):
+            self.step(f, dt, self_consistent, rho_known=(i > 0))
         return f
 
     def close(self):

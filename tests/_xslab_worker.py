@@ -53,7 +53,7 @@ class OracleSlabBackend:
     def set_halo(self, halo):
         self.halo = halo
 
-    def rk_stage(self, f_s, f_n, E_loc, out, c0, c1, dt):
+    def rk_stage(self, f_s, f_n, E_loc, out, c0, c1, dt, rho_out=None):
         n = self.n
         fs = f_s.numpy()
         h = self.halo.numpy()
@@ -66,6 +66,8 @@ class OracleSlabBackend:
         if f_n is not None and c0 != 0.0:
             res = c0 * f_n.numpy() + res
         out.copy_(torch.from_numpy(res))
+        if rho_out is not None:
+            rho_out.copy_(torch.from_numpy(ov.density(self.slab, res)))
         return out
 
 

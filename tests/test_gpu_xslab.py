@@ -75,6 +75,12 @@ def test_two_slabs_rhs_and_stage_match_unsharded_oracle(case):
         ctx.rk_stage(fs, fns, Es, o2, 0.75, 0.25, 1e-3)
         ref = 0.75 * fn[e0 * n:e1 * n] + 0.25 * (f[e0 * n:e1 * n] + 1e-3 * ro[e0 * n:e1 * n])
         assert relerr(o2.cpu().numpy(), ref) <= 1e-13
+        rho_out = torch.empty(fs.shape[0], dtype=torch.float64, device="cuda")
+        o3 = torch.empty_like(fs)
+        ctx.rk_stage(fs, fns, Es, o3, 0.75, 0.25, 1e-3, rho_out)   # density of `out` from the epilogue partials (S10)
+        assert torch.equal(o3, o2)
+        gs = ov.Grid(nelem=(e1 - e0,) + tuple(nelem[1:]), order=order, lo=lo, hi=hi, bc=bc, omega_c=omega_c)
+        assert relerr(rho_out.cpu().numpy(), ov.density(gs, ref)) <= 1e-13
         ctx.rk_stage(fs, None, None, o2, 0.0, 1.0, 1e-3)      # E = 0, no f_n
         ref0 = f[e0 * n:e1 * n] + 1e-3 * ov.rhs(g, f, None)[e0 * n:e1 * n]
         assert relerr(o2.cpu().numpy(), ref0) <= 1e-13
