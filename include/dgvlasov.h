@@ -118,6 +118,9 @@ int dg_fourier_project(dg_ctx* ctx, const double* rho_dev, int32_t batch, double
  *   rho_dev [in] [batch][N_x*n_x]     E_dev [out] [batch][N_x*n_x]
  * batch > 1 needs workspace room for batch*(pmax+1)*2 doubles (see dg_field_workspace_bytes). */
 int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_dev, void* stream);
+/* Potential instead of field: Phi_mj = sum_{p != 0} -(c_p / k_p^2) e^{i k_p x_mj} (Eq. 70); same
+ * arguments, layout and errors as dg_poisson_E.  E = -dPhi/dx. */
+int dg_poisson_phi(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* phi_dev, void* stream);
 size_t dg_field_workspace_bytes(const dg_ctx* ctx, int32_t batch);
 
 /* Introspection (host outputs; any pointer may be NULL to skip it). */
@@ -134,7 +137,10 @@ double dg_max_stable_dt(const dg_ctx* ctx, double E_bound);
 #define DG_OPT_RHS_KERNEL   1   /* 0 auto (tiled when supported), 1 generic, 2 tiled (error if unsupported) */
 #define DG_OPT_FIELD_KERNEL 2   /* 0 auto, 1 simple kernels (also inside dg_ssprk3_*: three launches per stage instead of the
                                   one-launch field solve), 2 tiled GEMM kernel (FP64 tensor cores, DMMA, when K is even and
-                                  the operands are 16-byte aligned; else the DFMA kernel), 3 tiled DFMA GEMM kernel */
+                                  the operands are 16-byte aligned; else the DFMA kernel), 3 tiled DFMA GEMM kernel,
+                                  4 FFT-factorised kernel (equal-width elements: N_x a power of two, even order; n FFTs of
+                                  length N_x per vector in shared memory + a (pmax+1) x n mode table instead of the dense
+                                  T and S; DG_ERR_UNSUPPORTED otherwise).  auto takes 4 for batched calls when supported. */
 #define DG_OPT_PROFILE      3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
 #define DG_OPT_PDL          4   /* 1 (default): consecutive kernels of dg_ssprk3_* are chained by programmatic dependent
                                   launch (the next kernel's prologue overlaps the previous kernel's tail); 0: plain launches */

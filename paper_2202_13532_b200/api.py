@@ -18,6 +18,7 @@ OPT_FIELD_KERNEL = 2
 OPT_PROFILE = 3
 OPT_PDL = 4
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
+FIELD_AUTO, FIELD_SIMPLE, FIELD_DMMA, FIELD_DFMA, FIELD_FFT = 0, 1, 2, 3, 4
 BC_PERIODIC, BC_ZERO_INFLOW, BC_HALO = 0, 1, 2
 
 
@@ -140,6 +141,13 @@ class DGContext:
         batch = rho2.shape[0]
         out = torch.empty_like(rho2) if out is None else out
         _check(_L.dg_poisson_E(self._h, _ptr(rho2), batch, _ptr(out), _stream(self.device)), "dg_poisson_E")
+        return out.reshape(rho.shape)
+
+    def poisson_phi(self, rho, out=None):
+        rho2 = rho.reshape(-1, self.flat_shape[0])
+        batch = rho2.shape[0]
+        out = torch.empty_like(rho2) if out is None else out
+        _check(_L.dg_poisson_phi(self._h, _ptr(rho2), batch, _ptr(out), _stream(self.device)), "dg_poisson_phi")
         return out.reshape(rho.shape)
 
     # --- introspection ------------------------------------------------------------------------

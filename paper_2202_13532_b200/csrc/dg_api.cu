@@ -12,6 +12,7 @@
 #include "dg_kernels_generic.cuh"
 #include "dg_kernels_tiled.cuh"
 #include "dg_kernels_field.cuh"
+#include "dg_kernels_fft.cuh"
 
 static thread_local std::string g_err;
 
@@ -71,10 +72,15 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   ctx->pmax = desc->pmax > 0 ? desc->pmax : desc->nelem[0];
   ctx->P1 = ctx->pmax + 1;
 
-  std::vector<double> T, S, x;
+  std::vector<double> T, S, x, AD, W;
+  const bool fft_ok = dgfft::fft_supported(ctx->N[0], ctx->n[0]);
+  // Large x-only contexts that the FFT kernel serves build the dense T and S (2 x 2.15 GB at config 5) only when a
+  // dense kernel or dg_get_transform asks for them (ensure_dense).
+  const bool dense_now = !(fft_ok && desc->ndim == 1 && (size_t)2 * ctx->P1 * ctx->G[0] > ((size_t)1 << 22));
   try {
     for (int d = 0; d < desc->ndim; ++d) ctx->basis[d] = dgsetup::make_basis(ctx->n[d], desc->mass_mode);
-    dgsetup::make_fourier(ctx->basis[0], ctx->N[0], desc->lo[0], desc->hi[0], ctx->pmax, T, S, x);
+    dgsetup::make_fourier(ctx->basis[0], ctx->N[0], desc->lo[0], desc->hi[0], ctx->pmax, T, S, x,
+                          fft_ok ? &AD : nullptr, fft_ok ? &W : nullptr, dense_now);
   } catch (const std::exception& e) {
     delete ctx;
     return fail(DG_ERR_INVALID_ARG, std::string("dg_create: setup failed: ") + e.what());
@@ -105,6 +111,8 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   }
   const size_t o_T = off; off = align_up(off + sizeof(double) * T.size(), 256);
   const size_t o_S = off; off = align_up(off + sizeof(double) * S.size(), 256);
+  const size_t o_AD = off; off = align_up(off + sizeof(double) * AD.size(), 256);
+  const size_t o_W = off; off = align_up(off + sizeof(double) * W.size(), 256);
   size_t o_cpart = 0, o_sync = 0;
   if (desc->ndim >= 2 && dgf::field_fused_supported(ctx->G[0], 2 * ctx->P1)) {
     dgf::field_fused_shape(ctx->G[0], &ctx->fused_rows, &ctx->fused_grid);
@@ -125,10 +133,20 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
     ok = ok && cudaMemcpy(ctx->d_coord[d], ctx->coord_h[d].data(), sizeof(double) * ctx->G[d], cudaMemcpyHostToDevice) == cudaSuccess;
     ok = ok && cudaMemcpy(ctx->d_wq[d], wq[d].data(), sizeof(double) * ctx->G[d], cudaMemcpyHostToDevice) == cudaSuccess;
   }
-  ctx->d_T = (double*)(base + o_T);
-  ctx->d_S = (double*)(base + o_S);
-  ok = ok && cudaMemcpy(ctx->d_T, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice) == cudaSuccess;
-  ok = ok && cudaMemcpy(ctx->d_S, S.data(), sizeof(double) * S.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+  if (dense_now) {
+    ctx->d_T = (double*)(base + o_T);
+    ctx->d_S = (double*)(base + o_S);
+  }
+  ok = ok && (!dense_now || cudaMemcpy(ctx->d_T, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice) == cudaSuccess);
+  ok = ok && (!dense_now || cudaMemcpy(ctx->d_S, S.data(), sizeof(double) * S.size(), cudaMemcpyHostToDevice) == cudaSuccess);
+  if (fft_ok) {
+    ctx->d_AD = (double*)(base + o_AD);
+    ctx->d_W = (double*)(base + o_W);
+    ok = ok && cudaMemcpy(ctx->d_AD, AD.data(), sizeof(double) * AD.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = ok && cudaMemcpy(ctx->d_W, W.data(), sizeof(double) * W.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, desc->device) == cudaSuccess && sms > 0) ctx->sm_count = sms;
+  }
   if (ctx->fused_grid > 0) {
     ctx->d_cpart = (double*)(base + o_cpart);
     ctx->d_sync = (unsigned int*)(base + o_sync);
@@ -139,7 +157,7 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
     delete ctx;
     return fail(DG_ERR_CUDA, "dg_create: upload failed");
   }
-  if (T.size() <= (size_t)1 << 22) ctx->T_h.swap(T);     // small tensors stay on the host for introspection
+  if (dense_now && T.size() <= (size_t)1 << 22) ctx->T_h.swap(T);     // small tensors stay on the host for introspection
   *out = ctx;
   return DG_OK;
 }
@@ -147,6 +165,7 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
 extern "C" int dg_destroy(dg_ctx* ctx) {
   if (!ctx) return DG_OK;
   if (ctx->dev_block) cudaFree(ctx->dev_block);
+  if (ctx->dense_block) cudaFree(ctx->dense_block);
   if (ctx->f_stage) cudaFree(ctx->f_stage);
   for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
   delete ctx;
@@ -302,8 +321,60 @@ static int launch_density_finish(dg_ctx* ctx, const double* partial, int nchunks
   return check_launch(ctx, "density_finish_kernel");
 }
 
+// Dense T and S on first use (contexts created without them, see dg_create).
+static int ensure_dense(dg_ctx* ctx) {
+  if (ctx->d_T && ctx->d_S) return DG_OK;
+  std::vector<double> T, S, x;
+  try {
+    dgsetup::make_fourier(ctx->basis[0], ctx->N[0], ctx->desc.lo[0], ctx->desc.hi[0], ctx->pmax, T, S, x);
+  } catch (const std::exception& e) {
+    return fail(DG_ERR_CUDA, std::string("dense transform setup failed: ") + e.what());
+  }
+  const size_t tb = align_up(sizeof(double) * T.size(), 256), sb = sizeof(double) * S.size();
+  CUDA_TRY(cudaMalloc(&ctx->dense_block, tb + sb));
+  double* dT = (double*)ctx->dense_block;
+  double* dS = (double*)((char*)ctx->dense_block + tb);
+  CUDA_TRY(cudaMemcpy(dT, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemcpy(dS, S.data(), sb, cudaMemcpyHostToDevice));
+  ctx->d_T = dT; ctx->d_S = dS;
+  return DG_OK;
+}
+
+// FFT-factorised field solve (dg_kernels_fft.cuh): c and/or E (or Phi) of `batch` density vectors in one launch.
+static bool use_fft(const dg_ctx* ctx, int batch) {
+  if (ctx->opt_field_kernel == 4) return true;
+  return ctx->opt_field_kernel == 0 && ctx->d_AD && (dgf::gemm_worthwhile(batch, 2 * ctx->P1, ctx->G[0]) || batch >= 16);
+}
+
+static int launch_fft(dg_ctx* ctx, const double* rho, int batch, double* c, double* out, int phi, cudaStream_t st) {
+  if (!ctx->d_AD) return fail(DG_ERR_UNSUPPORTED, "FFT field kernel needs a power-of-two element count and an even order that fit shared memory");
+  if (((uintptr_t)rho & 15) || ((uintptr_t)c & 15) || ((uintptr_t)out & 15)) return fail(DG_ERR_INVALID_ARG, "FFT field kernel: arrays must be 16-byte aligned");
+  dgfft::FftParams P;
+  P.rho = rho; P.c = c; P.out = out;
+  P.AD = reinterpret_cast<const double2*>(ctx->d_AD); P.W = reinterpret_cast<const double2*>(ctx->d_W);
+  P.N = ctx->N[0]; P.logN = 0; while ((1 << P.logN) < P.N) ++P.logN;
+  P.P1 = ctx->P1; P.batch = batch; P.phi = phi;
+  P.kinv = (ctx->desc.hi[0] - ctx->desc.lo[0]) / 6.283185307179586476925286766559;
+  int rc = dgfft::launch_fft(P, ctx->n[0], ctx->sm_count, st);
+  if (rc != 0) return fail(DG_ERR_CUDA, "field_fft_kernel launch failed");
+  return check_launch(ctx, "field_fft_kernel");
+}
+
+// Phi~_p = (i/k_p) E~_p: the synthesis matrix S carries the factor of E (Eq. 71), so the potential (Eq. 70) is the
+// same synthesis applied to c_p (i/k_p).
+__global__ void phi_scale_kernel(double* c, long long total, int P1, double kinv) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int p = (int)(i % P1);
+  const double s = p ? kinv / (double)p : 0.0;
+  const double re = c[2 * i], im = c[2 * i + 1];
+  c[2 * i] = -im * s; c[2 * i + 1] = re * s;
+}
+
 static int launch_project(dg_ctx* ctx, const double* rho, int batch, double* c, cudaStream_t st) {
   const int G = ctx->G[0], P1 = ctx->P1;
+  if (use_fft(ctx, batch)) return launch_fft(ctx, rho, batch, c, nullptr, 0, st);
+  if (int rc = ensure_dense(ctx)) return rc;
   const bool big = dgf::gemm_worthwhile(batch, 2 * P1, G);
   if (ctx->opt_field_kernel >= 2 || (ctx->opt_field_kernel == 0 && big)) {
     // C[batch][2*P1] = rho[batch][G] * T[2*P1][G]^T
@@ -318,6 +389,7 @@ static int launch_project(dg_ctx* ctx, const double* rho, int batch, double* c, 
 
 static int launch_synth(dg_ctx* ctx, const double* c, int batch, double* E, cudaStream_t st) {
   const int G = ctx->G[0], Q = 2 * ctx->P1;
+  if (int rc = ensure_dense(ctx)) return rc;
   const bool big = dgf::gemm_worthwhile(batch, G, Q);
   if (ctx->opt_field_kernel >= 2 || (ctx->opt_field_kernel == 0 && big)) {
     // E[batch][G] = c[batch][Q] * S[G][Q]^T
@@ -376,16 +448,33 @@ extern "C" int dg_fourier_project(dg_ctx* ctx, const double* rho_dev, int32_t ba
   return launch_project(ctx, rho_dev, batch, c_dev, (cudaStream_t)stream);
 }
 
-extern "C" int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_dev, void* stream) {
-  if (!ctx || !rho_dev || !E_dev) return fail(DG_ERR_INVALID_ARG, "dg_poisson_E: null argument");
-  if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_poisson_E: batch must be >= 1");
-  if (ctx->desc.bc[0] != 0) return fail(DG_ERR_INVALID_ARG, "dg_poisson_E: x must be periodic");
-  if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_poisson_E: set a workspace first");
+static int poisson_solve(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* out_dev, int phi, void* stream) {
+  if (!ctx || !rho_dev || !out_dev) return fail(DG_ERR_INVALID_ARG, "dg_poisson: null argument");
+  if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_poisson: batch must be >= 1");
+  if (ctx->desc.bc[0] != 0) return fail(DG_ERR_INVALID_ARG, "dg_poisson: x must be periodic");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (use_fft(ctx, batch)) return launch_fft(ctx, rho_dev, batch, nullptr, out_dev, phi, st);   // one launch, no c buffer
+  if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_poisson: set a workspace first");
   if ((size_t)batch * 2 * ctx->P1 > ctx->cbuf_doubles)
-    return fail(DG_ERR_WORKSPACE, "dg_poisson_E: workspace too small for this batch, see dg_field_workspace_bytes");
-  int rc = launch_project(ctx, rho_dev, batch, ctx->cbuf, (cudaStream_t)stream);
+    return fail(DG_ERR_WORKSPACE, "dg_poisson: workspace too small for this batch, see dg_field_workspace_bytes");
+  int rc = launch_project(ctx, rho_dev, batch, ctx->cbuf, st);
   if (rc) return rc;
-  return launch_synth(ctx, ctx->cbuf, batch, E_dev, (cudaStream_t)stream);
+  if (phi) {
+    const long long total = (long long)batch * ctx->P1;
+    phi_scale_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(ctx->cbuf, total, ctx->P1,
+        (ctx->desc.hi[0] - ctx->desc.lo[0]) / 6.283185307179586476925286766559);
+    rc = check_launch(ctx, "phi_scale_kernel");
+    if (rc) return rc;
+  }
+  return launch_synth(ctx, ctx->cbuf, batch, out_dev, st);
+}
+
+extern "C" int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_dev, void* stream) {
+  return poisson_solve(ctx, rho_dev, batch, E_dev, 0, stream);
+}
+
+extern "C" int dg_poisson_phi(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* phi_dev, void* stream) {
+  return poisson_solve(ctx, rho_dev, batch, phi_dev, 1, stream);
 }
 
 static int field_from_partials_or_f(dg_ctx* ctx, const double* f, int partial_chunks, cudaStream_t st) {
@@ -481,6 +570,7 @@ extern "C" int dg_get_transform(const dg_ctx* ctx, int32_t p_first, int32_t p_co
   if (!ctx || !T_host || p_first < 0 || p_count < 0 || p_first + p_count > ctx->P1)
     return fail(DG_ERR_INVALID_ARG, "dg_get_transform: bad argument");
   const int G = ctx->G[0];
+  if (int rc = ensure_dense(const_cast<dg_ctx*>(ctx))) return rc;
   std::vector<double> rows((size_t)2 * p_count * G);
   CUDA_TRY(cudaMemcpy(rows.data(), ctx->d_T + (size_t)2 * p_first * G, sizeof(double) * rows.size(), cudaMemcpyDeviceToHost));
   for (int p = 0; p < p_count; ++p)
@@ -530,7 +620,7 @@ extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_option: null context");
   if (key == DG_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
   if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
-  if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 3) { ctx->opt_field_kernel = (int)value; return DG_OK; }
+  if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 4) { ctx->opt_field_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_PDL && (value == 0 || value == 1)) { ctx->opt_pdl = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg_set_option: unknown key or value");
 }

@@ -29,6 +29,11 @@ struct dg_ctx {
   double* d_wq[3] = {nullptr, nullptr, nullptr};     // quadrature weight w_b / J_d per flat node [G_d]
   double* d_T = nullptr;      // [2*P1][G0]   rows 2p / 2p+1 = Re / Im of T_p (Eq. 63)
   double* d_S = nullptr;      // [G0][2*P1]   synthesis rows of Eq. 71 with -1/(i k_p) folded in
+  void* dense_block = nullptr;  // T and S when built on first use (large x-only contexts served by the FFT kernel)
+  // FFT-factorised field solve (field_fft_kernel): nullptr when the grid does not qualify
+  double* d_AD = nullptr;     // [P1][2][n0] complex: A_p^j, D_p^j
+  double* d_W = nullptr;      // [N0/2] complex twiddles
+  int sm_count = 148;
   // one-launch field solve (field_fused_kernel): per-CTA shares of c_q and the rendezvous words
   double* d_cpart = nullptr;  // [2*P1][fused_grid]
   unsigned int* d_sync = nullptr;

@@ -121,11 +121,15 @@ static void spherical_bessel(int smax, ld z, ld* out) {
 }
 
 void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
-                  std::vector<double>& T, std::vector<double>& S, std::vector<double>& x) {
+                  std::vector<double>& T, std::vector<double>& S, std::vector<double>& x,
+                  std::vector<double>* AD, std::vector<double>* W, bool dense) {
   const int n = b.n, G = nelem * n, P1 = pmax + 1;
   const ld L = (ld)hi - (ld)lo, dx = L / nelem;
-  T.assign((size_t)2 * P1 * G, 0.0);
-  S.assign((size_t)G * 2 * P1, 0.0);
+  T.clear(); S.clear();
+  if (dense) {
+    T.assign((size_t)2 * P1 * G, 0.0);
+    S.assign((size_t)G * 2 * P1, 0.0);
+  }
   x.resize(G);
   std::vector<ld> xi(n), w(n), Ps(n * n);      // Ps[s*n + j] = P_s(xi_j)
   for (int j = 0; j < n; ++j) { xi[j] = b.xi_ld[j]; w[j] = b.w_ld[j]; }
@@ -174,7 +178,7 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
     c = cosl(ang); s = sinl(ang);
   };
 #pragma omp parallel for schedule(static)
-  for (int p = 0; p <= pmax; ++p) {
+  for (int p = 0; p <= (dense ? pmax : -1); ++p) {
     for (int m = 0; m < nelem; ++m) {
       ld c0, s0; mid_phase(p, m, c0, s0);
       // e^{-i k xbar} * (dx/L)
@@ -187,10 +191,41 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
       }
     }
   }
+  // Tables of the FFT-factorised form (dg_kernels_fft.cuh), equal-width elements:
+  //   A_p^j = (1/N) e^{-i phi_p} (node factor of Eq. 63),  D_p^j = (i/k_p) e^{i phi_p} e^{i k_p xi_j dx/2},
+  //   phi_p = k_p lo + pi p / N  (the element-centre phase without its e^{-+2 pi i p m/N} part);  W_k = e^{-2 pi i k/N}.
+  if (AD && W) {
+    AD->assign((size_t)P1 * 2 * n * 2, 0.0);
+    W->assign((size_t)(nelem / 2 > 0 ? nelem / 2 : 1) * 2, 0.0);
+    for (int k = 0; k < nelem / 2; ++k) {
+      (*W)[2 * k] = (double)cosl(2 * PI_L * k / nelem);
+      (*W)[2 * k + 1] = (double)(-sinl(2 * PI_L * k / nelem));
+    }
+#pragma omp parallel for schedule(static)
+    for (int p = 0; p <= pmax; ++p) {
+      const ld kp = 2 * PI_L * p / L;
+      const ld ang = PI_L * (ld)(p % (2 * nelem)) / (ld)nelem;
+      const ld cm = cosl(ang), sm = sinl(ang);
+      const ld cphi = plc[p] * cm - pls[p] * sm, sphi = pls[p] * cm + plc[p] * sm;
+      for (int j = 0; j < n; ++j) {
+        const ld re = nre[(size_t)p * n + j], im = nim[(size_t)p * n + j];
+        double* a = AD->data() + ((size_t)(0 * n + j) * P1 + p) * 2;
+        a[0] = (double)((cphi * re + sphi * im) / nelem);
+        a[1] = (double)((cphi * im - sphi * re) / nelem);
+        if (p > 0) {
+          const ld cj = pjc[(size_t)p * n + j], sj = pjs[(size_t)p * n + j];
+          const ld ar = cphi * cj - sphi * sj, ai = sphi * cj + cphi * sj;      // e^{i phi_p} e^{i k_p xi_j dx/2}
+          double* d = AD->data() + ((size_t)(1 * n + j) * P1 + p) * 2;
+          d[0] = (double)(-ai / kp);                                             // times i / k_p
+          d[1] = (double)(ar / kp);
+        }
+      }
+    }
+  }
   // Synthesis with the Poisson factor folded in (Eq. 71): E = sum_{p>=1} 2 Re( (i c_p / k_p) e^{i k_p x} )
   //   = sum_p (-2/k_p) ( Re c_p sin(k_p x) + Im c_p cos(k_p x) ).
 #pragma omp parallel for schedule(static)
-  for (int m = 0; m < nelem; ++m) {
+  for (int m = 0; m < (dense ? nelem : 0); ++m) {
     for (int p = 1; p <= pmax; ++p) {
       const ld kp = 2 * PI_L * p / L;
       ld c0, s0; mid_phase(p, m, c0, s0);

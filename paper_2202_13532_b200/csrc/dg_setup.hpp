@@ -18,8 +18,12 @@ Basis1D make_basis(int n, int mass_mode);
 // S[g*2*(pmax+1) + 2p + c] : synthesis row of Eq. 71 with the Poisson factor -1/(i k_p) folded in,
 //                     so that E[g] = sum_{p,c} S[g][2p+c] * c_p[c]; columns of p = 0 are zero.
 // x[g]              : node coordinates.
+// dense = false     : T and S are left empty (only x and the tables below are built).
+// AD, W (optional)  : tables of the FFT-factorised form, AD[((t*n + j)*P1 + p)*2 + {re,im}] with t = 0: A_p^j,
+//                     t = 1: D_p^j; W[2k + {re,im}] = e^{-2 pi i k / nelem}, k < nelem/2 (see dg_kernels_fft.cuh).
 void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
-                  std::vector<double>& T, std::vector<double>& S, std::vector<double>& x);
+                  std::vector<double>& T, std::vector<double>& S, std::vector<double>& x,
+                  std::vector<double>* AD = nullptr, std::vector<double>* W = nullptr, bool dense = true);
 
 // Largest a*dt/dx for which SSP-RK3 is stable on the 1-D periodic upwind DG operator built from `b`.
 double rk3_cfl_limit(const Basis1D& b);
