@@ -30,7 +30,7 @@ struct FftParams {
   const double* rho;    // [batch][N*n]
   double* c;            // [batch][P1][2]  (nullptr: not wanted)
   double* out;          // [batch][N*n]    E or Phi (nullptr: projection only)
-  const double2* AD;    // [2][n][P1]      A_p^j then D_p^j, p fastest (lanes walk p: coalesced)
+  const double2* AD;    // [n+1][P1]       rows B_p^j (j < n/2), u_p^j (j < n/2), a_p; p fastest (lanes walk p: coalesced)
   const double2* W;     // [N/2]           e^{-2 pi i k / N}
   int N, logN, P1, batch;
   int phi;              // 1: potential (Eq. 70) instead of field (Eq. 71)
@@ -49,7 +49,7 @@ __host__ __device__ __forceinline__ int phys(int i, int kx) {
   return (i & ~7) | ((x ^ kx) & 7);
 }
 __host__ __device__ inline int arr_stride(int N) { return N < 8 ? 8 : N; }
-inline size_t fft_smem_bytes(int N, int NP) { return sizeof(double2) * ((size_t)NP * arr_stride(N) + N / 2); }
+inline size_t fft_smem_bytes(int N, int NP) { return sizeof(double2) * ((size_t)NP * arr_stride(N) + (N / 2 < 8 ? 8 : N / 2)); }
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
   return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
@@ -81,7 +81,7 @@ __device__ __forceinline__ void fft_pass(double2* z, const double2* Ws, int N, i
       for (int t = 0; t < M; ++t) {
         if (t & half_t) continue;
         const int pos = i0 + ((t & (half_t - 1)) << lh);
-        const double2 w = Ws[pos << shift];
+        const double2 w = Ws[phys(pos << shift, 0)];
         const double2 a = e[t];
         if (!INV) {
           const double2 b = e[t + half_t];
@@ -118,6 +118,12 @@ __device__ __forceinline__ void fft_all(double2* z, const double2* Ws, int N, in
 // Mode combination for bin q (and its mirror N-q unless q is its own mirror): reads the packed spectra at the
 // bit-reversed slots, writes c_p for every kept p = q, N-q (mod N), and leaves the packed Hermitian input of the
 // inverse transform in the same slots.
+//
+// The LGL nodes are symmetric (xi_{n-1-j} = -xi_j, w symmetric), so B_p^{n-1-j} = conj B_p^j and u_p^{n-1-j} =
+// conj u_p^j with  A_p^j = a_p B_p^j,  D_p^j = (i/k_p) conj(N a_p) u_p^j,  a_p = e^{-i(k_p lo + pi p/N)} / N:
+//   s_p = sum_{j<n/2} ( B_p^j X_j + conj(B_p^j) X_{n-1-j} ),   c_p = a_p s_p,
+//   D_p^j c_p = (i / (k_p N)) u_p^j s_p          (|a_p| = 1/N: the centre phase cancels between T and S)
+// i.e. n/2 + n/2 table entries per mode (+ a_p only when c_p itself is wanted) and 4 FMAs per node pair each way.
 template <int NP>
 __device__ __forceinline__ void combine_bin(const FftParams& P, double2* z, int stride, int b, int q) {
   constexpr int n = 2 * NP;
@@ -126,45 +132,72 @@ __device__ __forceinline__ void combine_bin(const FftParams& P, double2* z, int 
   const bool self = (qm == q);
   const int sq = (int)(__brev((unsigned)q) >> (32 - P.logN));
   const int sm = (int)(__brev((unsigned)qm) >> (32 - P.logN));
-  double2 X[n], H[n];
+  // node pair (j, n-1-j), j < NP: sums and differences of X_j[q] and X_{n-1-j}[q]
+  double Sx[NP], Dx[NP], Sy[NP], Dy[NP];
+  {
+    double2 X[n];
 #pragma unroll
-  for (int k = 0; k < NP; ++k) {
-    const double2 a = z[(size_t)k * stride + phys(sq, 2 * k)], m = z[(size_t)k * stride + phys(sm, 2 * k)];
-    X[2 * k] = make_double2(0.5 * (a.x + m.x), 0.5 * (a.y - m.y));          // (Z[q] + conj Z[N-q]) / 2
-    X[2 * k + 1] = make_double2(0.5 * (a.y + m.y), -0.5 * (a.x - m.x));     // (Z[q] - conj Z[N-q]) / (2i)
-    H[2 * k] = make_double2(0.0, 0.0); H[2 * k + 1] = make_double2(0.0, 0.0);
+    for (int k = 0; k < NP; ++k) {
+      const double2 a = z[(size_t)k * stride + phys(sq, 2 * k)], m = z[(size_t)k * stride + phys(sm, 2 * k)];
+      X[2 * k] = make_double2(0.5 * (a.x + m.x), 0.5 * (a.y - m.y));          // (Z[q] + conj Z[N-q]) / 2
+      X[2 * k + 1] = make_double2(0.5 * (a.y + m.y), -0.5 * (a.x - m.x));     // (Z[q] - conj Z[N-q]) / (2i)
+    }
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+      Sx[j] = X[j].x + X[n - 1 - j].x; Dx[j] = X[j].x - X[n - 1 - j].x;
+      Sy[j] = X[j].y + X[n - 1 - j].y; Dy[j] = X[j].y - X[n - 1 - j].y;
+    }
   }
+  // H_j[q] +- H_{n-1-j}[q] accumulate as sums (HS) and differences (HD)
+  double HSx[NP], HSy[NP], HDx[NP], HDy[NP];
+#pragma unroll
+  for (int j = 0; j < NP; ++j) { HSx[j] = 0.0; HSy[j] = 0.0; HDx[j] = 0.0; HDy[j] = 0.0; }
   double2* cb = P.c ? reinterpret_cast<double2*>(P.c) + (size_t)b * P.P1 : nullptr;
+  const double kn = P.kinv / (double)N;
 #pragma unroll 1
   for (int side = 0; side < 2; ++side) {
     if (side == 1 && self) break;
+    const double sg = side ? -1.0 : 1.0;             // side 1: X_j[N-q] = conj X_j[q] (rho is real)
     for (int p = side ? qm : q; p < P.P1; p += N) {
-      const double2* ad = P.AD + p;
-      double2 c = make_double2(0.0, 0.0);
+      const double2* tb = P.AD + p;
+      double sx = 0.0, sy = 0.0;
 #pragma unroll
-      for (int j = 0; j < n; ++j) {
-        const double2 a = __ldg(ad + (size_t)j * P.P1);
-        // side 1: X_j[N-q] = conj X_j[q] (rho is real)
-        const double xr = X[j].x, xi = side ? -X[j].y : X[j].y;
-        c.x = fma(a.x, xr, fma(-a.y, xi, c.x));
-        c.y = fma(a.x, xi, fma(a.y, xr, c.y));
+      for (int j = 0; j < NP; ++j) {
+        const double2 B = __ldg(tb + (size_t)j * P.P1);
+        sx = fma(B.x, Sx[j], fma(-sg * B.y, Dy[j], sx));
+        sy = fma(sg * B.x, Sy[j], fma(B.y, Dx[j], sy));
       }
-      if (cb) cb[p] = c;
+      if (cb) {
+        const double2 a = __ldg(tb + (size_t)n * P.P1);
+        cb[p] = make_double2(fma(a.x, sx, -a.y * sy), fma(a.x, sy, a.y * sx));
+      }
       if (P.out) {
-        if (P.phi) {                       // Phi~_p = E~_p * (i/k_p)  (Eq. 70 vs Eq. 71)
-          const double s = p ? P.kinv / (double)p : 0.0;
-          c = make_double2(-c.y * s, c.x * s);
+        const double f = p ? kn / (double)p : 0.0;
+        double cx = -sy * f, cy = sx * f;            // (i / (k_p N)) s_p
+        if (P.phi) {                                 // Phi~_p = E~_p (i/k_p)  (Eq. 70 vs Eq. 71)
+          const double g = P.kinv / (double)(p ? p : 1);
+          const double t = cx; cx = -cy * g; cy = t * g;
         }
+        cy *= sg;                                    // side 1 contributes conj(Y_j[N-q]) to bin q: u c -> conj(u) conj(c)
+        const double us = sg;
 #pragma unroll
-        for (int j = 0; j < n; ++j) {
-          const double2 d = cmul(__ldg(ad + (size_t)(n + j) * P.P1), c);
-          H[j].x += d.x;
-          H[j].y += side ? -d.y : d.y;     // side 1 contributes conj(Y_j[N-q]) to bin q
+        for (int j = 0; j < NP; ++j) {
+          const double2 u = __ldg(tb + (size_t)(NP + j) * P.P1);
+          const double ui = us * u.y;
+          // u c = (ur cx - ui cy) + i(ur cy + ui cx);  conj(u) c = (ur cx + ui cy) + i(ur cy - ui cx)
+          HSx[j] = fma(u.x, cx, HSx[j]); HSy[j] = fma(u.x, cy, HSy[j]);
+          HDx[j] = fma(-ui, cy, HDx[j]); HDy[j] = fma(ui, cx, HDy[j]);
         }
       }
     }
   }
   if (P.out) {
+    double2 H[n];
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+      H[j] = make_double2(HSx[j] + HDx[j], HSy[j] + HDy[j]);
+      H[n - 1 - j] = make_double2(HSx[j] - HDx[j], HSy[j] - HDy[j]);
+    }
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
       double2 h0 = H[2 * k], h1 = H[2 * k + 1];
@@ -181,7 +214,7 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) field_fft_kernel(const FftPara
   const int N = P.N, stride = arr_stride(N), tid = threadIdx.x;
   double2* z = fft_sm;
   double2* Ws = fft_sm + (size_t)NP * stride;
-  for (int i = tid; i < N / 2; i += FFT_THREADS) Ws[i] = P.W[i];
+  for (int i = tid; i < N / 2; i += FFT_THREADS) Ws[phys(i, 0)] = P.W[i];
   for (int b = blockIdx.x; b < P.batch; b += gridDim.x) {
     const double2* src = reinterpret_cast<const double2*>(P.rho + (size_t)b * N * 2 * NP);
     for (int e = tid; e < N * NP; e += FFT_THREADS) {

@@ -191,11 +191,15 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
       }
     }
   }
-  // Tables of the FFT-factorised form (dg_kernels_fft.cuh), equal-width elements:
-  //   A_p^j = (1/N) e^{-i phi_p} (node factor of Eq. 63),  D_p^j = (i/k_p) e^{i phi_p} e^{i k_p xi_j dx/2},
-  //   phi_p = k_p lo + pi p / N  (the element-centre phase without its e^{-+2 pi i p m/N} part);  W_k = e^{-2 pi i k/N}.
+  // Tables of the FFT-factorised form (dg_kernels_fft.cuh), equal-width elements, p fastest:
+  //   rows 0..n/2-1   B_p^j = node factor of Eq. 63 (B_p^{n-1-j} = conj B_p^j: the LGL nodes are symmetric)
+  //   rows n/2..n-1   u_p^j = e^{i k_p xi_j dx/2}                     (u_p^{n-1-j} = conj u_p^j)
+  //   row  n          a_p   = e^{-i phi_p} / N,  phi_p = k_p lo + pi p / N  (the element-centre phase without its
+  //                   e^{-2 pi i p m/N} part)
+  //   W_k = e^{-2 pi i k/N}.
   if (AD && W) {
-    AD->assign((size_t)P1 * 2 * n * 2, 0.0);
+    const int NPh = n / 2;
+    AD->assign((size_t)P1 * (n + 1) * 2, 0.0);
     W->assign((size_t)(nelem / 2 > 0 ? nelem / 2 : 1) * 2, 0.0);
     for (int k = 0; k < nelem / 2; ++k) {
       (*W)[2 * k] = (double)cosl(2 * PI_L * k / nelem);
@@ -203,23 +207,17 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
     }
 #pragma omp parallel for schedule(static)
     for (int p = 0; p <= pmax; ++p) {
-      const ld kp = 2 * PI_L * p / L;
       const ld ang = PI_L * (ld)(p % (2 * nelem)) / (ld)nelem;
       const ld cm = cosl(ang), sm = sinl(ang);
       const ld cphi = plc[p] * cm - pls[p] * sm, sphi = pls[p] * cm + plc[p] * sm;
-      for (int j = 0; j < n; ++j) {
-        const ld re = nre[(size_t)p * n + j], im = nim[(size_t)p * n + j];
-        double* a = AD->data() + ((size_t)(0 * n + j) * P1 + p) * 2;
-        a[0] = (double)((cphi * re + sphi * im) / nelem);
-        a[1] = (double)((cphi * im - sphi * re) / nelem);
-        if (p > 0) {
-          const ld cj = pjc[(size_t)p * n + j], sj = pjs[(size_t)p * n + j];
-          const ld ar = cphi * cj - sphi * sj, ai = sphi * cj + cphi * sj;      // e^{i phi_p} e^{i k_p xi_j dx/2}
-          double* d = AD->data() + ((size_t)(1 * n + j) * P1 + p) * 2;
-          d[0] = (double)(-ai / kp);                                             // times i / k_p
-          d[1] = (double)(ar / kp);
-        }
+      for (int j = 0; j < NPh; ++j) {
+        double* bq = AD->data() + ((size_t)j * P1 + p) * 2;
+        bq[0] = (double)nre[(size_t)p * n + j]; bq[1] = (double)nim[(size_t)p * n + j];
+        double* uq = AD->data() + ((size_t)(NPh + j) * P1 + p) * 2;
+        uq[0] = (double)pjc[(size_t)p * n + j]; uq[1] = (double)pjs[(size_t)p * n + j];
       }
+      double* aq = AD->data() + ((size_t)n * P1 + p) * 2;
+      aq[0] = (double)(cphi / nelem); aq[1] = (double)(-sphi / nelem);
     }
   }
   // Synthesis with the Poisson factor folded in (Eq. 71): E = sum_{p>=1} 2 Re( (i c_p / k_p) e^{i k_p x} )

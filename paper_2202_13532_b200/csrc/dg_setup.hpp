@@ -19,8 +19,9 @@ Basis1D make_basis(int n, int mass_mode);
 //                     so that E[g] = sum_{p,c} S[g][2p+c] * c_p[c]; columns of p = 0 are zero.
 // x[g]              : node coordinates.
 // dense = false     : T and S are left empty (only x and the tables below are built).
-// AD, W (optional)  : tables of the FFT-factorised form, AD[((t*n + j)*P1 + p)*2 + {re,im}] with t = 0: A_p^j,
-//                     t = 1: D_p^j; W[2k + {re,im}] = e^{-2 pi i k / nelem}, k < nelem/2 (see dg_kernels_fft.cuh).
+// AD, W (optional)  : tables of the FFT-factorised form (even n), AD[(row*P1 + p)*2 + {re,im}]: rows 0..n/2-1 the node
+//                     factors B_p^j of Eq. 63, rows n/2..n-1 the in-element phases u_p^j, row n the centre phase a_p;
+//                     W[2k + {re,im}] = e^{-2 pi i k / nelem}, k < nelem/2 (see dg_kernels_fft.cuh).
 void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
                   std::vector<double>& T, std::vector<double>& S, std::vector<double>& x,
                   std::vector<double>* AD = nullptr, std::vector<double>* W = nullptr, bool dense = true);
