@@ -30,7 +30,7 @@ struct FftParams {
   const double* rho;    // [batch][N*n]
   double* c;            // [batch][P1][2]  (nullptr: not wanted)
   double* out;          // [batch][N*n]    E or Phi (nullptr: projection only)
-  const double2* AD;    // [n+1][P1]       rows B_p^j (j < n/2), u_p^j (j < n/2), a_p; p fastest (lanes walk p: coalesced)
+  const double2* AD;    // [n+1][P1]       rows B_p^j (j < n/2), u_p^j/(k_p N) (j < n/2), a_p; p fastest (lanes walk p: coalesced)
   const double2* W;     // [N/2]           e^{-2 pi i k / N}
   int N, logN, P1, batch;
   int phi;              // 1: potential (Eq. 70) instead of field (Eq. 71)
@@ -122,7 +122,8 @@ __device__ __forceinline__ void fft_all(double2* z, const double2* Ws, int N, in
 // The LGL nodes are symmetric (xi_{n-1-j} = -xi_j, w symmetric), so B_p^{n-1-j} = conj B_p^j and u_p^{n-1-j} =
 // conj u_p^j with  A_p^j = a_p B_p^j,  D_p^j = (i/k_p) conj(N a_p) u_p^j,  a_p = e^{-i(k_p lo + pi p/N)} / N:
 //   s_p = sum_{j<n/2} ( B_p^j X_j + conj(B_p^j) X_{n-1-j} ),   c_p = a_p s_p,
-//   D_p^j c_p = (i / (k_p N)) u_p^j s_p          (|a_p| = 1/N: the centre phase cancels between T and S)
+//   D_p^j c_p = i u_p^j s_p / (k_p N)            (|a_p| = 1/N: the centre phase cancels between T and S; the table
+//                                                 row holds u_p^j / (k_p N), zero at p = 0)
 // i.e. n/2 + n/2 table entries per mode (+ a_p only when c_p itself is wanted) and 4 FMAs per node pair each way.
 template <int NP>
 __device__ __forceinline__ void combine_bin(const FftParams& P, double2* z, int stride, int b, int q) {
@@ -153,7 +154,6 @@ __device__ __forceinline__ void combine_bin(const FftParams& P, double2* z, int 
 #pragma unroll
   for (int j = 0; j < NP; ++j) { HSx[j] = 0.0; HSy[j] = 0.0; HDx[j] = 0.0; HDy[j] = 0.0; }
   double2* cb = P.c ? reinterpret_cast<double2*>(P.c) + (size_t)b * P.P1 : nullptr;
-  const double kn = P.kinv / (double)N;
 #pragma unroll 1
   for (int side = 0; side < 2; ++side) {
     if (side == 1 && self) break;
@@ -172,8 +172,7 @@ __device__ __forceinline__ void combine_bin(const FftParams& P, double2* z, int 
         cb[p] = make_double2(fma(a.x, sx, -a.y * sy), fma(a.x, sy, a.y * sx));
       }
       if (P.out) {
-        const double f = p ? kn / (double)p : 0.0;
-        double cx = -sy * f, cy = sx * f;            // (i / (k_p N)) s_p
+        double cx = -sy, cy = sx;                    // i s_p; the real factor 1/(k_p N) rides in the u table
         if (P.phi) {                                 // Phi~_p = E~_p (i/k_p)  (Eq. 70 vs Eq. 71)
           const double g = P.kinv / (double)(p ? p : 1);
           const double t = cx; cx = -cy * g; cy = t * g;

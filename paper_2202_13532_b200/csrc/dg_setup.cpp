@@ -193,7 +193,7 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
   }
   // Tables of the FFT-factorised form (dg_kernels_fft.cuh), equal-width elements, p fastest:
   //   rows 0..n/2-1   B_p^j = node factor of Eq. 63 (B_p^{n-1-j} = conj B_p^j: the LGL nodes are symmetric)
-  //   rows n/2..n-1   u_p^j = e^{i k_p xi_j dx/2}                     (u_p^{n-1-j} = conj u_p^j)
+  //   rows n/2..n-1   u_p^j / (k_p N),  u_p^j = e^{i k_p xi_j dx/2}   (u_p^{n-1-j} = conj u_p^j; zero at p = 0)
   //   row  n          a_p   = e^{-i phi_p} / N,  phi_p = k_p lo + pi p / N  (the element-centre phase without its
   //                   e^{-2 pi i p m/N} part)
   //   W_k = e^{-2 pi i k/N}.
@@ -214,7 +214,8 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
         double* bq = AD->data() + ((size_t)j * P1 + p) * 2;
         bq[0] = (double)nre[(size_t)p * n + j]; bq[1] = (double)nim[(size_t)p * n + j];
         double* uq = AD->data() + ((size_t)(NPh + j) * P1 + p) * 2;
-        uq[0] = (double)pjc[(size_t)p * n + j]; uq[1] = (double)pjs[(size_t)p * n + j];
+        const ld fk = p ? L / (2 * PI_L * p * nelem) : 0.0L;                 // 1 / (k_p N): Poisson factor of Eq. 71
+        uq[0] = (double)(fk * pjc[(size_t)p * n + j]); uq[1] = (double)(fk * pjs[(size_t)p * n + j]);
       }
       double* aq = AD->data() + ((size_t)n * P1 + p) * 2;
       aq[0] = (double)(cphi / nelem); aq[1] = (double)(-sphi / nelem);
