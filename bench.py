@@ -59,6 +59,20 @@ class ClockSampler:
 
     def __init__(self, index):
         self.index, self.lines, self.proc = index, [], None
+        self.t0 = self.t1 = None
+
+    def wait_ready(self, timeout=5.0):
+        """nvidia-smi takes a few hundred ms to print its first line: block until it has (so that a short timed region
+        is not over before the first sample)."""
+        t = time.perf_counter()
+        while self.proc is not None and not self.lines and time.perf_counter() - t < timeout:
+            time.sleep(0.01)
+
+    def mark_begin(self):
+        self.t0 = time.perf_counter()
+
+    def mark_end(self):
+        self.t1 = time.perf_counter()
 
     def start(self):
         try:
@@ -71,15 +85,19 @@ class ClockSampler:
 
     def _pump(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
 
     def stop(self):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.25)
         self.proc.terminate()
+        # samples taken inside the timed region [mark_begin, mark_end] (+ one sampling period of slack on both sides);
+        # all samples of the run if no marks were set
+        lines = [(t, l) for t, l in self.lines
+                 if self.t0 is None or self.t1 is None or (self.t0 - 0.05 <= t <= self.t1 + 0.05)]
         sm, mx, reasons = [], [], set()
-        for l in self.lines:
+        for _, l in lines:
             p = [s.strip() for s in l.split(",")]
             if len(p) < 8:
                 continue
@@ -181,18 +199,21 @@ def run_ours(args, w, name):
     f = torch.from_numpy(f0).to(dev)
 
     # warm-up, then K timed steps, device-timed, barrier + synchronize on both sides
-    ctx.ssprk3_run(f, dt, args.warmup, True)
-    barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+        sampler.wait_ready()
+    ctx.ssprk3_run(f, dt, args.warmup, True)
+    barrier()
     l0 = ctx.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    sampler.mark_begin()
     e0.record()
     ctx.ssprk3_run(f, dt, args.steps, True)
     e1.record()
     barrier()
+    sampler.mark_end()
     ms = max_over_ranks(e0.elapsed_time(e1))
     clocks = sampler.stop() if rank == 0 else None
     launches = ctx.launch_count - l0
@@ -272,7 +293,7 @@ def run_config4(args, name):
     for _ in range(max(args.warmup, 3)):
         ctx.rhs(f, E, out)
     torch.cuda.synchronize()
-    sampler = ClockSampler(0); sampler.start()
+    sampler = ClockSampler(0); sampler.start(); sampler.wait_ready()
     l0 = ctx.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
@@ -315,7 +336,7 @@ def run_config5(args, name):
     for _ in range(max(args.warmup, 3)):
         ctx.poisson_E(rho, E)
     torch.cuda.synchronize()
-    sampler = ClockSampler(0); sampler.start()
+    sampler = ClockSampler(0); sampler.start(); sampler.wait_ready()
     l0 = ctx.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()

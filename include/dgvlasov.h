@@ -121,6 +121,10 @@ int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_de
 /* Potential instead of field: Phi_mj = sum_{p != 0} -(c_p / k_p^2) e^{i k_p x_mj} (Eq. 70); same
  * arguments, layout and errors as dg_poisson_E.  E = -dPhi/dx. */
 int dg_poisson_phi(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* phi_dev, void* stream);
+/* Broken l2 norm of Eq. 72 on the x grid: eps_b = (1/N_x) sum_m sqrt( int_m (u_b - v_b)^2 dx ), the integrand
+ * being each element's nodal interpolant, integrated exactly with the LGL mass matrix of Eq. 50.
+ *   u_dev, v_dev [in] [batch][N_x*n_x]; v_dev may be NULL (norm of u)     eps_dev [out] [batch] */
+int dg_broken_l2(dg_ctx* ctx, const double* u_dev, const double* v_dev, int32_t batch, double* eps_dev, void* stream);
 size_t dg_field_workspace_bytes(const dg_ctx* ctx, int32_t batch);
 
 /* Introspection (host outputs; any pointer may be NULL to skip it). */

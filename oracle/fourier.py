@@ -3,14 +3,15 @@
 Plain NumPy/SciPy, fp64, written from PAPER.md Section 5.3 (Eq. 59-71).  Shares no code with
 the CUDA path.  Pins: tests/test_oracle_fourier.py (brute-force Gauss-Legendre quadrature of
 the Fourier integral of l_j, c_0[1] = 1, single-cosine closed forms for c_p and E, the
-O(dx^{n+1/2}) convergence of Fig. 4, C^0 continuity of E).
+O(dx^{n+1/2}) convergence of Fig. 4, C^0 continuity of E; broken_l2: Gauss quadrature of the squared
+interpolant and the closed forms ||1||, ||x||).
 """
 from __future__ import annotations
 
 import numpy as np
 from scipy.special import spherical_jn
 
-from .basis import lgl_nodes_weights, legendre_table, gamma_lgl
+from .basis import lgl_nodes_weights, legendre_table, gamma_lgl, mass_matrix
 
 
 def node_coordinates(lo: float, hi: float, nelem: int, n: int) -> np.ndarray:
@@ -71,3 +72,14 @@ def poisson_phi(lo: float, hi: float, x: np.ndarray, c: np.ndarray) -> np.ndarra
         kp = 2.0 * np.pi * p / L
         Phi += 2.0 * np.real((-c[..., p] / kp ** 2)[..., None] * np.exp(1j * kp * x))
     return Phi
+
+
+def broken_l2(lo: float, hi: float, nelem: int, n: int, u: np.ndarray, v=None) -> np.ndarray:
+    """Eq. 72: eps = (1/N) sum_m sqrt(int_m (u - v)^2 dx) for nodal vectors u, v [..., N*n]; the
+    integrand is the element's degree-(n-1) interpolant (Eq. 69), integrated exactly: d^T M d dx/2 with the LGL mass
+    matrix M of Eq. 50."""
+    d = np.asarray(u, dtype=np.float64) - (0.0 if v is None else np.asarray(v, dtype=np.float64))
+    d = d.reshape(d.shape[:-1] + (nelem, n))
+    M = mass_matrix(n)
+    q = np.einsum("...mi,ij,...mj->...m", d, M, d) * 0.5 * (hi - lo) / nelem
+    return np.sqrt(np.maximum(q, 0.0)).sum(axis=-1) / nelem

@@ -45,6 +45,7 @@ SIGNATURES = {
     "dg_fourier_project": (C.c_int, [_vp, _vp, _i32, _vp, _vp]),
     "dg_poisson_E": (C.c_int, [_vp, _vp, _i32, _vp, _vp]),
     "dg_poisson_phi": (C.c_int, [_vp, _vp, _i32, _vp, _vp]),
+    "dg_broken_l2": (C.c_int, [_vp, _vp, _vp, _i32, _vp, _vp]),
     "dg_get_operators": (C.c_int, [_vp, _i32, _dp, _dp, _dp, _dp]),
     "dg_get_nodes": (C.c_int, [_vp, _i32, _dp]),
     "dg_get_transform": (C.c_int, [_vp, _i32, _i32, _dp]),

@@ -150,6 +150,14 @@ class DGContext:
         _check(_L.dg_poisson_phi(self._h, _ptr(rho2), batch, _ptr(out), _stream(self.device)), "dg_poisson_phi")
         return out.reshape(rho.shape)
 
+    def broken_l2(self, u, v=None, out=None):
+        u2 = u.reshape(-1, self.flat_shape[0])
+        v2 = None if v is None else v.reshape(-1, self.flat_shape[0])
+        batch = u2.shape[0]
+        out = torch.empty(batch, dtype=torch.float64, device=self.device) if out is None else out
+        _check(_L.dg_broken_l2(self._h, _ptr(u2), _ptr(v2), batch, _ptr(out), _stream(self.device)), "dg_broken_l2")
+        return out
+
     # --- introspection ------------------------------------------------------------------------
     def operators(self, dim):
         n = self.order[dim]

@@ -111,6 +111,7 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   }
   const size_t o_T = off; off = align_up(off + sizeof(double) * T.size(), 256);
   const size_t o_S = off; off = align_up(off + sizeof(double) * S.size(), 256);
+  const size_t o_wg = off; off = align_up(off + sizeof(double) * 2 * ctx->n[0], 256);
   const size_t o_AD = off; off = align_up(off + sizeof(double) * AD.size(), 256);
   const size_t o_W = off; off = align_up(off + sizeof(double) * W.size(), 256);
   size_t o_cpart = 0, o_sync = 0;
@@ -139,6 +140,21 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   }
   ok = ok && (!dense_now || cudaMemcpy(ctx->d_T, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice) == cudaSuccess);
   ok = ok && (!dense_now || cudaMemcpy(ctx->d_S, S.data(), sizeof(double) * S.size(), cudaMemcpyHostToDevice) == cudaSuccess);
+  {
+    // w_j and w_j P_{n-1}(xi_j) of the x basis: the two vectors of the exact LGL mass matrix (Eq. 50)
+    const int n0 = ctx->n[0];
+    std::vector<double> wg(2 * n0);
+    for (int j = 0; j < n0; ++j) {
+      const long double x = ctx->basis[0].xi_ld[j];
+      long double p0 = 1.0L, p1 = x;
+      for (int s = 1; s < n0 - 1; ++s) { const long double p2 = ((2 * s + 1) * x * p1 - s * p0) / (s + 1); p0 = p1; p1 = p2; }
+      const long double pn1 = (n0 == 1) ? 1.0L : p1;           // P_{n-1}(xi_j)
+      wg[j] = (double)ctx->basis[0].w_ld[j];
+      wg[n0 + j] = (double)(ctx->basis[0].w_ld[j] * pn1);
+    }
+    ctx->d_wg = (double*)(base + o_wg);
+    ok = ok && cudaMemcpy(ctx->d_wg, wg.data(), sizeof(double) * wg.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+  }
   if (fft_ok) {
     ctx->d_AD = (double*)(base + o_AD);
     ctx->d_W = (double*)(base + o_W);
@@ -467,6 +483,16 @@ static int poisson_solve(dg_ctx* ctx, const double* rho_dev, int32_t batch, doub
     if (rc) return rc;
   }
   return launch_synth(ctx, ctx->cbuf, batch, out_dev, st);
+}
+
+extern "C" int dg_broken_l2(dg_ctx* ctx, const double* u_dev, const double* v_dev, int32_t batch, double* eps_dev, void* stream) {
+  if (!ctx || !u_dev || !eps_dev) return fail(DG_ERR_INVALID_ARG, "dg_broken_l2: null argument");
+  if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_broken_l2: batch must be >= 1");
+  const int n0 = ctx->n[0];
+  const double alpha = n0 * (n0 - 1) / (2.0 * (2 * n0 - 1));
+  const double half_dx = 0.5 * (ctx->desc.hi[0] - ctx->desc.lo[0]) / ctx->N[0];
+  dgk::broken_l2_kernel<<<(unsigned)batch, 256, 0, (cudaStream_t)stream>>>(u_dev, v_dev, ctx->d_wg, ctx->N[0], n0, alpha, half_dx, eps_dev);
+  return check_launch(ctx, "broken_l2_kernel");
 }
 
 extern "C" int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_dev, void* stream) {

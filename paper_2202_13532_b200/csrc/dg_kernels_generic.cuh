@@ -209,4 +209,33 @@ __global__ void __launch_bounds__(128) synth_simple_kernel(const double* __restr
   if (lane == 0) E[(size_t)b * G + g] = acc;
 }
 
+// Broken l2 norm of Eq. 72 of the difference of two nodal vectors on the x grid:
+//   eps = (1/N) sum_m sqrt( int_m (u - v)^2 dx ),  the integrand being the element's degree-(n-1) interpolant, integrated
+// exactly by the LGL mass matrix of Eq. 50: d^T M d = sum_j w_j d_j^2 - alpha (sum_j w_j P_{n-1}(xi_j) d_j)^2.
+// One CTA per vector; elements in a fixed order per thread, fixed shared-memory tree: deterministic.
+__global__ void __launch_bounds__(256) broken_l2_kernel(const double* __restrict__ u, const double* __restrict__ v,
+                                                        const double* __restrict__ wg /*[2][n]: w_j, w_j P_{n-1}(xi_j)*/,
+                                                        int N, int n, double alpha, double half_dx, double* __restrict__ eps) {
+  __shared__ double red[256];
+  const size_t off = (size_t)blockIdx.x * N * n;
+  double acc = 0.0;
+  for (int m = threadIdx.x; m < N; m += 256) {
+    double s2 = 0.0, sp = 0.0;
+    for (int j = 0; j < n; ++j) {
+      const size_t g = off + (size_t)m * n + j;
+      const double d = u[g] - (v ? v[g] : 0.0);
+      s2 = fma(wg[j] * d, d, s2);
+      sp = fma(wg[n + j], d, sp);
+    }
+    acc += sqrt(fmax(0.0, fma(-alpha * sp, sp, s2)) * half_dx);
+  }
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) eps[blockIdx.x] = red[0] / (double)N;
+}
+
 }  // namespace dgk

@@ -120,3 +120,46 @@ def test_fft_config5_grid_closed_form_and_sampled_oracle():
     To = ofr.transform_tensor(lo, hi, N, n, 95)
     assert relerr(cz[:, :96], ofr.fourier_project(To, rho)) <= 1e-12
     ctx.close()
+
+
+@pytest.mark.parametrize("N,n,batch", [(10, 3, 1), (25, 8, 4), (64, 8, 40), (300, 5, 7), (2048, 8, 3)])
+def test_broken_l2_matches_oracle(N, n, batch):
+    """dg_broken_l2 (Eq. 72 with the LGL mass matrix of Eq. 50) against the oracle, with and without v."""
+    A = api()
+    lo, hi = -0.5, 2.0
+    ctx = A.DGContext((N,), (n,), (lo,), (hi,), pmax=4, workspace=False)
+    u = wl.uniform_field((batch, N * n), 31) - 0.5
+    v = wl.uniform_field((batch, N * n), 32) - 0.5
+    e = ctx.broken_l2(dev(u), dev(v)).cpu().numpy()
+    assert relerr(e, ofr.broken_l2(lo, hi, N, n, u, v)) <= 1e-13
+    e0 = ctx.broken_l2(dev(u)).cpu().numpy()
+    assert relerr(e0, ofr.broken_l2(lo, hi, N, n, u)) <= 1e-13
+    assert np.array_equal(e, ctx.broken_l2(dev(u), dev(v)).cpu().numpy())
+    ctx.close()
+
+
+@pytest.mark.parametrize("n", [3, 4, 5, 6, 8])
+def test_poisson_hp_convergence_fig4_on_gpu(n):
+    """Fig. 4: Phi'' = sin(2 pi x) on [0, 1], N = 10, 15, 20, 25, pmax = N, through dg_poisson_phi and
+    dg_broken_l2: every error equals the oracle's (same chain on the CPU), and for n <= 6 (above round-off) the
+    h-convergence is at least the paper's O(dx^{n+1/2}).  dg_broken_l2 measures the NODAL error (interpolant of
+    Phi - Phi_exact at the LGL nodes), which superconverges (n = 4: rate 6.5); the rate of the continuous error that
+    Fig. 4 plots is pinned on the oracle in tests/test_oracle_fourier.py::test_poisson_convergence_fig4."""
+    A = api()
+    lo, hi = 0.0, 1.0
+    errs, Ns = [], [10, 15, 20, 25]
+    for N in Ns:
+        ctx = A.DGContext((N,), (n,), (lo,), (hi,), pmax=N, workspace=True)
+        x = ctx.nodes(0)
+        src = np.sin(2 * np.pi * x)
+        exact = -src / (4 * np.pi ** 2)
+        Phi = ctx.poisson_phi(dev(src))
+        eps = float(ctx.broken_l2(Phi, dev(exact)).cpu().numpy()[0])
+        co = ofr.fourier_project(ofr.transform_tensor(lo, hi, N, n, N), src)
+        eps_o = float(ofr.broken_l2(lo, hi, N, n, ofr.poisson_phi(lo, hi, ofr.node_coordinates(lo, hi, N, n), co), exact))
+        assert abs(eps - eps_o) <= 1e-9 * eps_o + 1e-16, (N, eps, eps_o)
+        errs.append(eps)
+        ctx.close()
+    if n <= 6:
+        slope = np.polyfit(np.log(1.0 / np.array(Ns)), np.log(errs), 1)[0]
+        assert slope > n - 0.2, (slope, errs)

@@ -120,3 +120,25 @@ def test_poisson_convergence_fig4(n):
         errs.append(_broken_l2(err, lo, hi, N))
     slope = np.polyfit(np.log(1.0 / np.array(Ns)), np.log(errs), 1)[0]
     assert n - 0.2 < slope < n + 1.6, (slope, errs)
+
+
+@pytest.mark.parametrize("n,N", [(2, 3), (3, 7), (4, 10), (7, 5), (8, 16), (10, 4)])
+def test_broken_l2_against_gauss_quadrature_and_closed_forms(n, N):
+    """fourier.broken_l2 (Eq. 72 with the exact LGL mass matrix, Eq. 50) against 20-point Gauss quadrature of the squared
+    interpolant per element (exact: degree 2n-2 <= 18), and closed forms: ||1|| = sqrt(dx); ||x|| on [0, L]."""
+    lo, hi = -0.5, 2.0
+    dx = (hi - lo) / N
+    xi, _ = basis.lgl_nodes_weights(n)
+    rng = np.random.default_rng(100 * n + N)
+    u, v = rng.standard_normal((3, N * n)), rng.standard_normal((3, N * n))
+    xg, wg = npleg.leggauss(20)
+    Lg = _lagrange_values(xi, xg)                                   # [n][20]
+    d = (u - v).reshape(3, N, n)
+    ref = np.sqrt(np.einsum("g,bmg->bm", wg, np.einsum("bmj,jg->bmg", d, Lg) ** 2) * 0.5 * dx).sum(axis=1) / N
+    assert np.allclose(fourier.broken_l2(lo, hi, N, n, u, v), ref, rtol=1e-13, atol=0)
+    assert np.allclose(fourier.broken_l2(lo, hi, N, n, u), fourier.broken_l2(lo, hi, N, n, u, np.zeros_like(u)), rtol=0, atol=0)
+    assert abs(fourier.broken_l2(lo, hi, N, n, np.ones(N * n)) - np.sqrt(dx)) < 1e-14
+    x = fourier.node_coordinates(lo, hi, N, n)
+    edges = lo + dx * np.arange(N + 1)
+    exact = np.sqrt((edges[1:] ** 3 - edges[:-1] ** 3) / 3.0).sum() / N      # int x^2 over each element
+    assert abs(fourier.broken_l2(lo, hi, N, n, x) - exact) < 1e-13
