@@ -131,6 +131,7 @@ size_t dg_field_workspace_bytes(const dg_ctx* ctx, int32_t batch);
 int dg_get_operators(const dg_ctx* ctx, int32_t dim, double* xi_host /*[n]*/, double* w_host /*[n]*/,
                      double* upsilon_host /*[n][n], row j = output node, reference element*/,
                      double* lift_host /*[n][2]: (L,R)*/);
+int dg_get_dmatrix(const dg_ctx* ctx, int32_t dim, double* D_host /*[n][n]: D[j][k] = l_k'(xi_j), Eq. 55*/);
 int dg_get_nodes(const dg_ctx* ctx, int32_t dim, double* coords_host /*[N_d*n_d]*/);
 int dg_get_transform(const dg_ctx* ctx, int32_t p_first, int32_t p_count, double* T_host /*[p_count][N_x*n_x][2]*/);
 /* Largest dt with sum_d |a_d| dt / Delta_d <= the SSP-RK3 limit of this order and mass mode
@@ -148,6 +149,9 @@ double dg_max_stable_dt(const dg_ctx* ctx, double E_bound);
 #define DG_OPT_PROFILE      3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
 #define DG_OPT_PDL          4   /* 1 (default): consecutive kernels of dg_ssprk3_* are chained by programmatic dependent
                                   launch (the next kernel's prologue overlaps the previous kernel's tail); 0: plain launches */
+#define DG_OPT_FORM         5   /* 0 (default): weak form, Eq. 14: Upsilon F - Xi F*;  1: strong form, Eq. 15
+                                  (PAPER.md:102): -D F + Xi (F - F*), D = Eq. 55.  Same scheme (Upsilon + D = Xi_R e_R^T -
+                                  Xi_L e_L^T), different rounding; both RHS kernels, every entry point. */
 int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value);
 /* Profile mode: total device time (ms) and count of the RHS-kernel launches since the last reset.
  * Synchronises on the recorded events. */

@@ -132,6 +132,26 @@ def rhs(grid: Grid, f: np.ndarray, E=None) -> np.ndarray:
     return out.reshape(grid.flat_shape)
 
 
+def rhs_strong(grid: Grid, f: np.ndarray, E=None) -> np.ndarray:
+    """Strong form Eq. 15: du/dt = sum_d J_d ( -D_d F_d + Xi_d (F_d|faces - NumFlux_d) ), with
+    D = Eq. 55 and the boundary values of F signed by the outward normal like the numerical flux
+    (Appendix A).  Equal to rhs() up to rounding (tests/test_oracle_vlasov.py)."""
+    u = np.asarray(f, dtype=np.float64).reshape(grid.shape)
+    a = speeds(grid, E)
+    out = np.zeros(grid.shape)
+    for d in range(grid.ndim):
+        n = grid.order[d]
+        D = basis.lagrange_derivative_matrix(n)
+        flux = a[d] * u
+        ax = grid.sub_element_axis(d)
+        left = [slice(None)] * flux.ndim;  left[ax] = slice(0, 1)
+        right = [slice(None)] * flux.ndim; right[ax] = slice(n - 1, n)
+        face_flux = np.concatenate((-flux[tuple(left)], flux[tuple(right)]), axis=ax)
+        out += grid.J[d] * (-basis_product(flux, D, ax) + basis_product(face_flux, grid.lift[d], ax)
+                            - flux_in_dim(grid, flux, a[d], d))
+    return out.reshape(grid.flat_shape)
+
+
 def density(grid: Grid, f: np.ndarray) -> np.ndarray:
     """Eq. 27 zeroth moment by LGL quadrature (reading C14):
     rho[g_x] = sum over velocity nodes of prod_d (w_b / J_d) f."""
@@ -149,12 +169,12 @@ def field_E(grid: Grid, f: np.ndarray) -> np.ndarray:
     return fourier.poisson_E(grid.lo[0], grid.hi[0], grid.x_nodes(), c)
 
 
-def ssprk3_step(grid: Grid, f: np.ndarray, dt: float, self_consistent: bool = True, E_fixed=None) -> np.ndarray:
+def ssprk3_step(grid: Grid, f: np.ndarray, dt: float, self_consistent: bool = True, E_fixed=None, strong: bool = False) -> np.ndarray:
     """Shu-Osher SSP-RK3 (reading C3), E from each stage's input (reading C4):
     u1 = u + dt L(u); u2 = 3/4 u + 1/4 (u1 + dt L(u1)); u+ = 1/3 u + 2/3 (u2 + dt L(u2))."""
     def L(u):
         E = field_E(grid, u) if self_consistent else E_fixed
-        return rhs(grid, u, E)
+        return rhs_strong(grid, u, E) if strong else rhs(grid, u, E)
     u = np.asarray(f, dtype=np.float64).reshape(grid.flat_shape)
     u1 = u + dt * L(u)
     u2 = 0.75 * u + 0.25 * (u1 + dt * L(u1))

@@ -48,6 +48,7 @@ SIGNATURES = {
     "dg_broken_l2": (C.c_int, [_vp, _vp, _vp, _i32, _vp, _vp]),
     "dg_get_operators": (C.c_int, [_vp, _i32, _dp, _dp, _dp, _dp]),
     "dg_get_nodes": (C.c_int, [_vp, _i32, _dp]),
+    "dg_get_dmatrix": (C.c_int, [_vp, _i32, _dp]),
     "dg_get_transform": (C.c_int, [_vp, _i32, _i32, _dp]),
     "dg_max_stable_dt": (_dbl, [_vp, _dbl]),
     "dg_set_option": (C.c_int, [_vp, _i32, _i64]),

@@ -17,6 +17,8 @@ OPT_RHS_KERNEL = 1
 OPT_FIELD_KERNEL = 2
 OPT_PROFILE = 3
 OPT_PDL = 4
+OPT_FORM = 5
+FORM_WEAK, FORM_STRONG = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 FIELD_AUTO, FIELD_SIMPLE, FIELD_DMMA, FIELD_DFMA, FIELD_FFT = 0, 1, 2, 3, 4
 BC_PERIODIC, BC_ZERO_INFLOW, BC_HALO = 0, 1, 2
@@ -166,6 +168,12 @@ class DGContext:
         dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
         _check(_L.dg_get_operators(self._h, dim, dp(xi), dp(w), dp(ups), dp(lift)), "dg_get_operators")
         return xi, w, ups, lift
+
+    def dmatrix(self, dim):
+        n = self.order[dim]
+        D = np.empty((n, n))
+        _check(_L.dg_get_dmatrix(self._h, dim, D.ctypes.data_as(C.POINTER(C.c_double))), "dg_get_dmatrix")
+        return D
 
     def nodes(self, dim):
         x = np.empty(self.flat_shape[dim])

@@ -102,10 +102,11 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
 
   // one device block for all constants
   size_t off = 0;
-  size_t o_ups[3], o_lift[3], o_coord[3], o_wq[3];
+  size_t o_ups[3], o_lift[3], o_coord[3], o_wq[3], o_negD[3];
   for (int d = 0; d < desc->ndim; ++d) {
     o_ups[d] = off;   off = align_up(off + sizeof(double) * ctx->n[d] * ctx->n[d], 256);
     o_lift[d] = off;  off = align_up(off + sizeof(double) * ctx->n[d] * 2, 256);
+    o_negD[d] = off;  off = align_up(off + sizeof(double) * ctx->n[d] * ctx->n[d], 256);
     o_coord[d] = off; off = align_up(off + sizeof(double) * ctx->G[d], 256);
     o_wq[d] = off;    off = align_up(off + sizeof(double) * ctx->G[d], 256);
   }
@@ -127,6 +128,12 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   for (int d = 0; d < desc->ndim && ok; ++d) {
     ctx->d_ups[d] = (double*)(base + o_ups[d]);
     ctx->d_lift[d] = (double*)(base + o_lift[d]);
+    ctx->d_negD[d] = (double*)(base + o_negD[d]);
+    {
+      std::vector<double> negD(ctx->basis[d].dmat);
+      for (double& v : negD) v = -v;
+      ok = ok && cudaMemcpy(ctx->d_negD[d], negD.data(), sizeof(double) * negD.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+    }
     ctx->d_coord[d] = (double*)(base + o_coord[d]);
     ctx->d_wq[d] = (double*)(base + o_wq[d]);
     ok = ok && cudaMemcpy(ctx->d_ups[d], ctx->basis[d].ups.data(), sizeof(double) * ctx->n[d] * ctx->n[d], cudaMemcpyHostToDevice) == cudaSuccess;
@@ -241,9 +248,10 @@ static int launch_rhs_generic(dg_ctx* ctx, const double* f, const double* fn, co
   p.ndim = ctx->ndim;
   for (int d = 0; d < 3; ++d) {
     p.N[d] = ctx->N[d]; p.n[d] = ctx->n[d]; p.G[d] = ctx->G[d]; p.bc[d] = ctx->desc.bc[d];
-    p.ups[d] = ctx->d_ups[d]; p.lift[d] = ctx->d_lift[d]; p.coord[d] = ctx->d_coord[d]; p.J[d] = ctx->J[d];
+    p.ups[d] = ctx->opt_form ? ctx->d_negD[d] : ctx->d_ups[d]; p.lift[d] = ctx->d_lift[d]; p.coord[d] = ctx->d_coord[d]; p.J[d] = ctx->J[d];
   }
   p.omega_c = ctx->desc.omega_c;
+  p.strong = ctx->opt_form;
   p.xhalo = ctx->xhalo;
   p.E = E; p.f = f; p.fn = fn; p.out = out; p.c0 = c0; p.c1 = c1; p.dt = dt; p.mode = mode;
   p.dof = (long long)ctx->dof;
@@ -586,6 +594,13 @@ extern "C" int dg_get_operators(const dg_ctx* ctx, int32_t dim, double* xi, doub
   return DG_OK;
 }
 
+extern "C" int dg_get_dmatrix(const dg_ctx* ctx, int32_t dim, double* D) {
+  if (!ctx || dim < 0 || dim >= ctx->ndim || !D) return fail(DG_ERR_INVALID_ARG, "dg_get_dmatrix: bad argument");
+  const dgsetup::Basis1D& b = ctx->basis[dim];
+  memcpy(D, b.dmat.data(), sizeof(double) * b.n * b.n);
+  return DG_OK;
+}
+
 extern "C" int dg_get_nodes(const dg_ctx* ctx, int32_t dim, double* coords) {
   if (!ctx || !coords || dim < 0 || dim >= ctx->ndim) return fail(DG_ERR_INVALID_ARG, "dg_get_nodes: bad argument");
   memcpy(coords, ctx->coord_h[dim].data(), sizeof(double) * ctx->G[dim]);
@@ -648,6 +663,7 @@ extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
   if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 4) { ctx->opt_field_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_PDL && (value == 0 || value == 1)) { ctx->opt_pdl = (int)value; return DG_OK; }
+  if (key == DG_OPT_FORM && (value == 0 || value == 1)) { ctx->opt_form = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg_set_option: unknown key or value");
 }
 

@@ -25,6 +25,7 @@ struct dg_ctx {
   void* dev_block = nullptr;
   double* d_ups[3] = {nullptr, nullptr, nullptr};    // reference Upsilon [n][n]
   double* d_lift[3] = {nullptr, nullptr, nullptr};   // reference Xi [n][2]
+  double* d_negD[3] = {nullptr, nullptr, nullptr};   // -D [n][n] (Eq. 55): the volume operator of the strong form, Eq. 15
   double* d_coord[3] = {nullptr, nullptr, nullptr};  // node coordinates [G_d]
   double* d_wq[3] = {nullptr, nullptr, nullptr};     // quadrature weight w_b / J_d per flat node [G_d]
   double* d_T = nullptr;      // [2*P1][G0]   rows 2p / 2p+1 = Re / Im of T_p (Eq. 63)
@@ -53,6 +54,7 @@ struct dg_ctx {
 
   int64_t launches = 0;
   int opt_rhs_kernel = 0, opt_field_kernel = 0, opt_profile = 0, opt_pdl = 1;
+  int opt_form = 0;           // 0 weak form (Eq. 14), 1 strong form (Eq. 15)
   std::vector<cudaEvent_t> prof_events;   // (start, stop) pairs around RHS launches in profile mode
   double prof_rhs_ms = 0.0;
   int64_t prof_rhs_launches = 0;

@@ -22,6 +22,7 @@ struct GenericParams {
   double* out;
   double c0, c1, dt;        // out = c0*fn + c1*(f + dt*rhs)   (mode 1);   out = rhs (mode 0)
   int mode;
+  int strong;               // 1: strong form Eq. 15 -- ups holds -D and the lift acts on (upwind state - own face value)
   long long dof;
 };
 
@@ -67,6 +68,7 @@ __global__ void __launch_bounds__(256) rhs_generic_kernel(const GenericParams p)
         else if (p.bc[d] == 0) uR = p.f[base - (long long)e * n * strd[d]];
         else if (p.bc[d] == 2) uR = p.xhalo[strd[0] + idx % strd[0]];             // right neighbour's first x plane
       }
+      if (p.strong) { uL -= own0; uR -= own1; }                  // Eq. 15: Xi (F - F*) with -D F
       const double xl = p.lift[d][2 * j], xr = p.lift[d][2 * j + 1];
       rhs += (p.J[d] * a[d]) * (vol - xr * uR + xl * uL);
     }

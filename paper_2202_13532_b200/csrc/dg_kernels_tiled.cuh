@@ -93,6 +93,7 @@ struct alignas(64) TiledParams {
   int N0, N1, N2, G0, G1, G2;
   int bc0, bc1, bc2;
   int tiles_v, mode, has_fn, want_partials;
+  int strong;            // 1: strong form Eq. 15 -- pe/qo are built from -D and the lift acts on (upwind state - own face value)
 };
 
 template <int NN, int KV>
@@ -139,6 +140,8 @@ __device__ __forceinline__ void apply_lines2(const TiledParams<NN>& P, const dou
     for (int k = 0; k < H; ++k) { e[l][k] = f[l][k] + f[l][NN - 1 - k]; o[l][k] = f[l][k] - f[l][NN - 1 - k]; }
     sp[l] = uL[l] + uR[l];
     dm[l] = uL[l] - uR[l];
+    // strong form (Eq. 15): (uL - f_0) +- (uR - f_{n-1})
+    if (P.strong) { sp[l] -= e[l][0]; dm[l] -= o[l][0]; }
   }
 #pragma unroll
   for (int j = 0; j < H; ++j) {
@@ -459,10 +462,13 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   }
   const dgsetup::Basis1D& b = ctx->basis[0];
   constexpr int H = NN / 2;
+  P.strong = ctx->opt_form;
+  // volume operator: Upsilon (weak form, Eq. 14) or -D (strong form, Eq. 15); both are centro-antisymmetric
+  auto vol = [&](int j, int k) { return ctx->opt_form ? -b.dmat[j * NN + k] : b.ups[j * NN + k]; };
   for (int j = 0; j < H; ++j) {
     for (int k = 0; k < H; ++k) {
-      P.pe[j * H + k] = 0.5 * (b.ups[j * NN + k] + b.ups[j * NN + NN - 1 - k]);
-      P.qo[j * H + k] = 0.5 * (b.ups[j * NN + k] - b.ups[j * NN + NN - 1 - k]);
+      P.pe[j * H + k] = 0.5 * (vol(j, k) + vol(j, NN - 1 - k));
+      P.qo[j * H + k] = 0.5 * (vol(j, k) - vol(j, NN - 1 - k));
     }
     P.la[j] = 0.5 * (b.lift[2 * j] - b.lift[2 * j + 1]);
     P.lb[j] = 0.5 * (b.lift[2 * j] + b.lift[2 * j + 1]);

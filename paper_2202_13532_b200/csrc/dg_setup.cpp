@@ -76,6 +76,8 @@ Basis1D make_basis(int n, int mass_mode) {
   dPN[0] = ((N + 1) % 2 == 0 ? 1.0L : -1.0L) * 0.5L * N * (N + 1);
   b.xi.resize(n); b.w.resize(n); b.ups.assign(n * n, 0.0); b.lift.assign(n * 2, 0.0);
   b.xi_ld = xi; b.w_ld = w;
+  b.dmat.resize(n * n);
+  for (int i = 0; i < n * n; ++i) b.dmat[i] = (double)dl[i];      // (D f)_j = sum_k l_k'(xi_j) f_k
   for (int j = 0; j < n; ++j) { b.xi[j] = (double)xi[j]; b.w[j] = (double)w[j]; }
   for (int j = 0; j < n; ++j) {
     for (int k = 0; k < n; ++k) {

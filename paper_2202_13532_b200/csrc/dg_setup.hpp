@@ -10,6 +10,7 @@ struct Basis1D {
   std::vector<long double> xi_ld, w_ld;
   std::vector<double> ups;          // Upsilon[j*n + k], reference element      (Eq. 53)
   std::vector<double> lift;         // Xi[j*2 + {0:L,1:R}]                      (Eq. 54)
+  std::vector<double> dmat;         // D[j*n + k] = l_k'(xi_j)                  (Eq. 55), strong form Eq. 15
 };
 
 Basis1D make_basis(int n, int mass_mode);
