@@ -112,3 +112,54 @@ def cosine_sum_density(x: np.ndarray, batch: int, seed: int, nterms: int = 16, m
         rho[bi] = r
         A[bi], M[bi], PH[bi] = a, m, ph
     return rho, A, M, PH
+
+
+# ---------------------------------------------------------------------------------------------
+# Cyclotron-harmonic instability of the paper's Section 4.1 / 6.1 (simulations A and B)
+# ---------------------------------------------------------------------------------------------
+def ring_distribution(vx: np.ndarray, vy: np.ndarray, j: int, alpha: float = 1.0) -> np.ndarray:
+    """Eq. 31: f0 = (v_perp^2 / 2 alpha^2)^j exp(-v_perp^2 / 2 alpha^2) / (2 pi alpha^2 j!), [G_u][G_v]."""
+    s = (vx[:, None] ** 2 + vy[None, :] ** 2) / (2.0 * alpha ** 2)
+    return s ** j * np.exp(-s) / (2.0 * math.pi * alpha ** 2 * math.factorial(j))
+
+
+def harris_dispersion(omega: complex, k: float, j: int, ratio: float, alpha: float = 1.0, npts: int = 50) -> complex:
+    """Eq. 34: eps(omega, k) = 1 + (omega_p/omega_c)^2 / sin(pi omega) *
+    int_0^pi sin(omega th) sin(th) L_j(beta) exp(-beta) dth,  beta = 2 k^2 alpha^2 cos^2(th/2); omega in units of
+    omega_c, k in units of 1/r_L; fifty-point Gauss-Legendre as in the paper."""
+    from scipy.special import eval_laguerre
+    xg, wg = np.polynomial.legendre.leggauss(npts)
+    th = 0.5 * math.pi * (xg + 1.0)
+    beta = 2.0 * (k * alpha) ** 2 * np.cos(0.5 * th) ** 2
+    integ = np.sum(0.5 * math.pi * wg * np.sin(omega * th) * np.sin(th) * eval_laguerre(j, beta) * np.exp(-beta))
+    return 1.0 + ratio ** 2 * integ / np.sin(math.pi * omega)
+
+
+def eigenmode_perturbation(x: np.ndarray, vx: np.ndarray, vy: np.ndarray, k_sim: float, k_larmor: float, omega: complex,
+                           j: int, alpha: float = 1.0, nmax: int = 20, sense: int = -1) -> np.ndarray:
+    """Eq. 35-36: f1 = (1/v_perp) d f0/d v_perp * Re(psi0),
+    psi0 = exp(i (k x + k_L v_perp sin(phi))) sum_{|n| <= nmax} n/(n - omega) J_n(k_L v_perp) exp(-i n phi),
+    with (u, v) = v_perp (cos phi, sin phi); k_sim is the wavenumber in the simulation's length unit (x), k_L the same
+    wavenumber in units of the Larmor radius (k_L = k_sim * omega_p/omega_c), omega in units of omega_c.
+    (1/v) d f0/dv = (j - v^2/2 alpha^2) f0 / v^2 (Eq. 32) is evaluated as (j - s) s^(j-1) e^{-s} / (2 alpha^2 Z), s = v^2/2 alpha^2,
+    which is finite at v = 0.  Returns [G_x][G_u][G_v], unnormalised.
+
+    sense: sign of the gyro-angle, (u, v) = v_perp (cos phi, sense * sin phi).  With the force of Eq. 28 as printed
+    (du/dt = -B v, dv/dt = +B u: counter-clockwise gyration, x - v/B invariant) integrating the linearised equation along
+    the unperturbed orbits gives psi0 = exp(i (k x - k_L v_perp sin phi)) sum n/(n - omega) J_n exp(+i n phi), i.e.
+    Eq. 36 with phi -> -phi; sense = -1 (default) is that form, sense = +1 is Eq. 36 literally.  DESIGN.md reading C24:
+    only sense = -1 grows at the paper's rate 0.349 omega_c from t = 0 (tests/test_gpu_physics.py)."""
+    from scipy.special import jv
+    U, V = vx[:, None], vy[None, :]
+    vp = np.sqrt(U ** 2 + V ** 2)
+    phi = np.arctan2(sense * V, U)
+    s = vp ** 2 / (2.0 * alpha ** 2)
+    grad = (j - s) * s ** (j - 1) * np.exp(-s) / (2.0 * alpha ** 2) / (2.0 * math.pi * alpha ** 2 * math.factorial(j))
+    series = np.zeros(vp.shape, dtype=np.complex128)
+    for n in range(-nmax, nmax + 1):
+        if n == 0:
+            continue
+        series += n / (n - omega) * jv(n, k_larmor * vp) * np.exp(-1j * n * phi)
+    psi_v = np.exp(1j * k_larmor * vp * np.sin(phi)) * series                     # velocity part of psi0
+    psi = np.exp(1j * k_sim * x)[:, None, None] * psi_v[None, :, :]
+    return grad[None, :, :] * np.real(psi)
