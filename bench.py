@@ -174,6 +174,9 @@ def run_reference(args, w, name):
 # -----------------------------------------------------------------------------------------------
 # our arm
 # -----------------------------------------------------------------------------------------------
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {("config3_1d2v_512^3", "rhs_tiled<8,4>"): (2.110807e9 + 3.199168e9 + 3.185062e9) / 3.0}
+
+
 def run_ours(args, w, name):
     import torch
     from paper_2202_13532_b200 import api, dist_util as du
@@ -191,6 +194,8 @@ def run_ours(args, w, name):
     def max_over_ranks(v):
         return du.max_over_ranks(v, dev)
 
+    if args.parallelism == "xslab":
+        return run_xslab(args, w, name, world, rank, local, dev, barrier, max_over_ranks)
     ga = grid_args(w)
     ctx = api.DGContext(device=local, **ga)
     f0 = make_f0(ctx.nodes(0), ctx.nodes(1), ctx.nodes(2), w)
@@ -231,8 +236,11 @@ def run_ours(args, w, name):
     peak, peak_src = measured_peak_hbm()
     avg_launch_s = rhs_ms * 1e-3 / max(rhs_n, 1)
     achieved = BYTES_PER_DOF_PER_STAGE * dof / avg_launch_s / 1e9
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this kernel on
+    # this workload (profiles/r1_kernels.md: 2.111, 3.199, 3.185 GB for the three stages of a step); null elsewhere
+    traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get((name, kernel))
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": kernel, "avg_launch_ms": avg_launch_s * 1e3, "launches_timed": rhs_n,
+                "traffic": traffic, "traffic_source": "profiles/r1_kernels.md (ncu --set full)" if traffic else None, "kernel": kernel, "avg_launch_ms": avg_launch_s * 1e3, "launches_timed": rhs_n,
                 "algorithmic_bytes_per_launch": BYTES_PER_DOF_PER_STAGE * dof, "peak_source": peak_src,
                 "rhs_share_of_step": (rhs_ms / psteps) / (ms / args.steps)}
 
@@ -268,6 +276,54 @@ def run_ours(args, w, name):
         }
         print(json.dumps(line), flush=True)
     ctx.close()
+    du.finalize()
+
+
+def run_xslab(args, w, name, world, rank, local, dev, barrier, max_over_ranks):
+    """ONE problem sharded by x-slabs over the ranks (paper_2202_13532_b200/sharded.py): the workload's x
+    extent and element count are multiplied by the number of ranks (weak scaling: every rank holds the workload's own
+    grid), per stage an all-gather of rho and a face-plane exchange with the two x-neighbours over NCCL."""
+    import torch
+    from paper_2202_13532_b200 import api, dist_util as du, sharded
+    ga = grid_args(w)
+    nelem = (ga["nelem"][0] * world,) + tuple(ga["nelem"][1:])
+    lo, hi = tuple(ga["lo"]), (ga["lo"][0] + (ga["hi"][0] - ga["lo"][0]) * world,) + tuple(ga["hi"][1:])
+    st = sharded.XSlabStepper(nelem, ga["order"], lo, hi, bc=ga["bc"], omega_c=ga["omega_c"], pmax=ga["pmax"] * world,
+                              rank=rank, world=world, device=local)
+    slab = st.be.slab
+    f0 = make_f0(slab.nodes(0), slab.nodes(1), slab.nodes(2), w)       # the same wave repeats in every slab
+    dof, dt = f0.size, w["dt"]
+    f = torch.from_numpy(f0).to(dev)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start(); sampler.wait_ready()
+    st.run(f, dt, args.warmup, True)
+    barrier()
+    l0 = slab.launch_count + st.be.field.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.mark_begin()
+    e0.record()
+    st.run(f, dt, args.steps, True)
+    e1.record()
+    barrier()
+    sampler.mark_end()
+    ms = max_over_ranks(e0.elapsed_time(e1))
+    clocks = sampler.stop() if rank == 0 else None
+    launches = slab.launch_count + st.be.field.launch_count - l0
+    finite = du.all_ranks_true(bool(torch.isfinite(f).all().item()), dev)
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": du.replica_throughput(dof, 3, args.steps, ms, world), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "grid": "x".join(str(n * o) for n, o in zip(nelem, ga["order"])), "dof": dof * world,
+                       "dt": dt, "self_consistent_poisson_each_stage": True, "mass_mode": 0,
+                       "l2": "inputs (3 x %.2f GB per rank) larger than L2; no flush needed" % (dof * 8 / 1e9),
+                       "parallelism": "xslab x%d (all-gather of rho + x-face exchange per stage)" % world, "finite": finite},
+            "clocks": clocks, "gpu_launches": launches,
+            "hbm_gbs_algorithmic_whole_step": 64.0 * dof * world * args.steps / (ms * 1e-3) / 1e9}), flush=True)
+    st.close()
     du.finalize()
 
 
@@ -389,6 +445,8 @@ def main():
     ap.add_argument("--workload", default="config3_1d2v_512^3", choices=sorted(WORKLOADS) + sorted(CONFIG4) + ["config5_field"])
     ap.add_argument("--batch", type=int, default=4096, help="config5_field only")
     ap.add_argument("--field-kernel", default="auto", choices=["auto", "dmma", "dfma", "fft"], help="config5_field only")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "xslab"],
+                    help="N > 1: independent replicas (default, DESIGN.md section 9) or one problem sharded by x-slabs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
