@@ -158,6 +158,7 @@ int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value);
 int dg_get_profile(dg_ctx* ctx, double* rhs_ms_total_host, int64_t* rhs_launches_host, int32_t reset);
 int64_t dg_launch_count(const dg_ctx* ctx);      /* kernels launched through this context so far */
 const char* dg_last_kernel(const dg_ctx* ctx);   /* name of the RHS kernel variant last used */
+const char* dg_last_field_kernel(const dg_ctx* ctx);   /* name of the projection / field-solve kernel last used */
 const char* dg_last_error(void);
 const char* dg_version(void);
 

@@ -22,26 +22,27 @@ def node_coordinates(lo: float, hi: float, nelem: int, n: int) -> np.ndarray:
     return (xbar[:, None] + 0.5 * dx * xi[None, :]).reshape(-1)
 
 
-def transform_tensor(lo: float, hi: float, nelem: int, n: int, pmax: int) -> np.ndarray:
+def transform_tensor(lo: float, hi: float, nelem: int, n: int, pmax: int, p_first: int = 0) -> np.ndarray:
     """Eq. 63: T[p, m*n+j] = (dx/L) exp(-i k_p xbar_m) w_j
     sum_{s<n} gamma_s^{-1} (-i)^s P_s(xi_j) j_s(k_p dx/2), p = 0..pmax, k_p = 2 pi p / L.
     (Eq. 64 as printed is wrong, reading C7; Eq. 63 is the definition.)  xbar_m and x_mj are
-    absolute coordinates; exp(i k_p x) is L-periodic so any interval [lo, lo+L) serves Eq. 60."""
+    absolute coordinates; exp(i k_p x) is L-periodic so any interval [lo, lo+L) serves Eq. 60.
+    p_first > 0 returns only the rows p = p_first..pmax (same arithmetic; for tests that walk a large pmax in slices)."""
     xi, w = lgl_nodes_weights(n)
     P, _ = legendre_table(n, xi)
     g = gamma_lgl(n)
     L = hi - lo
     dx = L / nelem
     xbar = lo + (np.arange(nelem) + 0.5) * dx
-    T = np.zeros((pmax + 1, nelem, n), dtype=np.complex128)
-    for p in range(pmax + 1):
+    T = np.zeros((pmax + 1 - p_first, nelem, n), dtype=np.complex128)
+    for p in range(p_first, pmax + 1):
         kp = 2.0 * np.pi * p / L
         z = kp * dx / 2.0
         node = np.zeros(n, dtype=np.complex128)
         for s in range(n):
             node += (1.0 / g[s]) * (-1j) ** s * P[s] * spherical_jn(s, z)
-        T[p] = (dx / L) * np.exp(-1j * kp * xbar)[:, None] * (w * node)[None, :]
-    return T.reshape(pmax + 1, nelem * n)
+        T[p - p_first] = (dx / L) * np.exp(-1j * kp * xbar)[:, None] * (w * node)[None, :]
+    return T.reshape(pmax + 1 - p_first, nelem * n)
 
 
 def fourier_project(T: np.ndarray, rho: np.ndarray) -> np.ndarray:

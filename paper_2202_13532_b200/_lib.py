@@ -55,6 +55,7 @@ SIGNATURES = {
     "dg_get_profile": (C.c_int, [_vp, _dp, C.POINTER(_i64), _i32]),
     "dg_launch_count": (_i64, [_vp]),
     "dg_last_kernel": (C.c_char_p, [_vp]),
+    "dg_last_field_kernel": (C.c_char_p, [_vp]),
     "dg_last_error": (C.c_char_p, []),
     "dg_version": (C.c_char_p, []),
 }

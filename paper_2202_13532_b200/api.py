@@ -204,3 +204,7 @@ class DGContext:
     @property
     def last_kernel(self):
         return _L.dg_last_kernel(self._h).decode()
+
+    @property
+    def last_field_kernel(self):
+        return _L.dg_last_field_kernel(self._h).decode()

@@ -381,6 +381,7 @@ static int launch_fft(dg_ctx* ctx, const double* rho, int batch, double* c, doub
   P.kinv = (ctx->desc.hi[0] - ctx->desc.lo[0]) / 6.283185307179586476925286766559;
   int rc = dgfft::launch_fft(P, ctx->n[0], ctx->sm_count, st);
   if (rc != 0) return fail(DG_ERR_CUDA, "field_fft_kernel launch failed");
+  ctx->last_field_kernel = "field_fft_kernel";
   return check_launch(ctx, "field_fft_kernel");
 }
 
@@ -404,10 +405,12 @@ static int launch_project(dg_ctx* ctx, const double* rho, int batch, double* c, 
     // C[batch][2*P1] = rho[batch][G] * T[2*P1][G]^T
     int rc = dgf::launch_gemm_tn(rho, ctx->d_T, c, batch, 2 * P1, G, st, ctx->opt_field_kernel == 3 ? 1 : 0);
     if (rc != DG_OK) return fail(rc, "projection GEMM launch failed");
+    ctx->last_field_kernel = ctx->opt_field_kernel == 3 ? "field_gemm_tn_kernel" : "field_gemm_dmma_kernel";
     return check_launch(ctx, "field_gemm_kernel");
   }
   dim3 grid(P1, batch);
   dgk::project_simple_kernel<<<grid, 128, 0, st>>>(ctx->d_T, rho, G, P1, c);
+  ctx->last_field_kernel = "project_simple_kernel";
   return check_launch(ctx, "project_simple_kernel");
 }
 
@@ -527,6 +530,7 @@ static int field_from_partials_or_f(dg_ctx* ctx, const double* f, int partial_ch
     P.nchunks = partial_chunks; P.G0 = ctx->G[0]; P.Q = 2 * ctx->P1; P.rows = ctx->fused_rows;
     rc = dgf::launch_field_fused(P, ctx->fused_grid, pdl, st);
     if (rc != DG_OK) return fail(rc, std::string("field_fused_kernel launch failed: ") + cudaGetErrorString(cudaGetLastError()));
+    ctx->last_field_kernel = "field_fused_kernel";
     return check_launch(ctx, "field_fused_kernel");
   }
   if (partial_chunks > 0) rc = launch_density_finish(ctx, ctx->partials, partial_chunks, ctx->rho, st);
@@ -669,3 +673,4 @@ extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
 
 extern "C" int64_t dg_launch_count(const dg_ctx* ctx) { return ctx ? ctx->launches : 0; }
 extern "C" const char* dg_last_kernel(const dg_ctx* ctx) { return ctx ? ctx->last_kernel.c_str() : "none"; }
+extern "C" const char* dg_last_field_kernel(const dg_ctx* ctx) { return ctx ? ctx->last_field_kernel.c_str() : "none"; }

@@ -59,5 +59,6 @@ struct dg_ctx {
   double prof_rhs_ms = 0.0;
   int64_t prof_rhs_launches = 0;
   std::string last_kernel = "none";
+  std::string last_field_kernel = "none";
   double cfl_limit = -1.0;    // lazily computed
 };
