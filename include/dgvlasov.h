@@ -61,6 +61,11 @@ typedef struct {
  * weights, node coordinates, the DG->Fourier tensor T (Eq. 63) and the synthesis matrix of
  * Eq. 71; uploads them.  *out owns that device memory until dg_destroy. */
 int dg_create(const dg_grid_desc* desc, dg_ctx** out);
+/* x-only context (field operations: dg_fourier_project, dg_poisson_E, dg_poisson_phi, dg_broken_l2, introspection) whose
+ * elements have the explicitly given edges: Eq. 63 with its per-element (Delta x)_m.
+ *   edges_host [in] [nelem+1], strictly ascending; x is periodic with L = edges[nelem] - edges[0]
+ * Dense kernels only (the FFT factorisation needs equal widths: DG_OPT_FIELD_KERNEL = 4 fails with DG_ERR_UNSUPPORTED). */
+int dg_create_field_nonuniform(const double* edges_host, int32_t nelem, int32_t order, int32_t pmax, int32_t device, dg_ctx** out);
 int dg_destroy(dg_ctx* ctx);
 
 /* Scratch for dg_ssprk3_* and dg_poisson_E: two stage arrays of the size of f, density

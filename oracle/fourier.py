@@ -45,6 +45,35 @@ def transform_tensor(lo: float, hi: float, nelem: int, n: int, pmax: int, p_firs
     return T.reshape(pmax + 1 - p_first, nelem * n)
 
 
+def node_coordinates_edges(edges: np.ndarray, n: int) -> np.ndarray:
+    """x_{mj} = xbar_m + xi_j (dx)_m / 2 for explicitly given element edges (non-uniform widths), flattened [m*n + j]."""
+    xi, _ = lgl_nodes_weights(n)
+    e = np.asarray(edges, dtype=np.float64)
+    xbar, dx = 0.5 * (e[:-1] + e[1:]), e[1:] - e[:-1]
+    return (xbar[:, None] + 0.5 * dx[:, None] * xi[None, :]).reshape(-1)
+
+
+def transform_tensor_edges(edges: np.ndarray, n: int, pmax: int) -> np.ndarray:
+    """Eq. 63 with its per-element width: T[p, m*n+j] = ((dx)_m/L) exp(-i k_p xbar_m) w_j
+    sum_{s<n} gamma_s^{-1} (-i)^s P_s(xi_j) j_s(k_p (dx)_m/2), L = edges[-1] - edges[0]."""
+    xi, w = lgl_nodes_weights(n)
+    P, _ = legendre_table(n, xi)
+    g = gamma_lgl(n)
+    e = np.asarray(edges, dtype=np.float64)
+    nelem = e.size - 1
+    L = e[-1] - e[0]
+    T = np.zeros((pmax + 1, nelem, n), dtype=np.complex128)
+    for p in range(pmax + 1):
+        kp = 2.0 * np.pi * p / L
+        for m in range(nelem):
+            dx, xbar = e[m + 1] - e[m], 0.5 * (e[m] + e[m + 1])
+            node = np.zeros(n, dtype=np.complex128)
+            for s in range(n):
+                node += (1.0 / g[s]) * (-1j) ** s * P[s] * spherical_jn(s, kp * dx / 2.0)
+            T[p, m] = (dx / L) * np.exp(-1j * kp * xbar) * w * node
+    return T.reshape(pmax + 1, nelem * n)
+
+
 def fourier_project(T: np.ndarray, rho: np.ndarray) -> np.ndarray:
     """c_p = T_p^{mj} f_mj (text after Eq. 64). rho: [..., G] -> c: [..., pmax+1]."""
     return np.einsum("pg,...g->...p", T, rho)
@@ -75,12 +104,13 @@ def poisson_phi(lo: float, hi: float, x: np.ndarray, c: np.ndarray) -> np.ndarra
     return Phi
 
 
-def broken_l2(lo: float, hi: float, nelem: int, n: int, u: np.ndarray, v=None) -> np.ndarray:
+def broken_l2(lo: float, hi: float, nelem: int, n: int, u: np.ndarray, v=None, edges=None) -> np.ndarray:
     """Eq. 72: eps = (1/N) sum_m sqrt(int_m (u - v)^2 dx) for nodal vectors u, v [..., N*n]; the
     integrand is the element's degree-(n-1) interpolant (Eq. 69), integrated exactly: d^T M d dx/2 with the LGL mass
-    matrix M of Eq. 50."""
+    matrix M of Eq. 50.  edges: explicit element edges [nelem+1] for non-uniform widths."""
     d = np.asarray(u, dtype=np.float64) - (0.0 if v is None else np.asarray(v, dtype=np.float64))
     d = d.reshape(d.shape[:-1] + (nelem, n))
     M = mass_matrix(n)
-    q = np.einsum("...mi,ij,...mj->...m", d, M, d) * 0.5 * (hi - lo) / nelem
+    half = 0.5 * (hi - lo) / nelem if edges is None else 0.5 * np.diff(np.asarray(edges, dtype=np.float64))
+    q = np.einsum("...mi,ij,...mj->...m", d, M, d) * half
     return np.sqrt(np.maximum(q, 0.0)).sum(axis=-1) / nelem

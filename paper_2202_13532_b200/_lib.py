@@ -32,6 +32,7 @@ _vp, _dp, _i32, _i64, _dbl = C.c_void_p, C.POINTER(C.c_double), C.c_int32, C.c_i
 SIGNATURES = {
     "dg_create": (C.c_int, [C.POINTER(GridDesc), C.POINTER(_vp)]),
     "dg_destroy": (C.c_int, [_vp]),
+    "dg_create_field_nonuniform": (C.c_int, [_dp, _i32, _i32, _i32, _i32, C.POINTER(_vp)]),
     "dg_workspace_bytes": (C.c_size_t, [_vp]),
     "dg_field_workspace_bytes": (C.c_size_t, [_vp, _i32]),
     "dg_set_workspace": (C.c_int, [_vp, _vp, C.c_size_t]),

@@ -79,6 +79,25 @@ class DGContext:
             base = (self._ws.data_ptr() + 255) // 256 * 256
             _check(_L.dg_set_workspace(self._h, base, nbytes), "dg_set_workspace")
 
+    @classmethod
+    def field_nonuniform(cls, edges, order, pmax=0, device=0, field_batch=1):
+        """dg_create_field_nonuniform: x-only context with explicitly given element edges (Eq. 63's (Delta x)_m)."""
+        e = np.ascontiguousarray(edges, dtype=np.float64)
+        self = cls.__new__(cls)
+        self._h = C.c_void_p()
+        nelem = e.size - 1
+        _check(_L.dg_create_field_nonuniform(e.ctypes.data_as(C.POINTER(C.c_double)), nelem, int(order), int(pmax), int(device),
+                                             C.byref(self._h)), "dg_create_field_nonuniform")
+        self.ndim, self.nelem, self.order = 1, (nelem,), (int(order),)
+        self.device = torch.device("cuda", device)
+        self.flat_shape = (nelem * int(order),)
+        self.pmax = int(pmax) if pmax > 0 else nelem
+        nbytes = _L.dg_field_workspace_bytes(self._h, int(field_batch))
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self._ws.data_ptr() + 255) // 256 * 256
+        _check(_L.dg_set_workspace(self._h, base, nbytes), "dg_set_workspace")
+        return self
+
     def close(self):
         if getattr(self, "_h", None) is not None and self._h:
             _L.dg_destroy(self._h)

@@ -40,7 +40,23 @@ extern "C" const char* dg_version(void) { return "dgvlasov-b200 0.1 (sm_100a)"; 
 // ------------------------------------------------------------------------------------------------
 // create / destroy
 // ------------------------------------------------------------------------------------------------
-extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
+static int create_impl(const dg_grid_desc* desc, const double* edges, dg_ctx** out);
+
+extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) { return create_impl(desc, nullptr, out); }
+
+extern "C" int dg_create_field_nonuniform(const double* edges_host, int32_t nelem, int32_t order, int32_t pmax, int32_t device,
+                                          dg_ctx** out) {
+  if (!edges_host || !out || nelem < 1) return fail(DG_ERR_INVALID_ARG, "dg_create_field_nonuniform: bad argument");
+  for (int m = 0; m < nelem; ++m)
+    if (!(edges_host[m + 1] > edges_host[m])) return fail(DG_ERR_INVALID_ARG, "dg_create_field_nonuniform: edges must ascend");
+  dg_grid_desc d;
+  memset(&d, 0, sizeof(d));
+  d.ndim = 1; d.nelem[0] = nelem; d.order[0] = order; d.lo[0] = edges_host[0]; d.hi[0] = edges_host[nelem];
+  d.pmax = pmax; d.device = device;
+  return create_impl(&d, edges_host, out);
+}
+
+static int create_impl(const dg_grid_desc* desc, const double* edges, dg_ctx** out) {
   if (!desc || !out) return fail(DG_ERR_INVALID_ARG, "dg_create: null argument");
   *out = nullptr;
   if (desc->ndim < 1 || desc->ndim > 3) return fail(DG_ERR_INVALID_ARG, "dg_create: ndim must be 1, 2 or 3");
@@ -73,14 +89,16 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   ctx->P1 = ctx->pmax + 1;
 
   std::vector<double> T, S, x, AD, W;
-  const bool fft_ok = dgfft::fft_supported(ctx->N[0], ctx->n[0]);
+  if (edges) ctx->edges.assign(edges, edges + ctx->N[0] + 1);
+  const bool fft_ok = !edges && dgfft::fft_supported(ctx->N[0], ctx->n[0]);      // the FFT factorisation needs equal widths
   // Large x-only contexts that the FFT kernel serves build the dense T and S (2 x 2.15 GB at config 5) only when a
   // dense kernel or dg_get_transform asks for them (ensure_dense).
   const bool dense_now = !(fft_ok && desc->ndim == 1 && (size_t)2 * ctx->P1 * ctx->G[0] > ((size_t)1 << 22));
   try {
     for (int d = 0; d < desc->ndim; ++d) ctx->basis[d] = dgsetup::make_basis(ctx->n[d], desc->mass_mode);
-    dgsetup::make_fourier(ctx->basis[0], ctx->N[0], desc->lo[0], desc->hi[0], ctx->pmax, T, S, x,
-                          fft_ok ? &AD : nullptr, fft_ok ? &W : nullptr, dense_now);
+    if (edges) dgsetup::make_fourier_nonuniform(ctx->basis[0], ctx->edges, ctx->pmax, T, S, x);
+    else dgsetup::make_fourier(ctx->basis[0], ctx->N[0], desc->lo[0], desc->hi[0], ctx->pmax, T, S, x,
+                               fft_ok ? &AD : nullptr, fft_ok ? &W : nullptr, dense_now);
   } catch (const std::exception& e) {
     delete ctx;
     return fail(DG_ERR_INVALID_ARG, std::string("dg_create: setup failed: ") + e.what());
@@ -113,6 +131,7 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
   const size_t o_T = off; off = align_up(off + sizeof(double) * T.size(), 256);
   const size_t o_S = off; off = align_up(off + sizeof(double) * S.size(), 256);
   const size_t o_wg = off; off = align_up(off + sizeof(double) * 2 * ctx->n[0], 256);
+  const size_t o_hdx = off; off = align_up(off + sizeof(double) * (edges ? ctx->N[0] : 0), 256);
   const size_t o_AD = off; off = align_up(off + sizeof(double) * AD.size(), 256);
   const size_t o_W = off; off = align_up(off + sizeof(double) * W.size(), 256);
   size_t o_cpart = 0, o_sync = 0;
@@ -158,6 +177,12 @@ extern "C" int dg_create(const dg_grid_desc* desc, dg_ctx** out) {
       const long double pn1 = (n0 == 1) ? 1.0L : p1;           // P_{n-1}(xi_j)
       wg[j] = (double)ctx->basis[0].w_ld[j];
       wg[n0 + j] = (double)(ctx->basis[0].w_ld[j] * pn1);
+    }
+    if (edges) {
+      std::vector<double> hdx(ctx->N[0]);
+      for (int m = 0; m < ctx->N[0]; ++m) hdx[m] = 0.5 * (ctx->edges[m + 1] - ctx->edges[m]);
+      ctx->d_half_dx = (double*)(base + o_hdx);
+      ok = ok && cudaMemcpy(ctx->d_half_dx, hdx.data(), sizeof(double) * hdx.size(), cudaMemcpyHostToDevice) == cudaSuccess;
     }
     ctx->d_wg = (double*)(base + o_wg);
     ok = ok && cudaMemcpy(ctx->d_wg, wg.data(), sizeof(double) * wg.size(), cudaMemcpyHostToDevice) == cudaSuccess;
@@ -348,6 +373,7 @@ static int launch_density_finish(dg_ctx* ctx, const double* partial, int nchunks
 // Dense T and S on first use (contexts created without them, see dg_create).
 static int ensure_dense(dg_ctx* ctx) {
   if (ctx->d_T && ctx->d_S) return DG_OK;
+  if (!ctx->edges.empty()) return fail(DG_ERR_CUDA, "dense transform missing on a non-uniform context");
   std::vector<double> T, S, x;
   try {
     dgsetup::make_fourier(ctx->basis[0], ctx->N[0], ctx->desc.lo[0], ctx->desc.hi[0], ctx->pmax, T, S, x);
@@ -502,7 +528,8 @@ extern "C" int dg_broken_l2(dg_ctx* ctx, const double* u_dev, const double* v_de
   const int n0 = ctx->n[0];
   const double alpha = n0 * (n0 - 1) / (2.0 * (2 * n0 - 1));
   const double half_dx = 0.5 * (ctx->desc.hi[0] - ctx->desc.lo[0]) / ctx->N[0];
-  dgk::broken_l2_kernel<<<(unsigned)batch, 256, 0, (cudaStream_t)stream>>>(u_dev, v_dev, ctx->d_wg, ctx->N[0], n0, alpha, half_dx, eps_dev);
+  dgk::broken_l2_kernel<<<(unsigned)batch, 256, 0, (cudaStream_t)stream>>>(u_dev, v_dev, ctx->d_wg, ctx->d_half_dx, ctx->N[0], n0, alpha,
+                                                                         half_dx, eps_dev);
   return check_launch(ctx, "broken_l2_kernel");
 }
 

@@ -35,6 +35,8 @@ struct dg_ctx {
   double* d_AD = nullptr;     // [P1][2][n0] complex: A_p^j, D_p^j
   double* d_W = nullptr;      // [N0/2] complex twiddles
   int sm_count = 148;
+  std::vector<double> edges;  // element edges of a non-uniform x-only context (dg_create_field_nonuniform), else empty
+  double* d_half_dx = nullptr;  // [N0] half widths of such a context
   double* d_wg = nullptr;     // [2][n0]: w_j and w_j P_{n-1}(xi_j) of the x basis (broken l2 norm, Eq. 50 / 72)
   // one-launch field solve (field_fused_kernel): per-CTA shares of c_q and the rendezvous words
   double* d_cpart = nullptr;  // [2*P1][fused_grid]

@@ -217,6 +217,7 @@ __global__ void __launch_bounds__(128) synth_simple_kernel(const double* __restr
 // One CTA per vector; elements in a fixed order per thread, fixed shared-memory tree: deterministic.
 __global__ void __launch_bounds__(256) broken_l2_kernel(const double* __restrict__ u, const double* __restrict__ v,
                                                         const double* __restrict__ wg /*[2][n]: w_j, w_j P_{n-1}(xi_j)*/,
+                                                        const double* __restrict__ half_dx_m /*[N] or nullptr: equal widths*/,
                                                         int N, int n, double alpha, double half_dx, double* __restrict__ eps) {
   __shared__ double red[256];
   const size_t off = (size_t)blockIdx.x * N * n;
@@ -229,7 +230,7 @@ __global__ void __launch_bounds__(256) broken_l2_kernel(const double* __restrict
       s2 = fma(wg[j] * d, d, s2);
       sp = fma(wg[n + j], d, sp);
     }
-    acc += sqrt(fmax(0.0, fma(-alpha * sp, sp, s2)) * half_dx);
+    acc += sqrt(fmax(0.0, fma(-alpha * sp, sp, s2)) * (half_dx_m ? half_dx_m[m] : half_dx));
   }
   red[threadIdx.x] = acc;
   __syncthreads();

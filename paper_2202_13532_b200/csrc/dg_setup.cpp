@@ -242,6 +242,66 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
   }
 }
 
+// Non-uniform element widths: Eq. 63 with its per-element (Delta x)_m, dense T and S only (the FFT
+// factorisation needs equal widths).  edges[0..N] ascending; x periodic with L = edges[N] - edges[0].
+void make_fourier_nonuniform(const Basis1D& b, const std::vector<double>& edges, int pmax,
+                             std::vector<double>& T, std::vector<double>& S, std::vector<double>& x) {
+  const int n = b.n, nelem = (int)edges.size() - 1, G = nelem * n, P1 = pmax + 1;
+  const ld lo = edges[0], L = (ld)edges[nelem] - (ld)edges[0];
+  T.assign((size_t)2 * P1 * G, 0.0);
+  S.assign((size_t)G * 2 * P1, 0.0);
+  x.resize(G);
+  std::vector<ld> Ps(n * n), xl(G);
+  for (int j = 0; j < n; ++j) {
+    ld p0 = 1.0L, p1 = b.xi_ld[j];
+    Ps[0 * n + j] = p0; if (n > 1) Ps[1 * n + j] = p1;
+    for (int s = 1; s < n - 1; ++s) {
+      ld p2 = ((2 * s + 1) * b.xi_ld[j] * p1 - s * p0) / (s + 1);
+      Ps[(s + 1) * n + j] = p2; p0 = p1; p1 = p2;
+    }
+  }
+  for (int m = 0; m < nelem; ++m)
+    for (int j = 0; j < n; ++j) {
+      xl[m * n + j] = 0.5L * ((ld)edges[m] + (ld)edges[m + 1]) + 0.5L * ((ld)edges[m + 1] - (ld)edges[m]) * b.xi_ld[j];
+      x[m * n + j] = (double)xl[m * n + j];
+    }
+  // cos, sin of k_p y with the argument reduced in units of the period: p (y - lo)/L mod 1, plus k_p lo
+  auto phase = [&](int p, ld y, ld& c, ld& s) {
+    ld t = (ld)p * ((y - lo) / L);
+    t -= floorl(t);
+    const ld ang = 2 * PI_L * t + 2 * PI_L * p * (lo / L);
+    c = cosl(ang); s = sinl(ang);
+  };
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int p = 0; p <= pmax; ++p) {
+    const ld kp = 2 * PI_L * p / L;
+    std::vector<ld> js(n);
+    for (int m = 0; m < nelem; ++m) {
+      const ld dx = (ld)edges[m + 1] - (ld)edges[m], xbar = 0.5L * ((ld)edges[m] + (ld)edges[m + 1]);
+      spherical_bessel(n - 1, kp * dx / 2, js.data());
+      ld c0, s0; phase(p, xbar, c0, s0);
+      const ld c = c0 * (dx / L), sgn = -s0 * (dx / L);                 // (dx_m / L) e^{-i k xbar_m}
+      for (int j = 0; j < n; ++j) {
+        ld re = 0.0L, im = 0.0L;
+        for (int s = 0; s < n; ++s) {
+          const ld ginv = (s < n - 1) ? (2 * s + 1) / 2.0L : (n - 1) / 2.0L;      // 1/gamma_s, Eq. 46
+          const ld v = ginv * Ps[s * n + j] * js[s];
+          switch (s & 3) { case 0: re += v; break; case 1: im -= v; break; case 2: re -= v; break; default: im += v; break; }
+        }
+        re *= b.w_ld[j]; im *= b.w_ld[j];
+        const size_t g = (size_t)m * n + j;
+        T[((size_t)(2 * p) * G) + g] = (double)(c * re - sgn * im);
+        T[((size_t)(2 * p + 1) * G) + g] = (double)(c * im + sgn * re);
+        if (p > 0) {
+          ld cth, sth; phase(p, xl[g], cth, sth);
+          S[g * 2 * P1 + 2 * p] = (double)(-2.0L / kp * sth);               // Eq. 71 with -1/(i k_p) folded in
+          S[g * 2 * P1 + 2 * p + 1] = (double)(-2.0L / kp * cth);
+        }
+      }
+    }
+  }
+}
+
 // SSP-RK3 stability limit of the 1-D periodic upwind DG operator (the paper defers its CFL numbers
 // to ref. [39]).  For Bloch phase th the element operator (a > 0, unit a, J = 2/dx) is
 // A(th) = Ups - Xi_R e_R^T + e^{-i th} Xi_L e_R^T;  the step matrix is R = I + Z + Z^2/2 + Z^3/6 with

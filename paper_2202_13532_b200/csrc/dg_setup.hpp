@@ -27,6 +27,10 @@ void make_fourier(const Basis1D& b, int nelem, double lo, double hi, int pmax,
                   std::vector<double>& T, std::vector<double>& S, std::vector<double>& x,
                   std::vector<double>* AD = nullptr, std::vector<double>* W = nullptr, bool dense = true);
 
+// The same dense T, S and x for explicitly given element edges (non-uniform widths, Eq. 63 with (Delta x)_m).
+void make_fourier_nonuniform(const Basis1D& b, const std::vector<double>& edges, int pmax,
+                             std::vector<double>& T, std::vector<double>& S, std::vector<double>& x);
+
 // Largest a*dt/dx for which SSP-RK3 is stable on the 1-D periodic upwind DG operator built from `b`.
 double rk3_cfl_limit(const Basis1D& b);
 

@@ -163,3 +163,31 @@ def test_poisson_hp_convergence_fig4_on_gpu(n):
     if n <= 6:
         slope = np.polyfit(np.log(1.0 / np.array(Ns)), np.log(errs), 1)[0]
         assert slope > n - 0.2, (slope, errs)
+
+
+@pytest.mark.parametrize("n,N,pmax,batch,kernel", [(8, 24, 30, 1, 0), (6, 37, 50, 40, 2), (5, 9, 12, 70, 3), (4, 64, 64, 5, 1)])
+def test_nonuniform_element_widths_match_oracle(n, N, pmax, batch, kernel):
+    """dg_create_field_nonuniform: Eq. 63 with per-element widths.  T, nodes, c_p, E, Phi and the broken l2 norm against the
+    oracle on a graded grid (widths varying 4x); the FFT kernel must refuse (it needs equal widths)."""
+    A = api()
+    w = 1.0 + 0.6 * np.sin(np.arange(N) * 0.7)
+    edges = -0.3 + np.concatenate([[0.0], np.cumsum(w)]) * (2 * math.pi / w.sum())
+    ctx = A.DGContext.field_nonuniform(edges, n, pmax=pmax, field_batch=batch)
+    x = ofr.node_coordinates_edges(edges, n)
+    assert np.max(np.abs(ctx.nodes(0) - x)) < 1e-15 * 8
+    To = ofr.transform_tensor_edges(edges, n, pmax)
+    assert np.max(np.abs(ctx.transform() - To)) <= 5e-16 * N * n
+    ctx.set_option(A.OPT_FIELD_KERNEL, kernel)
+    rho, _, _, _ = wl.cosine_sum_density(x, batch, 77, mmax=max(1, pmax // 3))
+    co = ofr.fourier_project(To, rho)
+    c = ctx.fourier_project(dev(rho)).cpu().numpy()
+    assert relerr(c[..., 0] + 1j * c[..., 1], co) <= 1e-12
+    assert relerr(ctx.poisson_E(dev(rho)).cpu().numpy(), ofr.poisson_E(edges[0], edges[-1], x, co)) <= 1e-12
+    Phio = ofr.poisson_phi(edges[0], edges[-1], x, co)
+    assert np.max(np.abs(ctx.poisson_phi(dev(rho)).cpu().numpy() - Phio)) <= 1e-12 * np.max(np.abs(Phio)) + 1e-14 * np.max(np.abs(rho))
+    u, v = wl.uniform_field((batch, N * n), 5), wl.uniform_field((batch, N * n), 6)
+    assert relerr(ctx.broken_l2(dev(u), dev(v)).cpu().numpy(), ofr.broken_l2(0, 0, N, n, u, v, edges=edges)) <= 1e-13
+    ctx.set_option(A.OPT_FIELD_KERNEL, A.FIELD_FFT)
+    with pytest.raises(A.DGError):
+        ctx.poisson_E(dev(rho))
+    ctx.close()

@@ -142,3 +142,40 @@ def test_broken_l2_against_gauss_quadrature_and_closed_forms(n, N):
     edges = lo + dx * np.arange(N + 1)
     exact = np.sqrt((edges[1:] ** 3 - edges[:-1] ** 3) / 3.0).sum() / N      # int x^2 over each element
     assert abs(fourier.broken_l2(lo, hi, N, n, x) - exact) < 1e-13
+
+
+def test_nonuniform_transform_brute_force_and_reduction_to_uniform():
+    """transform_tensor_edges (Eq. 63 with (dx)_m) against 80-point Gauss quadrature of the Fourier integral of l_j on each
+    element, c_0[1] = 1, and equality with transform_tensor when the edges are equally spaced."""
+    n, pmax = 6, 14
+    edges = np.array([-1.0, -0.4, -0.25, 0.3, 0.35, 1.1, 1.5])
+    N = edges.size - 1
+    T = fourier.transform_tensor_edges(edges, n, pmax).reshape(pmax + 1, N, n)
+    xi, _ = basis.lgl_nodes_weights(n)
+    xg, wg = npleg.leggauss(80)
+    Lg = _lagrange_values(xi, xg)
+    L = edges[-1] - edges[0]
+    for p in range(pmax + 1):
+        kp = 2 * np.pi * p / L
+        for m in range(N):
+            dx, xbar = edges[m + 1] - edges[m], 0.5 * (edges[m] + edges[m + 1])
+            integ = (Lg * (wg * np.exp(-1j * kp * (xbar + 0.5 * dx * xg)))[None, :]).sum(axis=1) * (0.5 * dx / L)
+            assert np.allclose(T[p, m], integ, atol=5e-16, rtol=1e-13), (p, m)
+    assert abs(fourier.fourier_project(T.reshape(pmax + 1, -1), np.ones(N * n))[0] - 1.0) < 1e-14
+    eq = np.linspace(0.5, 3.0, 9)
+    assert np.allclose(fourier.transform_tensor_edges(eq, 5, 9), fourier.transform_tensor(0.5, 3.0, 8, 5, 9), atol=1e-16, rtol=1e-13)
+    assert np.allclose(fourier.node_coordinates_edges(eq, 5), fourier.node_coordinates(0.5, 3.0, 8, 5), atol=1e-15)
+
+
+def test_nonuniform_poisson_single_cosine_closed_form():
+    """E = -(A/k) sin(kx + ph), Phi = -(A/k^2) cos(kx + ph) on a graded grid (widths varying 4x), n = 8."""
+    n, N = 8, 24
+    w = 1.0 + 0.6 * np.sin(np.arange(N) * 0.7)
+    edges = np.concatenate([[0.0], np.cumsum(w)]) * (2 * np.pi / w.sum())
+    x = fourier.node_coordinates_edges(edges, n)
+    A, m, ph = 0.03, 3, 0.8
+    c = fourier.fourier_project(fourier.transform_tensor_edges(edges, n, 12), 1 + A * np.cos(m * x + ph))
+    assert abs(c[m] - 0.5 * A * np.exp(1j * ph)) < 1e-12 and abs(c[0] - 1) < 1e-13
+    E = fourier.poisson_E(edges[0], edges[-1], x, c)
+    assert np.max(np.abs(E + (A / m) * np.sin(m * x + ph))) < 1e-10 * A / m
+    assert abs(fourier.broken_l2(0, 0, N, n, np.ones(N * n), edges=edges) - np.sqrt(np.diff(edges)).sum() / N) < 1e-14
