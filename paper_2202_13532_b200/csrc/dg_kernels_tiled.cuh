@@ -164,8 +164,12 @@ __device__ __forceinline__ void apply_lines2(const TiledParams<NN>& P, const dou
 // ------------------------------------------------------------------------------------------------
 // kernel
 // ------------------------------------------------------------------------------------------------
+// resident CTAs per SM the register allocation must allow: set for n = 10 only (134 -> 128 registers: 4 CTAs instead of 3);
+// the other orders reach the shared-memory limit with the default allocation (0 = unspecified)
+__host__ __device__ constexpr int tiled_min_ctas(int n) { return n == 10 ? 4 : 0; }   // 0: unspecified
+
 template <int NN, int KV>
-__global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
+__global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
   using Cfg = TileCfg<NN, KV>;
   constexpr int R = Cfg::R, H = Cfg::H, RP = R / 2;
   extern __shared__ __align__(1024) unsigned char smem[];
@@ -201,7 +205,10 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
   const double cf = (P.mode != 0) ? P.c1 : 0.0;
   const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
   const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
-  const int v_ju = t % H, v_ev = (t / H) % KV, v_jx = t / (KV * H);  // phase v: rows ju and ju + H of (jx, ev)
+  // phase v: rows ju and ju + H of (jx, ev).  Swizzled tiles: ju fastest (the XOR spreads the rows over the banks);
+  // plain row-major tiles (R != 32): ev fastest -- a row is R/2 16-byte units and an element n/2 of them, and
+  // (n/2) ev + (R/2) ju hits 8 different bank groups over 8 lanes for (n, KV) = (6, 4), (10, 2), (10, 3)
+  const int v_ju = Cfg::SWZ ? t % H : (t / KV) % H, v_ev = Cfg::SWZ ? (t / H) % KV : t % KV, v_jx = t / (KV * H);
   const double ax = cr * P.Jx * P.vx[gu0 + xu_hi];                                         // a_x = u
   double au[2], av[2];
 #pragma unroll
@@ -398,7 +405,7 @@ __global__ void __launch_bounds__(NN * NN * KV / 2) rhs_tiled_kernel(const __gri
 static thread_local std::string g_tiled_err;
 inline const char* last_error() { return g_tiled_err.c_str(); }
 
-inline int kv_for_order(int n) { return n == 4 ? 8 : (n == 6 ? 4 : (n == 8 ? 4 : (n == 10 ? 3 : 0))); }
+inline int kv_for_order(int n) { return n == 4 ? 8 : (n == 6 ? 4 : (n == 8 ? 4 : (n == 10 ? 2 : 0))); }
 
 inline bool tiled_supported(const dg_ctx* ctx) {
   if (ctx->ndim != 3) return false;
@@ -512,7 +519,7 @@ inline int launch_rhs_tiled(dg_ctx* ctx, const double* f, const double* fn, cons
     case 4: return launch_rhs_tiled_t<4, 8>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
     case 6: return launch_rhs_tiled_t<6, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
     case 8: return launch_rhs_tiled_t<8, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-    case 10: return launch_rhs_tiled_t<10, 3>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 10: return launch_rhs_tiled_t<10, 2>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
     default: g_tiled_err = "order not supported by the tiled kernel"; return DG_ERR_UNSUPPORTED;
   }
 }
