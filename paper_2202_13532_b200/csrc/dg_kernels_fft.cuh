@@ -58,30 +58,48 @@ __device__ __forceinline__ double2 cmulc(double2 a, double2 bconj) {   // a * co
   return make_double2(fma(a.x, bconj.x, a.y * bconj.y), fma(a.y, bconj.x, -a.x * bconj.y));
 }
 
+// XOR of the 3-bit digits of i (the bank-group part of phys): linear over GF(2), so for index parts with disjoint bits
+// digits(a + b) = digits(a) ^ digits(b) -- the passes below fold the thread-invariant parts once.
+__host__ __device__ __forceinline__ int digits(int i) {
+  int x = i ^ (i >> 3);
+  x ^= x >> 6;
+  return x & 7;
+}
+
 // One pass of R fused radix-2 stages over all NP arrays.  lh = log2 of the smallest half-size of the pass.
+// Element t of a work item sits at base + (t << lh) with base's bits disjoint from t's, so its slot is
+// ((base + (t << lh)) & ~7) | (digits(base) ^ digits(t << lh) ^ kx): one digit fold per item, the t part per pass.
 template <int R, bool INV>
 __device__ __forceinline__ void fft_pass(double2* z, const double2* Ws, int N, int logN, int lh, int NP, int stride, int tid) {
   constexpr int M = 1 << R;
-  const int groups = N >> R, h = 1 << lh;
-  for (int item = tid; item < groups * NP; item += FFT_THREADS) {
-    const int k = item / groups, g = item - k * groups;
+  const int lg = logN - R, h = 1 << lh;           // 2^lg work items per array
+  int dt[M];                                     // digits(t << lh): the same for every thread
+#pragma unroll
+  for (int t = 0; t < M; ++t) dt[t] = digits(t << lh);
+  for (int item = tid; item < (NP << lg); item += FFT_THREADS) {
+    const int k = item >> lg, g = item & ((1 << lg) - 1);
     const int blk = g >> lh, i0 = g & (h - 1);
     const int base = (blk << (lh + R)) + i0;
     double2* za = z + (size_t)k * stride;
-    const int kx = 2 * k;
+    const int db = digits(base) ^ ((2 * k) & 7);
+    int slot[M];
+#pragma unroll
+    for (int t = 0; t < M; ++t) slot[t] = ((base + (t << lh)) & ~7) | (db ^ dt[t]);
     double2 e[M];
 #pragma unroll
-    for (int t = 0; t < M; ++t) e[t] = za[phys(base + (t << lh), kx)];
+    for (int t = 0; t < M; ++t) e[t] = za[slot[t]];
 #pragma unroll
     for (int s = 0; s < R; ++s) {
       const int lt = INV ? s : (R - 1 - s);          // log2 of the half-size of this stage in units of t
       const int half_t = 1 << lt;
       const int shift = logN - 1 - (lh + lt);        // twiddle stride N / (2 hs)
+      const int wi0 = i0 << shift, dw0 = digits(wi0);
 #pragma unroll
       for (int t = 0; t < M; ++t) {
         if (t & half_t) continue;
-        const int pos = i0 + ((t & (half_t - 1)) << lh);
-        const double2 w = Ws[phys(pos << shift, 0)];
+        // twiddle index (i0 + (tt << lh)) << shift, tt = t mod half_t: again two disjoint parts
+        const int wt = (t & (half_t - 1)) << (lh + shift);
+        const double2 w = Ws[((wi0 + wt) & ~7) | (dw0 ^ digits(wt))];
         const double2 a = e[t];
         if (!INV) {
           const double2 b = e[t + half_t];
@@ -95,7 +113,7 @@ __device__ __forceinline__ void fft_pass(double2* z, const double2* Ws, int N, i
       }
     }
 #pragma unroll
-    for (int t = 0; t < M; ++t) za[phys(base + (t << lh), kx)] = e[t];
+    for (int t = 0; t < M; ++t) za[slot[t]] = e[t];
   }
 }
 
