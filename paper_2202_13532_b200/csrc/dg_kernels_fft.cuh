@@ -76,6 +76,7 @@ __device__ __forceinline__ void fft_pass(double2* z, const double2* Ws, int N, i
   int dt[M];                                     // digits(t << lh): the same for every thread
 #pragma unroll
   for (int t = 0; t < M; ++t) dt[t] = digits(t << lh);
+#pragma unroll 2
   for (int item = tid; item < (NP << lg); item += FFT_THREADS) {
     const int k = item >> lg, g = item & ((1 << lg) - 1);
     const int blk = g >> lh, i0 = g & (h - 1);
@@ -178,12 +179,19 @@ __device__ __forceinline__ void combine_bin(const FftParams& P, double2* z, int 
     const double sg = side ? -1.0 : 1.0;             // side 1: X_j[N-q] = conj X_j[q] (rho is real)
     for (int p = side ? qm : q; p < P.P1; p += N) {
       const double2* tb = P.AD + p;
+      // all table rows of this mode in flight together (one L2 latency per mode, not one per use)
+      double2 B[NP], U[NP];
+#pragma unroll
+      for (int j = 0; j < NP; ++j) B[j] = __ldg(tb + (size_t)j * P.P1);
+      if (P.out) {
+#pragma unroll
+        for (int j = 0; j < NP; ++j) U[j] = __ldg(tb + (size_t)(NP + j) * P.P1);
+      }
       double sx = 0.0, sy = 0.0;
 #pragma unroll
       for (int j = 0; j < NP; ++j) {
-        const double2 B = __ldg(tb + (size_t)j * P.P1);
-        sx = fma(B.x, Sx[j], fma(-sg * B.y, Dy[j], sx));
-        sy = fma(sg * B.x, Sy[j], fma(B.y, Dx[j], sy));
+        sx = fma(B[j].x, Sx[j], fma(-sg * B[j].y, Dy[j], sx));
+        sy = fma(sg * B[j].x, Sy[j], fma(B[j].y, Dx[j], sy));
       }
       if (cb) {
         const double2 a = __ldg(tb + (size_t)n * P.P1);
@@ -199,7 +207,7 @@ __device__ __forceinline__ void combine_bin(const FftParams& P, double2* z, int 
         const double us = sg;
 #pragma unroll
         for (int j = 0; j < NP; ++j) {
-          const double2 u = __ldg(tb + (size_t)(NP + j) * P.P1);
+          const double2 u = U[j];
           const double ui = us * u.y;
           // u c = (ur cx - ui cy) + i(ur cy + ui cx);  conj(u) c = (ur cx + ui cy) + i(ur cy - ui cx)
           HSx[j] = fma(u.x, cx, HSx[j]); HSy[j] = fma(u.x, cy, HSy[j]);
