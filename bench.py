@@ -194,7 +194,7 @@ def run_ours(args, w, name):
     def max_over_ranks(v):
         return du.max_over_ranks(v, dev)
 
-    if args.parallelism == "xslab":
+    if args.parallelism in ("xslab", "xslab-push"):
         return run_xslab(args, w, name, world, rank, local, dev, barrier, max_over_ranks)
     ga = grid_args(w)
     ctx = api.DGContext(device=local, **ga)
@@ -289,7 +289,7 @@ def run_xslab(args, w, name, world, rank, local, dev, barrier, max_over_ranks):
     nelem = (ga["nelem"][0] * world,) + tuple(ga["nelem"][1:])
     lo, hi = tuple(ga["lo"]), (ga["lo"][0] + (ga["hi"][0] - ga["lo"][0]) * world,) + tuple(ga["hi"][1:])
     st = sharded.XSlabStepper(nelem, ga["order"], lo, hi, bc=ga["bc"], omega_c=ga["omega_c"], pmax=ga["pmax"] * world,
-                              rank=rank, world=world, device=local)
+                              rank=rank, world=world, device=local, push=(args.parallelism == "xslab-push"))
     slab = st.be.slab
     f0 = make_f0(slab.nodes(0), slab.nodes(1), slab.nodes(2), w)       # the same wave repeats in every slab
     dof, dt = f0.size, w["dt"]
@@ -320,7 +320,9 @@ def run_xslab(args, w, name, world, rank, local, dev, barrier, max_over_ranks):
             "config": {"workload": name, "grid": "x".join(str(n * o) for n, o in zip(nelem, ga["order"])), "dof": dof * world,
                        "dt": dt, "self_consistent_poisson_each_stage": True, "mass_mode": 0,
                        "l2": "inputs (3 x %.2f GB per rank) larger than L2; no flush needed" % (dof * 8 / 1e9),
-                       "parallelism": "xslab x%d (all-gather of rho + x-face exchange per stage)" % world, "finite": finite},
+                       "parallelism": ("xslab x%d (all-gather of rho + x-face planes stored into the neighbours' halos by the RHS kernel)"
+                                       if st.push else "xslab x%d (all-gather of rho + x-face exchange per stage)") % world,
+                       "finite": finite},
             "clocks": clocks, "gpu_launches": launches,
             "hbm_gbs_algorithmic_whole_step": 64.0 * dof * world * args.steps / (ms * 1e-3) / 1e9}), flush=True)
     st.close()
@@ -445,8 +447,9 @@ def main():
     ap.add_argument("--workload", default="config3_1d2v_512^3", choices=sorted(WORKLOADS) + sorted(CONFIG4) + ["config5_field"])
     ap.add_argument("--batch", type=int, default=4096, help="config5_field only")
     ap.add_argument("--field-kernel", default="auto", choices=["auto", "dmma", "dfma", "fft"], help="config5_field only")
-    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "xslab"],
-                    help="N > 1: independent replicas (default, DESIGN.md section 9) or one problem sharded by x-slabs")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "xslab", "xslab-push"],
+                    help="N > 1: independent replicas (default, DESIGN.md section 9) or one problem sharded by x-slabs, with the "
+                         "face planes exchanged by send/recv (xslab) or stored by the RHS kernel into peer memory (xslab-push)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

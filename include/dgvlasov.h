@@ -91,6 +91,15 @@ int dg_rhs(dg_ctx* ctx, const double* f_dev, const double* E_dev, double* dfdt_d
 #define DG_BC_HALO 2
 int dg_set_xhalo(dg_ctx* ctx, const double* halo_dev);
 
+/* Fused face-plane exchange for x-slab contexts.  After this call every dg_rk_stage also stores the first x-node plane of
+ * out_dev into left_dst_dev and the last one into right_dst_dev, from inside the RHS kernel (a second TMA store of the
+ * boundary tiles' rows).  The destinations are planes [G_u][G_v] of the x-NEIGHBOURS' halo buffers: left_dst_dev = plane 1
+ * of the left neighbour's buffer (its exterior state right of its last node), right_dst_dev = plane 0 of the right
+ * neighbour's -- device pointers into peer memory (NVLink P2P / symmetric memory) or into this device's own memory.
+ * The caller double-buffers the halos (the stage that is running still reads the buffer set by dg_set_xhalo) and orders
+ * the ranks (the all-gather of the density between two stages does).  NULL disables a side.  16-byte aligned. */
+int dg_set_xhalo_push(dg_ctx* ctx, double* left_dst_dev, double* right_dst_dev);
+
 /* One Runge-Kutta stage in Shu-Osher form: out = c0 f_n + c1 (f_s + dt L(f_s; E)).
  *   f_s_dev [in] stage input   f_n_dev [in] step input (NULL when c0 = 0)   E_dev [in] field or NULL
  *   out_dev [out] may alias f_n_dev (each node is read and written by one thread), not f_s_dev

@@ -41,6 +41,7 @@ SIGNATURES = {
     "dg_ssprk3_run": (C.c_int, [_vp, _vp, _dbl, _i32, _i32, _vp]),
     "dg_ssprk3_run_host": (C.c_int, [_vp, _vp, _dbl, _i32, _i32]),
     "dg_set_xhalo": (C.c_int, [_vp, _vp]),
+    "dg_set_xhalo_push": (C.c_int, [_vp, _vp, _vp]),
     "dg_rk_stage": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _dbl, _vp, _vp]),
     "dg_density": (C.c_int, [_vp, _vp, _vp, _vp]),
     "dg_fourier_project": (C.c_int, [_vp, _vp, _i32, _vp, _vp]),

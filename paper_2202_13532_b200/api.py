@@ -121,6 +121,11 @@ class DGContext:
         self._xhalo = halo
         _check(_L.dg_set_xhalo(self._h, _ptr(halo)), "dg_set_xhalo")
 
+    def set_xhalo_push(self, left_dst, right_dst):
+        """left_dst / right_dst: [G_u][G_v] planes in the x-neighbours' halo buffers (or None); kept alive here."""
+        self._push = (left_dst, right_dst)
+        _check(_L.dg_set_xhalo_push(self._h, _ptr(left_dst), _ptr(right_dst)), "dg_set_xhalo_push")
+
     def rk_stage(self, f_s, f_n, E, out, c0, c1, dt, rho_out=None):
         _check(_L.dg_rk_stage(self._h, _ptr(f_s), _ptr(f_n), _ptr(E), _ptr(out), float(c0), float(c1), float(dt),
                               _ptr(rho_out), _stream(self.device)), "dg_rk_stage")

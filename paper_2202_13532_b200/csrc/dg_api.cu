@@ -277,6 +277,8 @@ static int launch_rhs_generic(dg_ctx* ctx, const double* f, const double* fn, co
   }
   p.omega_c = ctx->desc.omega_c;
   p.strong = ctx->opt_form;
+  p.push_left = mode != 0 ? ctx->push_left : nullptr;
+  p.push_right = mode != 0 ? ctx->push_right : nullptr;
   p.xhalo = ctx->xhalo;
   p.E = E; p.f = f; p.fn = fn; p.out = out; p.c0 = c0; p.c1 = c1; p.dt = dt; p.mode = mode;
   p.dof = (long long)ctx->dof;
@@ -470,6 +472,15 @@ extern "C" int dg_set_xhalo(dg_ctx* ctx, const double* halo_dev) {
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_set_xhalo: field-only context (ndim = 1)");
   if (halo_dev && ((uintptr_t)halo_dev & 15)) return fail(DG_ERR_INVALID_ARG, "dg_set_xhalo: pointer must be 16-byte aligned");
   ctx->xhalo = halo_dev;
+  return DG_OK;
+}
+
+extern "C" int dg_set_xhalo_push(dg_ctx* ctx, double* left_dst_dev, double* right_dst_dev) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_xhalo_push: null context");
+  if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_set_xhalo_push: field-only context (ndim = 1)");
+  if (ctx->desc.bc[0] != DG_BC_HALO) return fail(DG_ERR_INVALID_ARG, "dg_set_xhalo_push: context was not created with bc[0] = DG_BC_HALO");
+  if (((uintptr_t)left_dst_dev & 15) || ((uintptr_t)right_dst_dev & 15)) return fail(DG_ERR_INVALID_ARG, "dg_set_xhalo_push: planes must be 16-byte aligned");
+  ctx->push_left = left_dst_dev; ctx->push_right = right_dst_dev;
   return DG_OK;
 }
 

@@ -50,6 +50,8 @@ struct dg_ctx {
   size_t cbuf_doubles = 0, partials_doubles = 0;
 
   const double* xhalo = nullptr;   // caller-owned exterior x-face planes (bc[0] = DG_BC_HALO)
+  double* push_left = nullptr;     // dg_set_xhalo_push: where dg_rk_stage also stores the first / last x plane of out
+  double* push_right = nullptr;
 
   // library-owned staging for the host entry point
   double* f_stage = nullptr;

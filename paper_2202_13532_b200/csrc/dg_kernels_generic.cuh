@@ -22,6 +22,8 @@ struct GenericParams {
   double* out;
   double c0, c1, dt;        // out = c0*fn + c1*(f + dt*rhs)   (mode 1);   out = rhs (mode 0)
   int mode;
+  double* push_left;        // x-slab face push: plane [G1*G2] in the left neighbour's halo for this slab's first x plane of out
+  double* push_right;       // ... and in the right neighbour's halo for the last x plane (mode 1 only), or nullptr
   int strong;               // 1: strong form Eq. 15 -- ups holds -D and the lift acts on (upwind state - own face value)
   long long dof;
 };
@@ -75,7 +77,10 @@ __global__ void __launch_bounds__(256) rhs_generic_kernel(const GenericParams p)
     if (p.mode == 0) p.out[idx] = rhs;
     else {
       const double v = p.f[idx] + p.dt * rhs;
-      p.out[idx] = (p.fn ? p.c0 * p.fn[idx] : 0.0) + p.c1 * v;
+      const double o = (p.fn ? p.c0 * p.fn[idx] : 0.0) + p.c1 * v;
+      p.out[idx] = o;
+      if (p.push_left && g[0] == 0) p.push_left[idx % strd[0]] = o;
+      if (p.push_right && g[0] == p.G[0] - 1) p.push_right[idx % strd[0]] = o;
     }
   }
 }

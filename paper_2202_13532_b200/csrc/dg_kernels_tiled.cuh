@@ -78,6 +78,8 @@ struct alignas(64) TiledParams {
   CUtensorMap m_fn;      // f_n, box as m_main
   CUtensorMap m_out;     // output, box as m_main
   CUtensorMap m_xhalo;   // exterior x-face planes [2][G1][G2] of an x-slab (bc0 = 2), box (R, NN, 1)
+  CUtensorMap m_pushL;   // plane [G1][G2] in the LEFT x-neighbour's halo buffer: receives this slab's first x plane of out
+  CUtensorMap m_pushR;   // plane [G1][G2] in the RIGHT x-neighbour's halo buffer: receives this slab's last x plane of out
   double pe[NN * NN / 4];
   double qo[NN * NN / 4];
   double la[NN / 2];
@@ -93,6 +95,8 @@ struct alignas(64) TiledParams {
   int N0, N1, N2, G0, G1, G2;
   int bc0, bc1, bc2;
   int tiles_v, mode, has_fn, want_partials;
+  double* push_r_ptr;    // the same plane as m_pushR, for tiles whose last row block is not 128-byte aligned in shared memory
+  int push_l, push_r;    // x-slab face push (dg_set_xhalo_push): store the boundary planes of out into the neighbours' halos
   int strong;            // 1: strong form Eq. 15 -- pe/qo are built from -D and the lift acts on (upwind state - own face value)
 };
 
@@ -385,9 +389,29 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   }
   fence_proxy_async();       // generic-proxy writes to sN must be visible to the TMA store
   __syncthreads();
+  constexpr int ROFF = (NN - 1) * NN * (Cfg::SWZ ? 16 : R);          // last x-node row block of the tile
+  constexpr bool PUSHR_TMA = (ROFF * 8) % 128 == 0;                  // a TMA store needs a 128-byte aligned source
+  if (!PUSHR_TMA && P.push_r && ex == P.N0 - 1) {
+    // n = 10 (R = 20): the block starts at 14 400 B; the NN x R doubles leave by plain stores instead
+    for (int i = t; i < NN * R; i += Cfg::NT) {
+      const int row = i / R, c = i - row * R;
+      if (c0 + c < P.G2) P.push_r_ptr[(size_t)(gu0 + row) * P.G2 + c0 + c] = sN[ROFF + i];
+    }
+  }
   if (t == 0) {
     tma_store_3d(&P.m_out, smem_u32(sN), c0, gu0, gx0);
     if (Cfg::SWZ) tma_store_3d(&P.m_out, smem_u32(sN + Cfg::ROWS * 16), c0 + 16, gu0, gx0);
+    // Fused face-plane exchange of the x-slab sharding: the tiles at the slab's two x faces store their boundary plane of
+    // out a second time, straight into the neighbour's halo buffer (peer memory over NVLink, or the same device) -- the
+    // rows jx = 0 / NN-1 of the tile are contiguous in shared memory in both tile layouts.
+    if (P.push_l && ex == 0) {
+      tma_store_3d(&P.m_pushL, smem_u32(sN), c0, gu0, 0);
+      if (Cfg::SWZ) tma_store_3d(&P.m_pushL, smem_u32(sN + Cfg::ROWS * 16), c0 + 16, gu0, 0);
+    }
+    if (PUSHR_TMA && P.push_r && ex == P.N0 - 1) {
+      tma_store_3d(&P.m_pushR, smem_u32(sN + ROFF), c0, gu0, 0);
+      if (Cfg::SWZ) tma_store_3d(&P.m_pushR, smem_u32(sN + Cfg::ROWS * 16 + ROFF), c0 + 16, gu0, 0);
+    }
     tma_store_commit_and_wait_read();
   }
   if (!Cfg::SHFL_RED && P.want_partials && t >= 32 && t < 32 + NN) {
@@ -467,6 +491,11 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   } else {
     P.m_xhalo = P.m_xface;
   }
+  P.push_l = (mode != 0 && ctx->push_left) ? 1 : 0;
+  P.push_r = (mode != 0 && ctx->push_right) ? 1 : 0;
+  P.m_pushL = P.m_out; P.m_pushR = P.m_out; P.push_r_ptr = ctx->push_right;
+  if (P.push_l && !make_map(&P.m_pushL, ctx->push_left, ctx, RB, NN, 1, Cfg::SWZ, 1)) return DG_ERR_CUDA;
+  if (P.push_r && !make_map(&P.m_pushR, ctx->push_right, ctx, RB, NN, 1, Cfg::SWZ, 1)) return DG_ERR_CUDA;
   const dgsetup::Basis1D& b = ctx->basis[0];
   constexpr int H = NN / 2;
   P.strong = ctx->opt_form;

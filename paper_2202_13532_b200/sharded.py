@@ -14,6 +14,11 @@ whole, so the density moment (Eq. 27) is local.  Per Runge-Kutta s
      read (dg_set_xhalo)
   4. fused RHS + stage combination              (dg_rk_stage, local)
 
+With `push=True` step 3 disappears as a separate operation: every rank's dg_rk_stage stores the two boundary planes of
+its OUTPUT straight into the neighbours' halo buffers from inside the RHS kernel (dg_set_xhalo_push: peer memory over
+NVLink, symmetric-memory allocation), into the buffer of the other parity than the one the running stage reads; the
+all-gather of step 2 is then the only thing that orders the ranks between two stages.
+
 This module is host plumbing only: which planes go where, and in what order the C-ABI calls and the
 torch.distributed calls are issued.  The arithmetic runs behind the `backend` object -- `CudaBackend`
 (libdgvlasov kernels) in the product; there is no CPU backend here, and constructing `CudaBackend`
@@ -79,6 +84,31 @@ class TorchDistComm:
         for work in dist.batch_isend_irecv(ops):
             work.wait()
 
+    def alloc_halos(self, plane_shape, device, periodic: bool):
+        """Ping-pong halo buffers [parity][side][G_u][G_v] for the fused face push, plus views of the two x-neighbours'
+        buffers (None where there is no neighbour).  world == 1: the neighbour is this rank itself.  world > 1: the
+        buffers live in symmetric memory so that every rank can store into its neighbours' over NVLink."""
+        shape = (2, 2) + tuple(plane_shape)
+        r, w = self.rank, self.world
+        if w == 1:
+            own = torch.zeros(shape, dtype=torch.float64, device=device)
+            return own, (own if periodic else None), (own if periodic else None)
+        try:
+            import torch.distributed._symmetric_memory as symm
+        except Exception as e:                                      # pragma: no cover
+            raise RuntimeError("push mode with world > 1 needs torch.distributed._symmetric_memory") from e
+        own = symm.empty(shape, dtype=torch.float64, device=device)
+        own.zero_()
+        hdl = symm.rendezvous(own, self.group if self.group is not None else dist.group.WORLD)
+        left = hdl.get_buffer((r - 1) % w, shape, torch.float64) if (periodic or r > 0) else None
+        right = hdl.get_buffer((r + 1) % w, shape, torch.float64) if (periodic or r < w - 1) else None
+        return own, left, right
+
+    def device_barrier(self, token):
+        """Orders the ranks' streams when no all-gather does (runs without a field solve)."""
+        if self.world > 1:
+            dist.all_reduce(token, group=self.group)
+
     def all_gather_rho(self, rho_loc, counts, out):
         """out[G_x] <- concatenation of every rank's rho (counts[r] nodes each; padded to the longest slab on the wire)."""
         if self.world == 1:
@@ -127,6 +157,9 @@ class CudaBackend:
     def rk_stage(self, f_s, f_n, E_loc, out, c0, c1, dt, rho_out=None):
         return self.slab.rk_stage(f_s, f_n, E_loc, out, c0, c1, dt, rho_out)
 
+    def set_push(self, left_dst, right_dst):
+        self.slab.set_xhalo_push(left_dst, right_dst)
+
     def close(self):
         self.slab.close(); self.field.close()
 
@@ -135,7 +168,7 @@ class XSlabStepper:
     """SSP-RK3 on one x-slab.  `f` is this rank's slab [G_x_local][G_u][G_v] (device tensor for CudaBackend)."""
 
     def __init__(self, nelem, order, lo, hi, bc=None, omega_c=0.0, pmax=0, mass_mode=0, rank=0, world=1, device=0,
-                 backend=None, comm=None):
+                 backend=None, comm=None, push=False):
         ndim = len(nelem)
         self.bc = tuple(bc) if bc is not None else (0,) + (1,) * (ndim - 1)
         self.parts = slab_partition(nelem[0], world)
@@ -150,7 +183,15 @@ class XSlabStepper:
         self.comm = comm if comm is not None else TorchDistComm(rank, world)
         shp = tuple(self.be.flat_shape)
         self.u1, self.u2 = self.be.empty(shp), self.be.empty(shp)
-        self.halo = self.be.empty((2,) + shp[1:])
+        self.push = bool(push)
+        if self.push:
+            # [parity][side][G_u][G_v]; stage number `sidx` reads parity sidx % 2 and pushes into the neighbours' other one
+            self.H, self.H_left, self.H_right = self.comm.alloc_halos(shp[1:], self.u1.device, periodic=(self.bc[0] == 0))
+            self.sidx = 0
+            self.halo = self.H[0]
+            self.token = self.be.empty((1,))
+        else:
+            self.halo = self.be.empty((2,) + shp[1:])
         self.be.set_halo(self.halo)
         self.rho_loc, self.rho = self.be.empty((shp[0],)), self.be.empty((self.G0,))
         self.E = self.be.empty((self.G0,))
@@ -167,9 +208,22 @@ class XSlabStepper:
         return self.E_loc
 
     def stage(self, f_s, f_n, out, c0, c1, dt, self_consistent=True, rho_known=False):
-        """One stage; with self_consistent the density of `out` is left in self.rho_loc for the next stage."""
+        """One stage; with self_consistent the density of `out` is left in self.rho_loc for the next stage.
+        rho_known also says that the previous stage of this stepper produced f_s (push mode: its faces are in the halos)."""
         E = self.field(f_s, rho_known) if self_consistent else None
-        self.comm.exchange_faces(f_s[0], f_s[-1], self.halo, periodic=(self.bc[0] == 0))
+        if self.push:
+            cur, nxt = self.sidx % 2, (self.sidx + 1) % 2
+            self.halo = self.H[cur]
+            if not rho_known:          # f_s did not come from the previous stage: fill this parity by a plain exchange
+                self.comm.exchange_faces(f_s[0], f_s[-1], self.halo, periodic=(self.bc[0] == 0))
+            elif not self_consistent:  # no all-gather between the stages: order the ranks explicitly
+                self.comm.device_barrier(self.token)
+            self.be.set_halo(self.halo)
+            self.be.set_push(None if self.H_left is None else self.H_left[nxt][1],
+                             None if self.H_right is None else self.H_right[nxt][0])
+            self.sidx += 1
+        else:
+            self.comm.exchange_faces(f_s[0], f_s[-1], self.halo, periodic=(self.bc[0] == 0))
         self.be.rk_stage(f_s, f_n if c0 != 0.0 else None, E, out, c0, c1, dt, self.rho_loc if self_consistent else None)
         return out
 

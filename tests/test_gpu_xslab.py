@@ -90,7 +90,8 @@ def test_two_slabs_rhs_and_stage_match_unsharded_oracle(case):
 
 
 @pytest.mark.parametrize("kernel_n", [8, 4])
-def test_sharded_stepper_world1_matches_oracle(kernel_n):
+@pytest.mark.parametrize("push", [False, True])
+def test_sharded_stepper_world1_matches_oracle(kernel_n, push):
     """XSlabStepper with the CUDA backend, world = 1: the periodic wrap goes through the halo planes and the Poisson
     solve through the x-only global context; 3 self-consistent steps against the oracle."""
     from paper_2202_13532_b200 import sharded
@@ -100,19 +101,63 @@ def test_sharded_stepper_world1_matches_oracle(kernel_n):
     lo, hi = (0.0, -8.5, -8.5), (2 * math.pi / k, 8.5, 8.5)
     g = ov.Grid(nelem=nelem, order=order, lo=lo, hi=hi, bc=(0, 1, 1), omega_c=1.0, pmax=4)
     f0 = wl.add_uniform_noise(wl.ring_f0(g.coords[0].reshape(-1), g.coords[1].reshape(-1), g.coords[2].reshape(-1), k), 5, 1e-4)
-    st = sharded.XSlabStepper(nelem, order, lo, hi, bc=(0, 1, 1), omega_c=1.0, pmax=4, rank=0, world=1, device=0)
+    st = sharded.XSlabStepper(nelem, order, lo, hi, bc=(0, 1, 1), omega_c=1.0, pmax=4, rank=0, world=1, device=0, push=push)
     f = dev(f0)
     st.run(f, 5e-4, 3, True)
     fo = f0.copy()
     for _ in range(3):
         fo = ov.ssprk3_step(g, fo, 5e-4)
     assert relerr(f.cpu().numpy(), fo) <= 1e-12
+    # without the field solve (no all-gather between the stages), and single steps (halos primed by a plain exchange)
+    f = dev(f0)
+    st.run(f, 5e-4, 2, False)
+    st.step(f, 5e-4, False)
+    fo = f0.copy()
+    for _ in range(3):
+        fo = ov.ssprk3_step(g, fo, 5e-4, self_consistent=False)
+    assert relerr(f.cpu().numpy(), fo) <= 1e-12
     st.close()
 
 
-def test_two_slab_emulation_steps_match_unsharded_oracle():
-    """Two slabs of unequal size stepped on one GPU, exchange by device copies, rho gathered by concatenation:
-    the data path of a 2-rank run, kernel for kernel, against 2 unsharded oracle steps."""
+@pytest.mark.parametrize("case", [((3, 5, 9), (8, 8, 8), "auto"), ((3, 5, 9), (8, 8, 8), "generic"), ((2, 3, 17), (4, 4, 4), "auto"),
+                                  ((2, 3, 5), (6, 6, 6), "auto"), ((2, 2, 3), (10, 10, 10), "auto")])
+def test_rk_stage_pushes_boundary_planes(case):
+    """dg_set_xhalo_push: the first / last x plane of `out` lands in the given planes bit for bit (swizzled and row-major
+    tiles, ragged last v tile, generic kernel), `out` itself is unchanged, and NULL disables a side."""
+    nelem, order, kernel = case
+    A = api()
+    lo, hi = (0.0, -8.5, -8.5), (2 * math.pi / 0.1, 8.5, 8.5)
+    ctx = A.DGContext(nelem, order, lo, hi, bc=(A.BC_HALO, 1, 1), omega_c=1.0, pmax=1)
+    ctx.set_option(A.OPT_RHS_KERNEL, A.KERNEL_GENERIC if kernel == "generic" else A.KERNEL_AUTO)
+    shape = ctx.flat_shape
+    fs, fn = dev(wl.uniform_field(shape, 51) - 0.3), dev(wl.uniform_field(shape, 52))
+    E = dev(wl.normal_E(shape[0], 53))
+    halo = dev(wl.uniform_field((2,) + shape[1:], 54))
+    ctx.set_xhalo(halo)
+    ref = torch.empty_like(fs)
+    ctx.rk_stage(fs, fn, E, ref, 0.75, 0.25, 1e-3)
+    dst = torch.full((2, 2) + shape[1:], 7.0, dtype=torch.float64, device="cuda")
+    ctx.set_xhalo_push(dst[1][1], dst[0][0])
+    out = torch.empty_like(fs)
+    ctx.rk_stage(fs, fn, E, out, 0.75, 0.25, 1e-3)
+    assert torch.equal(out, ref)
+    assert torch.equal(dst[1][1], ref[0]) and torch.equal(dst[0][0], ref[-1])
+    assert bool((dst[0][1] == 7.0).all()) and bool((dst[1][0] == 7.0).all())
+    dst.fill_(7.0)
+    ctx.set_xhalo_push(None, dst[0][0])
+    ctx.rk_stage(fs, fn, E, out, 0.75, 0.25, 1e-3)
+    assert torch.equal(dst[0][0], ref[-1]) and bool((dst[1] == 7.0).all())
+    dst.fill_(7.0)
+    ctx.rhs(fs, E, out)                                   # the plain RHS never pushes
+    assert bool((dst == 7.0).all())
+    ctx.close()
+
+
+@pytest.mark.parametrize("push", [False, True])
+def test_two_slab_emulation_steps_match_unsharded_oracle(push):
+    """Two slabs of unequal size stepped on one GPU, exchange by device copies (or, push = True, by the RHS kernels storing
+    their boundary planes into the other slab's ping-pong halo buffers), rho gathered by concatenation: the data path
+    of a 2-rank run, kernel for kernel, against 2 unsharded oracle steps."""
     from paper_2202_13532_b200 import sharded
     A = api()
     k = 0.1
@@ -128,16 +173,28 @@ def test_two_slab_emulation_steps_match_unsharded_oracle():
     u1 = [torch.empty_like(x) for x in fs]
     u2 = [torch.empty_like(x) for x in fs]
     halos = [torch.zeros((2,) + x.shape[1:], dtype=torch.float64, device="cuda") for x in fs]
+    H = [torch.zeros((2, 2) + x.shape[1:], dtype=torch.float64, device="cuda") for x in fs]      # [parity][side] per slab
     for be, h in zip(bes, halos):
         be.set_halo(h)
+    sidx = [0]
     rho, E = torch.empty(g.flat_shape[0], dtype=torch.float64, device="cuda"), torch.empty(g.flat_shape[0], dtype=torch.float64, device="cuda")
 
     def stage(src, fn, dst, c0, c1, dt):
         for r, (e0, e1) in enumerate(parts):
             bes[r].density(src[r], rho[e0 * n:e1 * n])
         bes[0].poisson_E(rho, E)
-        for r in range(2):
-            halos[r][0].copy_(src[(r - 1) % 2][-1]); halos[r][1].copy_(src[(r + 1) % 2][0])
+        if push:
+            cur, nxt = sidx[0] % 2, (sidx[0] + 1) % 2
+            if sidx[0] == 0:                               # prime the first parity by a plain exchange
+                for r in range(2):
+                    H[r][0][0].copy_(src[(r - 1) % 2][-1]); H[r][0][1].copy_(src[(r + 1) % 2][0])
+            for r in range(2):
+                bes[r].set_halo(H[r][cur])
+                bes[r].set_push(H[(r - 1) % 2][nxt][1], H[(r + 1) % 2][nxt][0])
+            sidx[0] += 1
+        else:
+            for r in range(2):
+                halos[r][0].copy_(src[(r - 1) % 2][-1]); halos[r][1].copy_(src[(r + 1) % 2][0])
         for r, (e0, e1) in enumerate(parts):
             bes[r].rk_stage(src[r], fn[r] if c0 else None, E[e0 * n:e1 * n].contiguous(), dst[r], c0, c1, dt)
 
