@@ -1,4 +1,4 @@
-"""ctypes loader for libdgvlasov.so -- the C ABI declared in include/dgvlasov.h.
+"""ctypes loader for libdgvlasov.so -- the C ABI declared in include/dgvlasov.h and include/dgvlasov2d2v.h.
 
 There is no fallback: if the library has not been built (python -m paper_2202_13532_b200.build)
 importing the binding raises."""
@@ -21,6 +21,21 @@ class GridDesc(C.Structure):
         ("bc", C.c_int32 * 3),
         ("omega_c", C.c_double),
         ("pmax", C.c_int32),
+        ("mass_mode", C.c_int32),
+        ("device", C.c_int32),
+    ]
+
+
+class GridDesc4(C.Structure):
+    """dg4_grid_desc of include/dgvlasov2d2v.h."""
+    _fields_ = [
+        ("nelem", C.c_int32 * 4),
+        ("order", C.c_int32 * 4),
+        ("lo", C.c_double * 4),
+        ("hi", C.c_double * 4),
+        ("bc", C.c_int32 * 4),
+        ("omega_c", C.c_double),
+        ("pmax", C.c_int32 * 2),
         ("mass_mode", C.c_int32),
         ("device", C.c_int32),
     ]
@@ -60,6 +75,23 @@ SIGNATURES = {
     "dg_last_field_kernel": (C.c_char_p, [_vp]),
     "dg_last_error": (C.c_char_p, []),
     "dg_version": (C.c_char_p, []),
+    # include/dgvlasov2d2v.h
+    "dg4_create": (C.c_int, [C.POINTER(GridDesc4), C.POINTER(_vp)]),
+    "dg4_destroy": (C.c_int, [_vp]),
+    "dg4_workspace_bytes": (C.c_size_t, [_vp]),
+    "dg4_set_workspace": (C.c_int, [_vp, _vp, C.c_size_t]),
+    "dg4_rhs": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "dg4_rk_stage": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _dbl, _vp, _vp]),
+    "dg4_density": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "dg4_fourier_project": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "dg4_poisson_E": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "dg4_ssprk3_run": (C.c_int, [_vp, _vp, _dbl, _i32, _i32, _vp]),
+    "dg4_ssprk3_run_host": (C.c_int, [_vp, _vp, _dbl, _i32, _i32]),
+    "dg4_get_nodes": (C.c_int, [_vp, _i32, _dp]),
+    "dg4_set_option": (C.c_int, [_vp, _i32, _i64]),
+    "dg4_get_profile": (C.c_int, [_vp, _dp, C.POINTER(_i64), _i32]),
+    "dg4_launch_count": (_i64, [_vp]),
+    "dg4_last_kernel": (C.c_char_p, [_vp]),
 }
 
 

@@ -232,3 +232,101 @@ class DGContext:
     @property
     def last_field_kernel(self):
         return _L.dg_last_field_kernel(self._h).decode()
+
+
+OPT4_RHS_KERNEL, OPT4_PROFILE, OPT4_TILE_ORDER = 1, 3, 6
+
+
+class DG4Context:
+    """2D2V variant (include/dgvlasov2d2v.h): dg4_create / dg4_destroy plus one method per C entry point.
+    f: [G_x][G_y][G_u][G_v]; fields and density: [G_x][G_y]."""
+
+    def __init__(self, nelem, order, lo, hi, bc=(0, 0, 1, 1), omega_c=0.0, pmax=(0, 0), mass_mode=0, device=0, workspace=True):
+        d = _lib.GridDesc4()
+        for i in range(4):
+            d.nelem[i], d.order[i], d.lo[i], d.hi[i], d.bc[i] = int(nelem[i]), int(order[i]), float(lo[i]), float(hi[i]), int(bc[i])
+        d.pmax[0], d.pmax[1] = int(pmax[0]), int(pmax[1])
+        d.omega_c, d.mass_mode, d.device = float(omega_c), int(mass_mode), int(device)
+        self._h = C.c_void_p()
+        _check(_L.dg4_create(C.byref(d), C.byref(self._h)), "dg4_create")
+        self.nelem, self.order = tuple(nelem), tuple(order)
+        self.device = torch.device("cuda", device)
+        self.flat_shape = tuple(int(nelem[i]) * int(order[i]) for i in range(4))
+        self.pmax = (int(pmax[0]) or int(nelem[0]), int(pmax[1]) or int(nelem[1]))
+        self._ws = None
+        if workspace:
+            nbytes = _L.dg4_workspace_bytes(self._h)
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            _check(_L.dg4_set_workspace(self._h, base, nbytes), "dg4_set_workspace")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            _L.dg4_destroy(self._h)
+            self._h = C.c_void_p()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _field(self):
+        return torch.empty(self.flat_shape[:2], dtype=torch.float64, device=self.device)
+
+    def rhs(self, f, Ex=None, Ey=None, out=None):
+        out = torch.empty_like(f) if out is None else out
+        _check(_L.dg4_rhs(self._h, _ptr(f), _ptr(Ex), _ptr(Ey), _ptr(out), _stream(self.device)), "dg4_rhs")
+        return out
+
+    def rk_stage(self, f_s, f_n, Ex, Ey, out, c0, c1, dt, rho_out=None):
+        _check(_L.dg4_rk_stage(self._h, _ptr(f_s), _ptr(f_n), _ptr(Ex), _ptr(Ey), _ptr(out), float(c0), float(c1), float(dt),
+                               _ptr(rho_out), _stream(self.device)), "dg4_rk_stage")
+        return out
+
+    def density(self, f, out=None):
+        out = self._field() if out is None else out
+        _check(_L.dg4_density(self._h, _ptr(f), _ptr(out), _stream(self.device)), "dg4_density")
+        return out
+
+    def fourier_project(self, rho, out=None):
+        out = torch.empty((self.pmax[0] + 1, 2 * self.pmax[1] + 1, 2), dtype=torch.float64, device=self.device) if out is None else out
+        _check(_L.dg4_fourier_project(self._h, _ptr(rho), _ptr(out), _stream(self.device)), "dg4_fourier_project")
+        return out
+
+    def poisson_E(self, rho, Ex=None, Ey=None):
+        Ex = self._field() if Ex is None else Ex
+        Ey = self._field() if Ey is None else Ey
+        _check(_L.dg4_poisson_E(self._h, _ptr(rho), _ptr(Ex), _ptr(Ey), _stream(self.device)), "dg4_poisson_E")
+        return Ex, Ey
+
+    def ssprk3_run(self, f, dt, nsteps, self_consistent=True):
+        _check(_L.dg4_ssprk3_run(self._h, _ptr(f), float(dt), int(nsteps), int(bool(self_consistent)), _stream(self.device)), "dg4_ssprk3_run")
+        return f
+
+    def ssprk3_run_host(self, f_host, dt, nsteps, self_consistent=True):
+        p = f_host.ctypes.data if isinstance(f_host, np.ndarray) else f_host.data_ptr()
+        _check(_L.dg4_ssprk3_run_host(self._h, p, float(dt), int(nsteps), int(bool(self_consistent))), "dg4_ssprk3_run_host")
+        return f_host
+
+    def nodes(self, dim):
+        x = np.empty(self.flat_shape[dim])
+        _check(_L.dg4_get_nodes(self._h, dim, x.ctypes.data_as(C.POINTER(C.c_double))), "dg4_get_nodes")
+        return x
+
+    def set_option(self, key, value):
+        _check(_L.dg4_set_option(self._h, int(key), int(value)), "dg4_set_option")
+
+    def get_profile(self, reset=True):
+        ms, cnt = C.c_double(0.0), C.c_int64(0)
+        _check(_L.dg4_get_profile(self._h, C.byref(ms), C.byref(cnt), int(bool(reset))), "dg4_get_profile")
+        return ms.value, cnt.value
+
+    @property
+    def launch_count(self):
+        return int(_L.dg4_launch_count(self._h))
+
+    @property
+    def last_kernel(self):
+        return _L.dg4_last_kernel(self._h).decode()

@@ -23,7 +23,7 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "dgvlasov.h"),
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "dgvlasov.h"), os.path.join(HERE, "..", "include", "dgvlasov2d2v.h"),
                                                                os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 

@@ -712,3 +712,5 @@ extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
 extern "C" int64_t dg_launch_count(const dg_ctx* ctx) { return ctx ? ctx->launches : 0; }
 extern "C" const char* dg_last_kernel(const dg_ctx* ctx) { return ctx ? ctx->last_kernel.c_str() : "none"; }
 extern "C" const char* dg_last_field_kernel(const dg_ctx* ctx) { return ctx ? ctx->last_field_kernel.c_str() : "none"; }
+
+#include "dg4_api.cuh"

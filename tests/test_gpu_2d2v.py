@@ -1,0 +1,172 @@
+"""GPU parity of the 2D2V path (include/dgvlasov2d2v.h) against oracle/vlasov2d2v.py on the same seeded inputs.
+Tolerances as for the 1D2V path: max-norm relative error <= 1e-12 per RHS / density / field
+evaluation, <= 1e-11 after a few RK steps."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import vlasov2d2v as o4      # noqa: E402
+import workloads as wl                   # noqa: E402
+
+LO, HI = (0.0, -1.0, -6.0, -5.5), (2.0 * math.pi, 2.0, 6.0, 5.5)
+
+
+def api():
+    from paper_2202_13532_b200 import api as _api
+    return _api
+
+
+def relerr(a, b):
+    a = np.asarray(a); b = np.asarray(b)
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_pair(N, n, bc=(0, 0, 1, 1), omega_c=0.8, pmax=(0, 0), mass_mode=0, lo=LO, hi=HI):
+    g = o4.make_grid(N, n, lo, hi, bc=bc, omega_c=omega_c, pmax=pmax, mass_mode=mass_mode)
+    ctx = api().DG4Context(N, n, lo, hi, bc=bc, omega_c=omega_c, pmax=pmax, mass_mode=mass_mode)
+    return g, ctx
+
+
+def seeded_inputs(g):
+    dof = int(np.prod(g.flat_shape))
+    f = wl.counter_uniform_chunked(wl.SEED_CFG6_NOISE, dof).reshape(g.flat_shape)
+    gxy = g.flat_shape[0] * g.flat_shape[1]
+    E = 0.5 * wl.counter_normal(wl.SEED_CFG6_E, 0, 2 * gxy)
+    return f, E[:gxy].reshape(g.flat_shape[:2]), E[gxy:].reshape(g.flat_shape[:2])
+
+
+# (N, n): generic kernel for mixed orders, tiled kernel <2>, <4>, <8> for n = 4 (several tiles + zero-inflow / periodic edges)
+SHAPES = [((3, 2, 3, 4), (3, 4, 5, 2)), ((2, 3, 2, 3), (4, 4, 4, 4)), ((3, 2, 3, 2), (4, 4, 4, 4)), ((2, 3, 3, 4), (4, 4, 4, 4)),
+          ((3, 2, 2, 8), (4, 4, 4, 4)), ((2, 2, 3, 16), (4, 4, 4, 4)), ((2, 2, 2, 2), (6, 6, 6, 6))]
+
+
+@pytest.mark.parametrize("N,n", SHAPES)
+@pytest.mark.parametrize("bc", [(0, 0, 1, 1), (0, 0, 0, 0), (1, 1, 1, 1)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_rhs_matches_oracle(N, n, bc, mode):
+    g, ctx = make_pair(N, n, bc=bc, mass_mode=mode)
+    f, Ex, Ey = seeded_inputs(g)
+    r = ctx.rhs(dev(f), dev(Ex), dev(Ey)).cpu().numpy()
+    ro = o4.rhs(g, f, Ex, Ey)
+    assert relerr(r, ro) < 1e-12, ctx.last_kernel
+    expect_tiled = all(k == 4 for k in n) and N[3] % 2 == 0
+    assert ctx.last_kernel.startswith("rhs4_tile" if expect_tiled else "rhs4_generic")
+    ctx.close()
+
+
+@pytest.mark.parametrize("order", [1, 2])
+def test_tiled_equals_generic_kernel_and_tile_orders(order):
+    g, ctx = make_pair((10, 3, 3, 8), (4, 4, 4, 4))
+    f, Ex, Ey = seeded_inputs(g)
+    fd, exd, eyd = dev(f), dev(Ex), dev(Ey)
+    ctx.set_option(api().OPT4_TILE_ORDER, order)
+    a = ctx.rhs(fd, exd, eyd).cpu().numpy()
+    assert ctx.last_kernel == "rhs4_tile<8>"
+    ctx.set_option(api().OPT4_RHS_KERNEL, 1)
+    b = ctx.rhs(fd, exd, eyd).cpu().numpy()
+    assert ctx.last_kernel == "rhs4_generic"
+    assert relerr(a, b) < 1e-13
+    assert relerr(a, o4.rhs(g, f, Ex, Ey)) < 1e-12
+    ctx.close()
+
+
+def test_rhs_without_field_and_zero_speed_nodes():
+    """E = NULL; an even number of velocity elements puts nodes at u = 0, v = 0 (zero flux there, Eq. 23)."""
+    g, ctx = make_pair((2, 2, 4, 8), (4, 4, 4, 4), omega_c=0.0, lo=(0, 0, -2, -2), hi=(1, 1, 2, 2))
+    f, _, _ = seeded_inputs(g)
+    r = ctx.rhs(dev(f)).cpu().numpy()
+    assert relerr(r, o4.rhs(g, f)) < 1e-12
+    ctx.close()
+
+
+@pytest.mark.parametrize("N,n", [((3, 2, 3, 4), (3, 4, 5, 2)), ((2, 3, 3, 8), (4, 4, 4, 4)), ((2, 2, 5, 3), (4, 4, 4, 5))])
+def test_density_matches_oracle(N, n):
+    g, ctx = make_pair(N, n)
+    f, _, _ = seeded_inputs(g)
+    rho = ctx.density(dev(f)).cpu().numpy()
+    assert relerr(rho, o4.density(g, f)) < 1e-13
+    ctx.close()
+
+
+@pytest.mark.parametrize("N,n,pmax", [((8, 6, 1, 1), (8, 8, 2, 2), (5, 4)), ((5, 7, 1, 1), (4, 6, 2, 2), (0, 0)), ((16, 16, 1, 1), (4, 4, 2, 2), (16, 16))])
+def test_projection_and_field_match_oracle(N, n, pmax):
+    g, ctx = make_pair(N, n, pmax=pmax, lo=(0.0, 1.0, -1, -1), hi=(2 * math.pi, 4.0, 1, 1))
+    x, y = g.coords[0].reshape(-1), g.coords[1].reshape(-1)
+    rng_u = wl.counter_uniform(wl.SEED_CFG6_E, 0, 64)
+    rho = np.ones((x.size, y.size))
+    for i in range(8):                                     # seeded sum of plane waves + noise
+        p, q = 1 + int(rng_u[4 * i] * 3), int(rng_u[4 * i + 1] * 7) - 3
+        rho += 0.05 * rng_u[4 * i + 2] * np.cos(p * x[:, None] + 2 * math.pi * q / 3.0 * y[None, :] + 6.28 * rng_u[4 * i + 3])
+    rho += 1e-3 * wl.counter_normal(wl.SEED_CFG6_NOISE, 0, rho.size).reshape(rho.shape)
+    c = ctx.fourier_project(dev(rho)).cpu().numpy()
+    co = o4.fourier_project(g, rho)
+    assert relerr(c[..., 0] + 1j * c[..., 1], co) < 1e-12
+    Ex, Ey = ctx.poisson_E(dev(rho))
+    Exo, Eyo = o4.poisson_E(g, co)
+    scale = max(np.max(np.abs(Exo)), np.max(np.abs(Eyo)))
+    assert np.max(np.abs(Ex.cpu().numpy() - Exo)) < 1e-12 * scale + 1e-14      # reading C26: rho carries the mean 1
+    assert np.max(np.abs(Ey.cpu().numpy() - Eyo)) < 1e-12 * scale + 1e-14
+    ctx.close()
+
+
+def test_plane_wave_field_closed_form():
+    g, ctx = make_pair((8, 8, 1, 1), (8, 8, 2, 2), pmax=(3, 3), lo=(0.0, 0.0, -1, -1), hi=(2 * math.pi, 3.0, 1, 1))
+    x, y = ctx.nodes(0), ctx.nodes(1)
+    kx, ky = 2.0, -2 * math.pi / 3.0
+    arg = kx * x[:, None] + ky * y[None, :] + 0.3
+    Ex, Ey = ctx.poisson_E(dev(1.0 + 0.05 * np.cos(arg)))
+    k2 = kx * kx + ky * ky
+    assert np.max(np.abs(Ex.cpu().numpy() + 0.05 * kx / k2 * np.sin(arg))) < 1e-11
+    assert np.max(np.abs(Ey.cpu().numpy() + 0.05 * ky / k2 * np.sin(arg))) < 1e-11
+    ctx.close()
+
+
+@pytest.mark.parametrize("N,n", [((3, 2, 3, 8), (4, 4, 4, 4)), ((2, 2, 3, 2), (3, 4, 4, 3))])
+def test_self_consistent_steps_match_oracle(N, n):
+    """Ring workload, three SSP-RK3 steps with the 2-D Poisson solve at every stage (density partials from the tile epilogue)."""
+    g, ctx = make_pair(N, n, omega_c=1.0, lo=(0.0, 0.0, -8.5, -8.5), hi=(20 * math.pi, 10 * math.pi, 8.5, 8.5))
+    x, y, u, v = [c.reshape(-1) for c in g.coords]
+    f = wl.ring2d_f0(x, y, u, v, 0.1, 0.2)
+    f = wl.add_uniform_noise(f, wl.SEED_CFG6_NOISE, 1e-4)
+    dt = 2e-3
+    fo = f.copy()
+    for _ in range(3):
+        fo = o4.ssprk3_step(g, fo, dt)
+    fd = ctx.ssprk3_run(dev(f), dt, 3).cpu().numpy()
+    assert relerr(fd, fo) < 1e-11
+    fh = f.copy()
+    ctx.ssprk3_run_host(fh, dt, 3)
+    assert np.array_equal(fh, fd)
+    ctx.close()
+
+
+def test_rk_stage_density_output():
+    g, ctx = make_pair((2, 2, 3, 8), (4, 4, 4, 4), bc=(0, 0, 0, 0))
+    f, Ex, Ey = seeded_inputs(g)
+    fd = dev(f)
+    out, rho = torch.empty_like(fd), torch.empty(g.flat_shape[:2], dtype=torch.float64, device="cuda")
+    ctx.rk_stage(fd, fd, dev(Ex), dev(Ey), out, 0.75, 0.25, 1e-3, rho_out=rho)
+    oo = 0.75 * f + 0.25 * (f + 1e-3 * o4.rhs(g, f, Ex, Ey))
+    assert relerr(out.cpu().numpy(), oo) < 1e-13
+    assert relerr(rho.cpu().numpy(), o4.density(g, oo)) < 1e-13
+    ctx.close()
+
+
+def test_errors():
+    a = api()
+    with pytest.raises(a.DGError):
+        a.DG4Context((2, 2, 2, 2), (4, 4, 4, 11), LO, HI)
+    ctx = a.DG4Context((2, 2, 2, 3), (4, 4, 4, 4), LO, HI)
+    ctx.set_option(a.OPT4_RHS_KERNEL, 2)
+    f = torch.zeros(ctx.flat_shape, dtype=torch.float64, device="cuda")
+    with pytest.raises(a.DGError):
+        ctx.rhs(f)                     # odd N_v: no tiled kernel
+    ctx.close()

@@ -24,6 +24,8 @@ SEED_CFG3_NOISE = 0xD60003
 SEED_CFG4_F = 0xD60004
 SEED_CFG4_E = 0xD61004
 SEED_CFG5 = 0xD60005
+SEED_CFG6_NOISE = 0xD60006      # 2D2V workload
+SEED_CFG6_E = 0xD61006
 
 
 def counter_uniform(seed: int, start: int, count: int) -> np.ndarray:
@@ -70,6 +72,16 @@ def ring_f0(x: np.ndarray, vx: np.ndarray, vy: np.ndarray, k: float, amp: float 
     s = v2 / (2.0 * alpha * alpha)
     ring = s ** j * np.exp(-s) / (2.0 * math.pi * alpha * alpha * math.factorial(j))
     return (1.0 + amp * np.sin(k * x))[:, None, None] * ring[None, :, :]
+
+
+def ring2d_f0(x: np.ndarray, y: np.ndarray, vx: np.ndarray, vy: np.ndarray, kx: float, ky: float, amp: float = 0.01,
+              j: int = 3, alpha: float = 1.0) -> np.ndarray:
+    """2D2V workload: the ring distribution of Eq. 31 times (1 + amp sin(kx x) + amp cos(ky y)), [len(x), len(y), len(vx), len(vy)]."""
+    v2 = (vx * vx)[:, None] + (vy * vy)[None, :]
+    s = v2 / (2.0 * alpha * alpha)
+    ring = s ** j * np.exp(-s) / (2.0 * math.pi * alpha * alpha * math.factorial(j))
+    space = 1.0 + amp * np.sin(kx * x)[:, None] + amp * np.cos(ky * y)[None, :]
+    return space[:, :, None, None] * ring[None, None, :, :]
 
 
 def add_uniform_noise(f: np.ndarray, seed: int, amp: float) -> np.ndarray:
