@@ -375,6 +375,71 @@ def run_config4(args, name):
     ctx.close()
 
 
+CONFIG6 = {"config6_2d2v_128^4": 32, "config6_2d2v_64^4": 16}
+
+
+def run_config6(args, name):
+    """2D2V: N^4 elements x 4^4 LGL nodes, ring workload in (v_x, v_y) with a seeded perturbation in x and y,
+    one SSP-RK3 step with the 2-D Poisson solve at every stage (dg4_ssprk3_run)."""
+    import torch
+    import workloads as wl
+    from paper_2202_13532_b200 import api
+    N = CONFIG6[name]
+    lo, hi = (0.0, 0.0, -8.5, -8.5), (2 * math.pi / K_WAVE, 2 * math.pi / K_WAVE, 8.5, 8.5)
+    ctx = api.DG4Context((N,) * 4, (4,) * 4, lo, hi, bc=(0, 0, 1, 1), omega_c=1.0)
+    x, y, u, v = (ctx.nodes(d) for d in range(4))
+    f0 = wl.add_uniform_noise(wl.ring2d_f0(x, y, u, v, K_WAVE, K_WAVE), wl.SEED_CFG6_NOISE, 1e-4)
+    f = torch.from_numpy(f0).cuda()
+    dt = 2e-4
+    ctx.ssprk3_run(f, dt, max(args.warmup, 3))
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0); sampler.start(); sampler.wait_ready()
+    l0 = ctx.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.mark_begin()
+    e0.record()
+    ctx.ssprk3_run(f, dt, args.steps)
+    e1.record()
+    torch.cuda.synchronize()
+    sampler.mark_end()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = ctx.launch_count - l0
+    finite = bool(torch.isfinite(f).all().item())
+    # per-launch time of the RHS kernel: events recorded by the library around each launch, in a separate pass
+    ctx.set_option(api.OPT4_PROFILE, 1)
+    ctx.get_profile(reset=True)
+    ctx.ssprk3_run(f, dt, 10)
+    rhs_ms, rhs_n = ctx.get_profile(reset=True)
+    ctx.set_option(api.OPT4_PROFILE, 0)
+    dof = (4 * N) ** 4
+    peak, peak_src = measured_peak_hbm()
+    bytes_per_launch = 64.0 / 3.0 * dof
+    achieved = bytes_per_launch / (rhs_ms / rhs_n * 1e-3) / 1e9
+    # end to end through dg4_ssprk3_run_host
+    fh = torch.from_numpy(f0).pin_memory()
+    ctx.ssprk3_run_host(fh, dt, 1)
+    t0 = time.perf_counter()
+    e2e_steps = 2
+    for _ in range(e2e_steps):
+        ctx.ssprk3_run_host(fh, dt, 1)
+    e2e_s = time.perf_counter() - t0
+    print(json.dumps({
+        "metric": "FP64 phase-space DOF-updates/s per RK stage", "value": dof * 3.0 * args.steps / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "grid": "x".join([str(4 * N)] * 4), "dof": dof, "dt": dt, "self_consistent_poisson_each_stage": True,
+                   "l2": "arrays (3 x %.2f GB) larger than L2" % (dof * 8 / 1e9), "finite": finite},
+        "clocks": clocks, "gpu_launches": launches,
+        "e2e": {"value": dof * 3.0 * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": dof * 8, "d2h_bytes_per_step": dof * 8,
+                "steps": e2e_steps, "api": "dg4_ssprk3_run_host (pinned host buffer)"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "kernel": ctx.last_kernel, "avg_launch_ms": rhs_ms / rhs_n, "launches_timed": rhs_n,
+                     "algorithmic_bytes_per_launch": bytes_per_launch, "peak_source": peak_src,
+                     "rhs_share_of_step": 3.0 * (rhs_ms / rhs_n) / (ms / args.steps)}}), flush=True)
+    ctx.close()
+
+
 def run_config5(args, name):
     """DG->Fourier projection + spectral Poisson solve alone: 2048 x 8 x-nodes, batch 4096, modes <= 8192."""
     import torch
@@ -444,7 +509,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config3_1d2v_512^3", choices=sorted(WORKLOADS) + sorted(CONFIG4) + ["config5_field"])
+    ap.add_argument("--workload", default="config3_1d2v_512^3", choices=sorted(WORKLOADS) + sorted(CONFIG4) + ["config5_field"] + sorted(CONFIG6))
     ap.add_argument("--batch", type=int, default=4096, help="config5_field only")
     ap.add_argument("--field-kernel", default="auto", choices=["auto", "dmma", "dfma", "fft"], help="config5_field only")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "xslab", "xslab-push"],
@@ -457,6 +522,8 @@ def main():
         return run_config4(args, args.workload)
     if args.workload == "config5_field":
         return run_config5(args, args.workload)
+    if args.workload in CONFIG6:
+        return run_config6(args, args.workload)
     w = WORKLOADS[args.workload]
     if args.impl == "reference":
         run_reference(args, w, args.workload)

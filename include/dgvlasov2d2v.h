@@ -71,7 +71,6 @@ int dg4_ssprk3_run_host(dg4_ctx* ctx, double* f_host, double dt, int32_t nsteps,
 int dg4_get_nodes(const dg4_ctx* ctx, int32_t dim, double* coords_host /*[N_d*n_d]*/);
 #define DG4_OPT_RHS_KERNEL 1   /* 0 auto (tiled when all orders are 4 and N_v is even), 1 generic, 2 tiled (error if unsupported) */
 #define DG4_OPT_PROFILE    3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
-#define DG4_OPT_TILE_ORDER 6   /* rasterisation of the tiles over the grid of CTAs: 0 auto, 1 row-major (v fastest), 2 blocked */
 int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value);
 int dg4_get_profile(dg4_ctx* ctx, double* rhs_ms_total_host, int64_t* rhs_launches_host, int32_t reset);
 int64_t dg4_launch_count(const dg4_ctx* ctx);

@@ -234,7 +234,7 @@ class DGContext:
         return _L.dg_last_field_kernel(self._h).decode()
 
 
-OPT4_RHS_KERNEL, OPT4_PROFILE, OPT4_TILE_ORDER = 1, 3, 6
+OPT4_RHS_KERNEL, OPT4_PROFILE = 1, 3
 
 
 class DG4Context:

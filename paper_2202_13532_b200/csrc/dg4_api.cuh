@@ -24,7 +24,8 @@ struct dg4_ctx {
   size_t partials_doubles = 0;
   double* f_stage = nullptr;
   int64_t launches = 0;
-  int opt_kernel = 0, opt_profile = 0, opt_order = 0;
+  int opt_kernel = 0, opt_profile = 0;
+  bool smem_attr_done = false;
   std::vector<cudaEvent_t> prof_events;
   double prof_ms = 0.0;
   int64_t prof_launches = 0;
@@ -220,16 +221,19 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
       p.partials = ctx->partials;
       if (chunks_out) *chunks_out = p.chunks;
     }
-    // rasterisation: blocked in x once an x-element slab no longer fits comfortably in the 126 MB L2
-    int order = ctx->opt_order;
-    if (order == 0) order = ((double)ctx->dof / ctx->N[0] * 8.0 * 2.0 > 48e6) ? 2 : 1;
-    p.order_mode = order == 1 ? 1 : (ctx->N[0] >= 8 ? 8 : ctx->N[0]);
-    const long long tiles = (long long)ctx->N[0] * ctx->N[1] * ctx->N[2] * nvb;
-    if (tiles > 2147483647LL) return fail(DG_ERR_UNSUPPORTED, "dg4: too many tiles for one grid");
-    const size_t smem = (size_t)2 * 64 * 4 * kv * sizeof(double);
-    if (kv == 8) dg4::rhs4_tile_kernel<8><<<(unsigned)tiles, 128, smem, st>>>(p);
-    else if (kv == 4) dg4::rhs4_tile_kernel<4><<<(unsigned)tiles, 64, smem, st>>>(p);
-    else dg4::rhs4_tile_kernel<2><<<(unsigned)tiles, 32, smem, st>>>(p);
+    if (ctx->N[1] > 65535 || ctx->N[0] > 65535) return fail(DG_ERR_UNSUPPORTED, "dg4: more than 65535 elements in x or y");
+    const dim3 tiles(ctx->N[2] * nvb, ctx->N[1], ctx->N[0]);
+    const bool with_fn = mode != 0 && fn != nullptr;
+    const size_t smem = sizeof(double) * (kv == 8 ? dg4::tile_smem_doubles<8>(with_fn) : kv == 4 ? dg4::tile_smem_doubles<4>(with_fn)
+                                                                                              : dg4::tile_smem_doubles<2>(with_fn));
+    if (kv == 8 && !ctx->smem_attr_done) {
+      CUDA_TRY(cudaFuncSetAttribute(dg4::rhs4_tile_kernel<8, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(double) * dg4::tile_smem_doubles<8>(true))));
+      ctx->smem_attr_done = true;
+    }
+    if (kv == 8) dg4::rhs4_tile_kernel<8, 3><<<tiles, 128, smem, st>>>(p);
+    else if (kv == 4) dg4::rhs4_tile_kernel<4, 1><<<tiles, 64, smem, st>>>(p);
+    else dg4::rhs4_tile_kernel<2, 1><<<tiles, 32, smem, st>>>(p);
     ctx->last_kernel = kv == 8 ? "rhs4_tile<8>" : (kv == 4 ? "rhs4_tile<4>" : "rhs4_tile<2>");
     return check4(ctx, "rhs4_tile_kernel");
   }
@@ -404,7 +408,6 @@ extern "C" int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_set_option: null context");
   if (key == DG4_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_kernel = (int)value; return DG_OK; }
   if (key == DG4_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
-  if (key == DG4_OPT_TILE_ORDER && value >= 0 && value <= 2) { ctx->opt_order = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg4_set_option: unknown key or value");
 }
 

@@ -24,7 +24,6 @@ struct Params {
   const double* wqv;
   double* partials;          // [G0*G1][chunks] per-tile density partials of out, or nullptr
   int chunks;
-  int order_mode;            // tile rasterisation
   long long dof;
 };
 

@@ -1,16 +1,18 @@
 // 2D2V tiled RHS + stage kernel for n = 4 LGL nodes in all four dimensions (sm_100a).
 //
 // Tile = one (x, y, u) element x KV v-elements = 4 x 4 x 4 x (4 KV) nodes: 64 rows of R = 4 KV contiguous doubles
-// (KV = 8: 256-byte rows, 16 KB).  One CTA of 16 KV threads per tile; shared memory holds the f_s tile and a tile of partial
-// sums (2 x 16 KB), so 7 CTAs are resident per SM and the loads of one overlap the arithmetic of the others.
-//   fill    cp.async (16 bytes per request, L2 only) of the 64 rows, chunk-swizzled so that both phases below are
-//           bank-conflict free; the upwind x / y face values of phase A are fetched into registers meanwhile.
+// (KV = 8: 256-byte rows, 16 KB).  One CTA of 16 KV threads per tile.
+//   fill    EVERY global read of the CTA is a cp.async into shared memory issued at the top of the kernel -- the f_s tile
+//           and the f_n tile (16 bytes per request, chunk-swizzled so that both phases below are bank-conflict free), the
+//           upwind x / y face values of phase A (8 bytes per request, only the side the sign of u / v selects), both u-face
+//           rows and the two tile-edge v faces of phase B -- followed by ONE wait: a CTA pays the memory latency once and
+//           holds nothing in registers across it; 3 (stages with f_n, 66 KB) or 4 (50 KB) CTAs per SM overlap each other.
 //   phase A thread = (u node, v node of the tile) owns the 4 x 4 (x, y) nodes above it: x and y contractions + lifts in
 //           registers (the speeds a_x = u, a_y = v are per-thread constants), partial sums to shared memory.
 //   phase B thread = (x node, y node, v element) owns the 4 x 4 (u, v) nodes of that element: u and v contractions + lifts;
-//           v-face neighbours inside the tile come from the adjacent lanes by warp shuffle, the two tile-edge faces and the
-//           u faces from global memory (L2: the neighbouring tiles are a few CTAs away); stage combination, 128-bit stores;
-//           LGL-weighted sum of the 16 outputs, reduced over the KV lanes -> one density partial per (g_x, g_y, tile).
+//           v-face neighbours inside the tile come from the adjacent lanes by warp shuffle; stage combination, 128-bit
+//           stores; LGL-weighted sum of the 16 outputs, reduced over the KV lanes -> one density partial per
+//           (g_x, g_y, tile).
 // f is read once and written once per stage from HBM; every operator coefficient is a kernel-parameter constant.
 #pragma once
 #include "dg4_kernels.cuh"
@@ -24,61 +26,61 @@ __device__ __forceinline__ int swz(int row, int chunk) {      // 16-byte chunk p
   return chunk;
 }
 
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
 
-// Tile rasterisation.  Row-major (v fastest, x slowest) puts a whole x-element slab (G_y G_u G_v n doubles) between a tile
-// and its x neighbour -- more than the L2 holds on large grids, so every x-face value would come from HBM a second time.
-// Blocked: x elements in groups of BX, inside a group (y, u, x, v-block) row-major -> the x neighbour is N_v/KV tiles away,
-// the y neighbour N_u BX N_v/KV tiles.
-__device__ __forceinline__ void decode_tile(const Params& p, int nvb, long long t, int& ex, int& ey, int& eu, int& evb) {
-  if (p.order_mode <= 1) {
-    evb = (int)(t % nvb); t /= nvb;
-    eu = (int)(t % p.N[2]); t /= p.N[2];
-    ey = (int)(t % p.N[1]); t /= p.N[1];
-    ex = (int)t;
-  } else {
-    const int BX = p.order_mode;
-    const long long per_group = (long long)p.N[1] * p.N[2] * BX * nvb;
-    const int xb = (int)(t / per_group);
-    t -= xb * per_group;
-    const int bx = min(BX, p.N[0] - xb * BX);          // the last group may be narrower
-    evb = (int)(t % nvb); t /= nvb;
-    const int xi = (int)(t % bx); t /= bx;
-    eu = (int)(t % p.N[2]); t /= p.N[2];
-    ey = (int)t;
-    ex = xb * BX + xi;
-  }
-}
-
+// Shared memory (doubles): f_s tile 64 R | partial sums 64 R | x faces 4 NT | y faces 4 NT | u faces 8 NT | v edge faces 128 |
+// f_n tile 64 R (only when the stage has an f_n).
 template <int KV>
-__global__ void __launch_bounds__(16 * KV) rhs4_tile_kernel(const Params p) {
+constexpr int tile_smem_doubles(bool with_fn) { return (with_fn ? 3 : 2) * 64 * 4 * KV + 16 * (16 * KV) + 128; }
+
+template <int KV, int MINB>
+__global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p) {
   constexpr int R = 4 * KV, ROWS = 64, NT = 16 * KV, HC = R / 2;
   extern __shared__ double2 smem_raw[];
   double* tile = reinterpret_cast<double*>(smem_raw);
   double* accT = tile + ROWS * R;
+  double* hXs = accT + ROWS * R;          // [jy][tid]
+  double* hYs = hXs + 4 * NT;             // [jx][tid]
+  double* hUs = hYs + 4 * NT;             // double2 [lo0, lo1, hi0, hi1][tid]
+  double* eVs = hUs + 8 * NT;             // [side][row]
+  double* fnT = eVs + 128;
+  // grid = (N_u * N_v/KV, N_y, N_x): consecutive CTAs walk v, then u -- the u and v neighbours of a tile are in flight with it
   const int nvb = p.N[3] / KV;
-  int ex, ey, eu, evb;
-  decode_tile(p, nvb, blockIdx.x, ex, ey, eu, evb);
+  const int eu = blockIdx.x / nvb, evb = blockIdx.x - eu * nvb, ey = blockIdx.y, ex = blockIdx.z;
   const int gx0 = ex * 4, gy0 = ey * 4, gu0 = eu * 4, gv0 = evb * R;
   const long long s2 = p.G[3], s1 = s2 * p.G[2], s0 = s1 * p.G[1];
   const int tid = threadIdx.x;
-
-  // ---- fill -------------------------------------------------------------------------------------------------------
-#pragma unroll
-  for (int t = tid; t < ROWS * HC; t += NT) {
-    const int row = t / HC, ch = t % HC;
-    const int jx = row >> 4, jy = (row >> 2) & 3, ju = row & 3;
-    const double* src = p.f + (gx0 + jx) * s0 + (gy0 + jy) * s1 + (gu0 + ju) * s2 + gv0 + 2 * ch;
-    cp_async16(tile + row * R + swz<KV>(row, ch) * 2, src);
-  }
-  asm volatile("cp.async.commit_group;" ::: "memory");
-
-  // ---- phase A: upwind x / y face values while the tile is in flight -----------------------------------------------
+  const bool use_fn = p.mode != 0 && p.fn != nullptr;
+  // phase A / phase B coordinates of this thread
   const int ju_a = tid / R, rv = tid % R;
+  const int ev = tid % KV, jy_b = (tid / KV) & 3, jx_b = tid / (4 * KV);
+  const int gx = gx0 + jx_b, gy = gy0 + jy_b;
+  const long long xy = gx * s0 + gy * s1;
+  const long long gxy = (long long)gx * p.G[1] + gy;
+  const int gvb = gv0 + ev * 4;                                   // first v node of this thread's element (phase B)
   const double ax = p.coord[2][gu0 + ju_a], ay = p.coord[3][gv0 + rv];
-  double hX[4] = {0.0, 0.0, 0.0, 0.0}, hY[4] = {0.0, 0.0, 0.0, 0.0};
+
+  // ---- all global reads, asynchronously ---------------------------------------------------------------------------
+  // tile rows: pass i of the CTA covers rows r0 + 8 i (NT / HC = 8 rows per pass): jx = i / 2, jy = r0 / 4 + 2 (i % 2), ju = r0 % 4
+  const long long tile_off = gx0 * s0 + gy0 * s1 + gu0 * s2 + gv0;
+  const int r0 = tid / HC, ch = tid % HC;
+  const long long fill_off = tile_off + (r0 >> 2) * s1 + (r0 & 3) * s2 + 2 * ch;
+  const int fill_dst = r0 * R + swz<KV>(r0, ch) * 2;           // swz(r0 + 8 i, ch) = swz(r0, ch)
+  {
+    const double* src = p.f + fill_off;
+#pragma unroll
+    for (int jx = 0; jx < 4; ++jx) {
+      cp_async16(tile + fill_dst + (16 * jx) * R, src);
+      cp_async16(tile + fill_dst + (16 * jx + 8) * R, src + 2 * s1);
+      src += s0;
+    }
+  }
   {
     const long long uv = (long long)(gu0 + ju_a) * s2 + gv0 + rv;
     int hx = -1, hy = -1;
@@ -86,18 +88,63 @@ __global__ void __launch_bounds__(16 * KV) rhs4_tile_kernel(const Params p) {
     else if (ax < 0.0) hx = ex < p.N[0] - 1 ? gx0 + 4 : (p.bc[0] == 0 ? 0 : -1);
     if (ay > 0.0) hy = ey > 0 ? gy0 - 1 : (p.bc[1] == 0 ? p.G[1] - 1 : -1);
     else if (ay < 0.0) hy = ey < p.N[1] - 1 ? gy0 + 4 : (p.bc[1] == 0 ? 0 : -1);
-    if (hx >= 0) {
+    const double* px = p.f + hx * s0 + gy0 * s1 + uv;
+    const double* py = p.f + gx0 * s0 + hy * s1 + uv;
 #pragma unroll
-      for (int jy = 0; jy < 4; ++jy) hX[jy] = __ldg(p.f + hx * s0 + (gy0 + jy) * s1 + uv);
+    for (int j = 0; j < 4; ++j) {
+      if (hx >= 0) cp_async8(hXs + j * NT + tid, px);
+      else hXs[j * NT + tid] = 0.0;
+      if (hy >= 0) cp_async8(hYs + j * NT + tid, py);
+      else hYs[j * NT + tid] = 0.0;
+      px += s1; py += s0;
     }
-    if (hy >= 0) {
+  }
+  {
+    const int lo = eu > 0 ? gu0 - 1 : (p.bc[2] == 0 ? p.G[2] - 1 : -1);
+    const int hi = eu < p.N[2] - 1 ? gu0 + 4 : (p.bc[2] == 0 ? 0 : -1);
+    double2* h2 = reinterpret_cast<double2*>(hUs);
+    if (lo >= 0) {
+      cp_async16(h2 + tid, p.f + xy + lo * s2 + gvb);
+      cp_async16(h2 + NT + tid, p.f + xy + lo * s2 + gvb + 2);
+    } else { h2[tid] = make_double2(0.0, 0.0); h2[NT + tid] = make_double2(0.0, 0.0); }
+    if (hi >= 0) {
+      cp_async16(h2 + 2 * NT + tid, p.f + xy + hi * s2 + gvb);
+      cp_async16(h2 + 3 * NT + tid, p.f + xy + hi * s2 + gvb + 2);
+    } else { h2[2 * NT + tid] = make_double2(0.0, 0.0); h2[3 * NT + tid] = make_double2(0.0, 0.0); }
+  }
+  {
+    const int vlo = evb > 0 ? gv0 - 1 : (p.bc[3] == 0 ? p.G[3] - 1 : -1);
+    const int vhi = evb < nvb - 1 ? gv0 + R : (p.bc[3] == 0 ? 0 : -1);
 #pragma unroll
-      for (int jx = 0; jx < 4; ++jx) hY[jx] = __ldg(p.f + (gx0 + jx) * s0 + hy * s1 + uv);
+    for (int t = tid; t < 128; t += NT) {
+      const int side = t >> 6, row = t & 63;
+      const int vv = side == 0 ? vlo : vhi;
+      if (vv >= 0) cp_async8(eVs + t, p.f + tile_off - gv0 + (row >> 4) * s0 + ((row >> 2) & 3) * s1 + (row & 3) * s2 + vv);
+      else eVs[t] = 0.0;
     }
+  }
+  if (use_fn) {
+    const double* src = p.fn + fill_off;
+#pragma unroll
+    for (int jx = 0; jx < 4; ++jx) {
+      cp_async16(fnT + fill_dst + (16 * jx) * R, src);
+      cp_async16(fnT + fill_dst + (16 * jx + 8) * R, src + 2 * s1);
+      src += s0;
+    }
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  const double exf = p.Ex ? __ldg(p.Ex + gxy) : 0.0, eyf = p.Ey ? __ldg(p.Ey + gxy) : 0.0;
+  double au[4], av[4];
+  {
+    const double2 v01 = *reinterpret_cast<const double2*>(p.coord[3] + gvb), v23 = *reinterpret_cast<const double2*>(p.coord[3] + gvb + 2);
+    const double2 u01 = *reinterpret_cast<const double2*>(p.coord[2] + gu0), u23 = *reinterpret_cast<const double2*>(p.coord[2] + gu0 + 2);
+    au[0] = -exf - p.omega_c * v01.x; au[1] = -exf - p.omega_c * v01.y; au[2] = -exf - p.omega_c * v23.x; au[3] = -exf - p.omega_c * v23.y;
+    av[0] = -eyf + p.omega_c * u01.x; av[1] = -eyf + p.omega_c * u01.y; av[2] = -eyf + p.omega_c * u23.x; av[3] = -eyf + p.omega_c * u23.y;
   }
   asm volatile("cp.async.wait_all;" ::: "memory");
   __syncthreads();
 
+  // ---- phase A: x and y ---------------------------------------------------------------------------------------------
   {
     double fa[4][4], acc[4][4];
     const int col = rv;
@@ -111,7 +158,8 @@ __global__ void __launch_bounds__(16 * KV) rhs4_tile_kernel(const Params p) {
     const double sx = p.J[0] * ax, sy = p.J[1] * ay;
 #pragma unroll
     for (int jy = 0; jy < 4; ++jy) {
-      const double uL = ax > 0.0 ? hX[jy] : fa[0][jy], uR = ax > 0.0 ? fa[3][jy] : hX[jy];
+      const double h = hXs[jy * NT + tid];
+      const double uL = ax > 0.0 ? h : fa[0][jy], uR = ax > 0.0 ? fa[3][jy] : h;
 #pragma unroll
       for (int jx = 0; jx < 4; ++jx) {
         double v = p.Xi[2 * jx] * uL;
@@ -123,7 +171,8 @@ __global__ void __launch_bounds__(16 * KV) rhs4_tile_kernel(const Params p) {
     }
 #pragma unroll
     for (int jx = 0; jx < 4; ++jx) {
-      const double uL = ay > 0.0 ? hY[jx] : fa[jx][0], uR = ay > 0.0 ? fa[jx][3] : hY[jx];
+      const double h = hYs[jx * NT + tid];
+      const double uL = ay > 0.0 ? h : fa[jx][0], uR = ay > 0.0 ? fa[jx][3] : h;
 #pragma unroll
       for (int jy = 0; jy < 4; ++jy) {
         double v = p.Xi[2 * jy] * uL;
@@ -141,68 +190,9 @@ __global__ void __launch_bounds__(16 * KV) rhs4_tile_kernel(const Params p) {
         accT[row * R + swz<KV>(row, col >> 1) * 2 + (col & 1)] = acc[jx][jy];
       }
   }
-
-  // ---- phase B ----------------------------------------------------------------------------------------------------
-  const int ev = tid % KV, jy_b = (tid / KV) & 3, jx_b = tid / (4 * KV);
-  const int gx = gx0 + jx_b, gy = gy0 + jy_b;
-  const long long xy = gx * s0 + gy * s1;
-  const long long gxy = (long long)gx * p.G[1] + gy;
-  const double exf = p.Ex ? __ldg(p.Ex + gxy) : 0.0, eyf = p.Ey ? __ldg(p.Ey + gxy) : 0.0;
-  const int gvb = gv0 + ev * 4;                                   // first v node of this thread's element
-  double au[4], av[4];
-  {
-    const double2 v01 = *reinterpret_cast<const double2*>(p.coord[3] + gvb), v23 = *reinterpret_cast<const double2*>(p.coord[3] + gvb + 2);
-    const double2 u01 = *reinterpret_cast<const double2*>(p.coord[2] + gu0), u23 = *reinterpret_cast<const double2*>(p.coord[2] + gu0 + 2);
-    au[0] = -exf - p.omega_c * v01.x; au[1] = -exf - p.omega_c * v01.y; au[2] = -exf - p.omega_c * v23.x; au[3] = -exf - p.omega_c * v23.y;
-    av[0] = -eyf + p.omega_c * u01.x; av[1] = -eyf + p.omega_c * u01.y; av[2] = -eyf + p.omega_c * u23.x; av[3] = -eyf + p.omega_c * u23.y;
-  }
-  // u faces: the row below / above the tile, the four v nodes of this element
-  double hUlo[4] = {0.0, 0.0, 0.0, 0.0}, hUhi[4] = {0.0, 0.0, 0.0, 0.0};
-  {
-    const int lo = eu > 0 ? gu0 - 1 : (p.bc[2] == 0 ? p.G[2] - 1 : -1);
-    const int hi = eu < p.N[2] - 1 ? gu0 + 4 : (p.bc[2] == 0 ? 0 : -1);
-    const bool pos = au[0] > 0.0 || au[1] > 0.0 || au[2] > 0.0 || au[3] > 0.0;
-    const bool neg = au[0] < 0.0 || au[1] < 0.0 || au[2] < 0.0 || au[3] < 0.0;
-    if (lo >= 0 && pos) {
-      const double2* q = reinterpret_cast<const double2*>(p.f + xy + lo * s2 + gvb);
-      const double2 a = __ldg(q), b = __ldg(q + 1);
-      hUlo[0] = a.x; hUlo[1] = a.y; hUlo[2] = b.x; hUlo[3] = b.y;
-    }
-    if (hi >= 0 && neg) {
-      const double2* q = reinterpret_cast<const double2*>(p.f + xy + hi * s2 + gvb);
-      const double2 a = __ldg(q), b = __ldg(q + 1);
-      hUhi[0] = a.x; hUhi[1] = a.y; hUhi[2] = b.x; hUhi[3] = b.y;
-    }
-  }
-  // v faces at the two tile edges (lanes ev = 0 and ev = KV-1 only)
-  double eVlo[4] = {0.0, 0.0, 0.0, 0.0}, eVhi[4] = {0.0, 0.0, 0.0, 0.0};
-  if (ev == 0) {
-    const int lo = evb > 0 ? gv0 - 1 : (p.bc[3] == 0 ? p.G[3] - 1 : -1);
-    if (lo >= 0) {
-#pragma unroll
-      for (int ju = 0; ju < 4; ++ju) if (av[ju] > 0.0) eVlo[ju] = __ldg(p.f + xy + (gu0 + ju) * s2 + lo);
-    }
-  }
-  if (ev == KV - 1) {
-    const int hi = evb < nvb - 1 ? gv0 + R : (p.bc[3] == 0 ? 0 : -1);
-    if (hi >= 0) {
-#pragma unroll
-      for (int ju = 0; ju < 4; ++ju) if (av[ju] < 0.0) eVhi[ju] = __ldg(p.f + xy + (gu0 + ju) * s2 + hi);
-    }
-  }
-  // step input of the stage combination
-  double fnv[4][4];
-  const bool use_fn = p.mode != 0 && p.fn != nullptr;
-  if (use_fn) {
-#pragma unroll
-    for (int ju = 0; ju < 4; ++ju) {
-      const double2* q = reinterpret_cast<const double2*>(p.fn + xy + (gu0 + ju) * s2 + gvb);
-      const double2 a = __ldcs(q), b = __ldcs(q + 1);
-      fnv[ju][0] = a.x; fnv[ju][1] = a.y; fnv[ju][2] = b.x; fnv[ju][3] = b.y;
-    }
-  }
   __syncthreads();
 
+  // ---- phase B: u and v, stage combination --------------------------------------------------------------------------
   double fb[4][4], res[4][4];
   const int rowb = (jx_b * 4 + jy_b) * 4;
 #pragma unroll
@@ -215,25 +205,28 @@ __global__ void __launch_bounds__(16 * KV) rhs4_tile_kernel(const Params p) {
     const double2 d = *reinterpret_cast<const double2*>(accT + row * R + swz<KV>(row, 2 * ev + 1) * 2);
     res[ju][0] = c.x; res[ju][1] = c.y; res[ju][2] = d.x; res[ju][3] = d.y;
   }
-  // u lines (fixed jv)
+  {
+    const double2* h2 = reinterpret_cast<const double2*>(hUs);
+    const double2 l0 = h2[tid], l1 = h2[NT + tid], h0 = h2[2 * NT + tid], h1 = h2[3 * NT + tid];
+    const double hUlo[4] = {l0.x, l0.y, l1.x, l1.y}, hUhi[4] = {h0.x, h0.y, h1.x, h1.y};
 #pragma unroll
-  for (int jv = 0; jv < 4; ++jv) {
-    const double uL = au[jv] > 0.0 ? hUlo[jv] : fb[0][jv], uR = au[jv] > 0.0 ? fb[3][jv] : hUhi[jv];
-    const double su = p.J[2] * au[jv];
+    for (int jv = 0; jv < 4; ++jv) {                                  // u lines (fixed jv)
+      const double uL = au[jv] > 0.0 ? hUlo[jv] : fb[0][jv], uR = au[jv] > 0.0 ? fb[3][jv] : hUhi[jv];
+      const double su = p.J[2] * au[jv];
 #pragma unroll
-    for (int ju = 0; ju < 4; ++ju) {
-      double v = p.Xi[2 * ju] * uL;
-      v = fma(-p.Xi[2 * ju + 1], uR, v);
+      for (int ju = 0; ju < 4; ++ju) {
+        double v = p.Xi[2 * ju] * uL;
+        v = fma(-p.Xi[2 * ju + 1], uR, v);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) v = fma(p.U[ju * 4 + k], fb[k][jv], v);
-      res[ju][jv] = fma(su, v, res[ju][jv]);
+        for (int k = 0; k < 4; ++k) v = fma(p.U[ju * 4 + k], fb[k][jv], v);
+        res[ju][jv] = fma(su, v, res[ju][jv]);
+      }
     }
   }
-  // v lines (fixed ju): neighbours inside the tile from the adjacent lanes
 #pragma unroll
-  for (int ju = 0; ju < 4; ++ju) {
+  for (int ju = 0; ju < 4; ++ju) {                                    // v lines (fixed ju): neighbours from the adjacent lanes
     const double from_lo = __shfl_up_sync(0xffffffffu, fb[ju][3], 1), from_hi = __shfl_down_sync(0xffffffffu, fb[ju][0], 1);
-    const double nlo = ev > 0 ? from_lo : eVlo[ju], nhi = ev < KV - 1 ? from_hi : eVhi[ju];
+    const double nlo = ev > 0 ? from_lo : eVs[rowb + ju], nhi = ev < KV - 1 ? from_hi : eVs[64 + rowb + ju];
     const double uL = av[ju] > 0.0 ? nlo : fb[ju][0], uR = av[ju] > 0.0 ? fb[ju][3] : nhi;
     const double sv = p.J[3] * av[ju];
 #pragma unroll
@@ -245,24 +238,29 @@ __global__ void __launch_bounds__(16 * KV) rhs4_tile_kernel(const Params p) {
       res[ju][jv] = fma(sv, v, res[ju][jv]);
     }
   }
-  // stage combination, stores, density partial
   double dens = 0.0;
+  double2* q = reinterpret_cast<double2*>(p.out + xy + gu0 * s2 + gvb);
+  const double2 w01 = *reinterpret_cast<const double2*>(p.wqv + gvb), w23 = *reinterpret_cast<const double2*>(p.wqv + gvb + 2);
 #pragma unroll
   for (int ju = 0; ju < 4; ++ju) {
     double o[4];
+    if (p.mode == 0) {
 #pragma unroll
-    for (int jv = 0; jv < 4; ++jv) {
-      if (p.mode == 0) o[jv] = res[ju][jv];
-      else {
-        const double v = fma(p.dt, res[ju][jv], fb[ju][jv]);
-        o[jv] = use_fn ? fma(p.c1, v, p.c0 * fnv[ju][jv]) : p.c1 * v;
+      for (int jv = 0; jv < 4; ++jv) o[jv] = res[ju][jv];
+    } else {
+#pragma unroll
+      for (int jv = 0; jv < 4; ++jv) o[jv] = p.c1 * fma(p.dt, res[ju][jv], fb[ju][jv]);
+      if (use_fn) {
+        const int row = rowb + ju;
+        const double2 a = *reinterpret_cast<const double2*>(fnT + row * R + swz<KV>(row, 2 * ev) * 2);
+        const double2 b = *reinterpret_cast<const double2*>(fnT + row * R + swz<KV>(row, 2 * ev + 1) * 2);
+        o[0] = fma(p.c0, a.x, o[0]); o[1] = fma(p.c0, a.y, o[1]); o[2] = fma(p.c0, b.x, o[2]); o[3] = fma(p.c0, b.y, o[3]);
       }
     }
-    double2* q = reinterpret_cast<double2*>(p.out + xy + (gu0 + ju) * s2 + gvb);
     __stcs(q, make_double2(o[0], o[1]));
     __stcs(q + 1, make_double2(o[2], o[3]));
+    q += s2 / 2;
     if (p.partials) {
-      const double2 w01 = *reinterpret_cast<const double2*>(p.wqv + gvb), w23 = *reinterpret_cast<const double2*>(p.wqv + gvb + 2);
       const double rowsum = fma(w01.x, o[0], fma(w01.y, o[1], fma(w23.x, o[2], w23.y * o[3])));
       dens = fma(p.wqu[gu0 + ju], rowsum, dens);
     }

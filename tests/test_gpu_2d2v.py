@@ -62,12 +62,10 @@ def test_rhs_matches_oracle(N, n, bc, mode):
     ctx.close()
 
 
-@pytest.mark.parametrize("order", [1, 2])
-def test_tiled_equals_generic_kernel_and_tile_orders(order):
+def test_tiled_equals_generic_kernel():
     g, ctx = make_pair((10, 3, 3, 8), (4, 4, 4, 4))
     f, Ex, Ey = seeded_inputs(g)
     fd, exd, eyd = dev(f), dev(Ex), dev(Ey)
-    ctx.set_option(api().OPT4_TILE_ORDER, order)
     a = ctx.rhs(fd, exd, eyd).cpu().numpy()
     assert ctx.last_kernel == "rhs4_tile<8>"
     ctx.set_option(api().OPT4_RHS_KERNEL, 1)
