@@ -168,3 +168,58 @@ def test_errors():
     with pytest.raises(a.DGError):
         ctx.rhs(f)                     # odd N_v: no tiled kernel
     ctx.close()
+
+
+def test_bench_size_64_full_array_stage_against_oracle():
+    """config6_2d2v_64^4 (16.7 M DOF, the launch configuration bench.py times: rhs4_tile<8>, 8192 tiles): one Shu-Osher stage
+    with a seeded field, the whole output array and the epilogue density against the oracle."""
+    N = (16, 16, 16, 16)
+    lo, hi = (0.0, 0.0, -8.5, -8.5), (20 * math.pi, 20 * math.pi, 8.5, 8.5)
+    g, ctx = make_pair(N, (4, 4, 4, 4), omega_c=1.0, lo=lo, hi=hi)
+    x, y, u, v = [c.reshape(-1) for c in g.coords]
+    f = wl.add_uniform_noise(wl.ring2d_f0(x, y, u, v, 0.1, 0.1), wl.SEED_CFG6_NOISE, 1e-4)
+    gxy = g.flat_shape[0] * g.flat_shape[1]
+    E = 0.1 * wl.counter_normal(wl.SEED_CFG6_E, 0, 2 * gxy)
+    Ex, Ey = E[:gxy].reshape(g.flat_shape[:2]), E[gxy:].reshape(g.flat_shape[:2])
+    fd = dev(f)
+    out, rho = torch.empty_like(fd), torch.empty(g.flat_shape[:2], dtype=torch.float64, device="cuda")
+    ctx.rk_stage(fd, fd, dev(Ex), dev(Ey), out, 0.75, 0.25, 2e-4, rho_out=rho)
+    assert ctx.last_kernel == "rhs4_tile<8>"
+    ro = o4.rhs(g, f, Ex, Ey)
+    oo = 0.75 * f + 0.25 * (f + 2e-4 * ro)
+    assert relerr(out.cpu().numpy(), oo) < 1e-13
+    assert relerr(rho.cpu().numpy(), o4.density(g, oo)) < 1e-13
+    r = ctx.rhs(fd, dev(Ex), dev(Ey)).cpu().numpy()
+    assert relerr(r, ro) < 1e-12
+    ctx.close()
+
+
+def test_bench_size_128_sampled_against_oracle():
+    """config6_2d2v_128^4 (268 M DOF, 2.1 GB per array): dg4_rhs on the full grid, 400 seeded sample nodes (tile corners, box
+    faces and interior) against the oracle's node-by-node loops, and the full-grid density against its plain definition."""
+    N = (32, 32, 32, 32)
+    lo, hi = (0.0, 0.0, -8.5, -8.5), (20 * math.pi, 20 * math.pi, 8.5, 8.5)
+    g, ctx = make_pair(N, (4, 4, 4, 4), omega_c=1.0, lo=lo, hi=hi)
+    x, y, u, v = [c.reshape(-1) for c in g.coords]
+    f = wl.add_uniform_noise(wl.ring2d_f0(x, y, u, v, 0.1, 0.1), wl.SEED_CFG6_NOISE, 1e-4)
+    gxy = g.flat_shape[0] * g.flat_shape[1]
+    E = 0.1 * wl.counter_normal(wl.SEED_CFG6_E, 0, 2 * gxy)
+    Ex, Ey = E[:gxy].reshape(g.flat_shape[:2]), E[gxy:].reshape(g.flat_shape[:2])
+    fd = dev(f)
+    r = ctx.rhs(fd, dev(Ex), dev(Ey))
+    assert ctx.last_kernel == "rhs4_tile<8>"
+    G = g.flat_shape[0]
+    pick = (wl.counter_uniform(wl.SEED_CFG6_E, 1 << 20, 4 * 400) * G).astype(np.int64).reshape(400, 4)
+    edge = np.array([0, 3, 4, 31, 32, 63, 64, 127, G - 4, G - 1])
+    pick[:120] = edge[(pick[:120] % edge.size)]                      # element / tile / box boundaries in every dimension
+    idx = torch.from_numpy(pick).cuda()
+    got = r[idx[:, 0], idx[:, 1], idx[:, 2], idx[:, 3]].cpu().numpy()
+    scale = float(r.abs().max().item())
+    for k in range(pick.shape[0]):
+        want = o4.rhs_at(g, f, Ex, Ey, tuple(int(i) for i in pick[k]))
+        assert abs(got[k] - want) < 1e-12 * scale, (pick[k], got[k], want)
+    rho = ctx.density(fd).cpu().numpy()
+    wu, wv = np.tile(g.w[2] / g.J[2], g.nelem[2]), np.tile(g.w[3] / g.J[3], g.nelem[3])
+    for gx, gy in [(0, 0), (5, 77), (127, 64), (64, 127)]:
+        assert abs(rho[gx, gy] - wu @ f[gx, gy] @ wv) < 1e-13 * abs(rho[gx, gy])
+    ctx.close()
