@@ -222,7 +222,15 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
       if (chunks_out) *chunks_out = p.chunks;
     }
     if (ctx->N[1] > 65535 || ctx->N[0] > 65535) return fail(DG_ERR_UNSUPPORTED, "dg4: more than 65535 elements in x or y");
-    const dim3 tiles(ctx->N[2] * nvb, ctx->N[1], ctx->N[0]);
+    // x-elements per rasterisation group: a power of two (<= 8) dividing N_x, grown while the tiles between a tile and its
+    // y neighbour (read + read + written bytes) stay within ~32 MB, a quarter of the L2
+    int bxl = 0;
+    {
+      const double tile_bytes = 3.0 * 64 * 4 * kv * 8;
+      while (bxl < 3 && ctx->N[0] % (2 << bxl) == 0 && (double)ctx->N[2] * nvb * (2 << bxl) * tile_bytes <= 32e6) ++bxl;
+    }
+    p.bx_log2 = bxl;
+    const dim3 tiles(nvb * (1 << bxl) * ctx->N[2], ctx->N[1], ctx->N[0] >> bxl);
     const bool with_fn = mode != 0 && fn != nullptr;
     const size_t smem = sizeof(double) * (kv == 8 ? dg4::tile_smem_doubles<8>(with_fn) : kv == 4 ? dg4::tile_smem_doubles<4>(with_fn)
                                                                                               : dg4::tile_smem_doubles<2>(with_fn));

@@ -24,6 +24,7 @@ struct Params {
   const double* wqv;
   double* partials;          // [G0*G1][chunks] per-tile density partials of out, or nullptr
   int chunks;
+  int bx_log2;               // tiled kernel: log2 of the x-elements per rasterisation group
   long long dof;
 };
 

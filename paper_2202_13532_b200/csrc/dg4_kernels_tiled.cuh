@@ -50,9 +50,13 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
   double* hUs = hYs + 4 * NT;             // double2 [lo0, lo1, hi0, hi1][tid]
   double* eVs = hUs + 8 * NT;             // [side][row]
   double* fnT = eVs + 128;
-  // grid = (N_u * N_v/KV, N_y, N_x): consecutive CTAs walk v, then u -- the u and v neighbours of a tile are in flight with it
+  // grid = (N_v/KV * BX * N_u, N_y, N_x / BX), BX = 2^bx_log2 x-elements per group: consecutive CTAs walk v, then the x elements
+  // of a group, then u -- the v, x and u neighbours of a tile are in flight with it and the y neighbour is N_u BX N_v/KV tiles
+  // away (L2), where a row-major walk would put a whole x slab (G_y G_u G_v n doubles, more than the L2 on large grids)
+  // between a tile and its x neighbour.
   const int nvb = p.N[3] / KV;
-  const int eu = blockIdx.x / nvb, evb = blockIdx.x - eu * nvb, ey = blockIdx.y, ex = blockIdx.z;
+  const int bq = blockIdx.x / nvb, evb = blockIdx.x - bq * nvb;
+  const int eu = bq >> p.bx_log2, ex = (blockIdx.z << p.bx_log2) + (bq & ((1 << p.bx_log2) - 1)), ey = blockIdx.y;
   const int gx0 = ex * 4, gy0 = ey * 4, gu0 = eu * 4, gv0 = evb * R;
   const long long s2 = p.G[3], s1 = s2 * p.G[2], s0 = s1 * p.G[1];
   const int tid = threadIdx.x;
