@@ -301,7 +301,7 @@ static int launch_density4_finish(dg4_ctx* ctx, int nchunks, double* rho, cudaSt
 
 static int launch_project4(dg4_ctx* ctx, const double* rho, double* c, double* Et, cudaStream_t st) {
   const int G0 = ctx->G[0], G1 = ctx->G[1], NQ = 2 * ctx->Q + 1;
-  dg4::proj_x_kernel<<<dim3((G1 + 127) / 128, ctx->P1), 128, 0, st>>>(ctx->d_Tx, rho, G0, G1, ctx->A);
+  dg4::proj_x_kernel<<<dim3((G1 + 31) / 32, ctx->P1), 256, 0, st>>>(ctx->d_Tx, rho, G0, G1, ctx->A);
   int rc = check4(ctx, "proj_x_kernel");
   if (rc) return rc;
   dg4::proj_y_poisson_kernel<<<(ctx->P1 * NQ + 3) / 4, 128, 0, st>>>(ctx->d_Ty, ctx->A, G1, ctx->P1, ctx->Q, ctx->kx1, ctx->ky1, c, Et);
@@ -312,11 +312,11 @@ static int launch_field4(dg4_ctx* ctx, const double* rho, double* Ex, double* Ey
   const int G0 = ctx->G[0], G1 = ctx->G[1];
   int rc = launch_project4(ctx, rho, nullptr, ctx->Et, st);
   if (rc) return rc;
-  dg4::synth_y_kernel<<<dim3((G1 + 127) / 128, ctx->P1, 2), 128, 0, st>>>(ctx->Et, ctx->d_Wy, G1, ctx->P1, ctx->Q, ctx->B);
+  dg4::synth_y_kernel<<<dim3((G1 + 31) / 32, ctx->P1, 2), 256, 0, st>>>(ctx->Et, ctx->d_Wy, G1, ctx->P1, ctx->Q, ctx->B);
   rc = check4(ctx, "synth_y_kernel");
   if (rc) return rc;
   if (G0 > 65535) return fail(DG_ERR_UNSUPPORTED, "dg4: G_x above 65535");
-  dg4::synth_x_kernel<<<dim3((G1 + 127) / 128, G0, 2), 128, 0, st>>>(ctx->B, ctx->d_Wx, G0, G1, ctx->P1, Ex, Ey);
+  dg4::synth_x_kernel<<<dim3((G1 + 31) / 32, G0, 2), 128, 0, st>>>(ctx->B, ctx->d_Wx, G0, G1, ctx->P1, Ex, Ey);
   return check4(ctx, "synth_x_kernel");
 }
 

@@ -73,21 +73,32 @@ __global__ void __launch_bounds__(256) rhs4_generic_kernel(const Params p) {
 // T rows: T[(2p+c)*G + g], c = 0 real / 1 imaginary part of Eq. 63.  Waves: W[(p*G + g)*2 + c] = e^{i k_p x_g}.
 // ---------------------------------------------------------------------------------------------------------------
 
-// A[p][gy] = sum_gx T^x_p[gx] rho[gx][gy].  grid (ceil(G1/128), P+1).
-__global__ void __launch_bounds__(128) proj_x_kernel(const double* __restrict__ Tx, const double* __restrict__ rho, int G0, int G1,
+// A[p][gy] = sum_gx T^x_p[gx] rho[gx][gy].  grid (ceil(G1/32), P+1), 256 threads = 32 g_y x 8 slices of g_x; the slices
+// are summed in a fixed order (deterministic).
+__global__ void __launch_bounds__(256) proj_x_kernel(const double* __restrict__ Tx, const double* __restrict__ rho, int G0, int G1,
                                                       double* __restrict__ A) {
-  const int gy = blockIdx.x * 128 + threadIdx.x, p = blockIdx.y;
-  if (gy >= G1) return;
+  __shared__ double red[2][8][32];
+  const int gl = threadIdx.x & 31, sl = threadIdx.x >> 5;
+  const int gy = blockIdx.x * 32 + gl, p = blockIdx.y;
   const double* tr = Tx + (size_t)(2 * p) * G0;
   const double* ti = tr + G0;
   double are = 0.0, aim = 0.0;
-  for (int gx = 0; gx < G0; ++gx) {
-    const double r = rho[(size_t)gx * G1 + gy];
-    are = fma(tr[gx], r, are);
-    aim = fma(ti[gx], r, aim);
+  if (gy < G1) {
+    for (int gx = sl; gx < G0; gx += 8) {
+      const double r = rho[(size_t)gx * G1 + gy];
+      are = fma(tr[gx], r, are);
+      aim = fma(ti[gx], r, aim);
+    }
   }
-  A[((size_t)p * G1 + gy) * 2] = are;
-  A[((size_t)p * G1 + gy) * 2 + 1] = aim;
+  red[0][sl][gl] = are; red[1][sl][gl] = aim;
+  __syncthreads();
+  if (threadIdx.x < 64) {
+    const int c = threadIdx.x >> 5;
+    double v = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v += red[c][k][gl];
+    if (gy < G1) A[((size_t)p * G1 + gy) * 2 + c] = v;
+  }
 }
 
 // c[p][q'] = sum_gy T^y_q[gy] A[p][gy], q = q' - Q (T_{-q} = conj T_q), and the Poisson factors of Eq. 68/71:
@@ -129,36 +140,54 @@ __global__ void __launch_bounds__(128) proj_y_poisson_kernel(const double* __res
   }
 }
 
-// B[s][p][gy] = sum_q' Et[s][p][q'] e^{i k_q y_gy}.  grid (ceil(G1/128), P1, 2).
-__global__ void __launch_bounds__(128) synth_y_kernel(const double* __restrict__ Et, const double* __restrict__ Wy, int G1, int P1, int Q,
+// B[s][p][gy] = sum_q' Et[s][p][q'] e^{i k_q y_gy}.  grid (ceil(G1/32), P1, 2), 256 threads = 32 g_y x 8 slices of q'.
+__global__ void __launch_bounds__(256) synth_y_kernel(const double* __restrict__ Et, const double* __restrict__ Wy, int G1, int P1, int Q,
                                                        double* __restrict__ B) {
-  const int gy = blockIdx.x * 128 + threadIdx.x, p = blockIdx.y, s = blockIdx.z;
-  if (gy >= G1) return;
+  __shared__ double red[2][8][32];
+  const int gl = threadIdx.x & 31, sl = threadIdx.x >> 5;
+  const int gy = blockIdx.x * 32 + gl, p = blockIdx.y, s = blockIdx.z;
   const int NQ = 2 * Q + 1;
   const double* e = Et + ((size_t)s * P1 + p) * NQ * 2;
   double bre = 0.0, bim = 0.0;
-  for (int qi = 0; qi < NQ; ++qi) {
-    const int q = qi - Q, qa = q < 0 ? -q : q;
-    const double wr = Wy[((size_t)qa * G1 + gy) * 2], wi = (q < 0 ? -1.0 : 1.0) * Wy[((size_t)qa * G1 + gy) * 2 + 1];
-    bre += e[2 * qi] * wr - e[2 * qi + 1] * wi;
-    bim += e[2 * qi] * wi + e[2 * qi + 1] * wr;
+  if (gy < G1) {
+    for (int qi = sl; qi < NQ; qi += 8) {
+      const int q = qi - Q, qa = q < 0 ? -q : q;
+      const double wr = Wy[((size_t)qa * G1 + gy) * 2], wi = (q < 0 ? -1.0 : 1.0) * Wy[((size_t)qa * G1 + gy) * 2 + 1];
+      bre += e[2 * qi] * wr - e[2 * qi + 1] * wi;
+      bim += e[2 * qi] * wi + e[2 * qi + 1] * wr;
+    }
   }
-  B[(((size_t)s * P1 + p) * G1 + gy) * 2] = bre;
-  B[(((size_t)s * P1 + p) * G1 + gy) * 2 + 1] = bim;
+  red[0][sl][gl] = bre; red[1][sl][gl] = bim;
+  __syncthreads();
+  if (threadIdx.x < 64) {
+    const int c = threadIdx.x >> 5;
+    double v = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v += red[c][k][gl];
+    if (gy < G1) B[(((size_t)s * P1 + p) * G1 + gy) * 2 + c] = v;
+  }
 }
 
-// E_s[gx][gy] = Re B[s][0][gy] + 2 Re sum_{p>=1} B[s][p][gy] e^{i k_p x_gx}.  grid (ceil(G1/128), G0, 2).
+// E_s[gx][gy] = Re B[s][0][gy] + 2 Re sum_{p>=1} B[s][p][gy] e^{i k_p x_gx}.  grid (ceil(G1/32), G0, 2), 128 threads =
+// 32 g_y x 4 slices of p.
 __global__ void __launch_bounds__(128) synth_x_kernel(const double* __restrict__ B, const double* __restrict__ Wx, int G0, int G1, int P1,
                                                        double* __restrict__ Ex, double* __restrict__ Ey) {
-  const int gy = blockIdx.x * 128 + threadIdx.x, gx = blockIdx.y, s = blockIdx.z;
-  if (gy >= G1) return;
+  __shared__ double red[4][32];
+  const int gl = threadIdx.x & 31, sl = threadIdx.x >> 5;
+  const int gy = blockIdx.x * 32 + gl, gx = blockIdx.y, s = blockIdx.z;
   double acc = 0.0;
-  for (int p = 1; p < P1; ++p) {
-    const double br = B[(((size_t)s * P1 + p) * G1 + gy) * 2], bi = B[(((size_t)s * P1 + p) * G1 + gy) * 2 + 1];
-    acc += br * Wx[((size_t)p * G0 + gx) * 2] - bi * Wx[((size_t)p * G0 + gx) * 2 + 1];
+  if (gy < G1) {
+    for (int p = 1 + sl; p < P1; p += 4) {
+      const double br = B[(((size_t)s * P1 + p) * G1 + gy) * 2], bi = B[(((size_t)s * P1 + p) * G1 + gy) * 2 + 1];
+      acc += br * Wx[((size_t)p * G0 + gx) * 2] - bi * Wx[((size_t)p * G0 + gx) * 2 + 1];
+    }
   }
-  const double v = B[(((size_t)s * P1) * G1 + gy) * 2] + 2.0 * acc;
-  (s == 0 ? Ex : Ey)[(size_t)gx * G1 + gy] = v;
+  red[sl][gl] = acc;
+  __syncthreads();
+  if (threadIdx.x < 32 && gy < G1) {
+    const double v = B[(((size_t)s * P1) * G1 + gy) * 2] + 2.0 * (((red[0][gl] + red[1][gl]) + red[2][gl]) + red[3][gl]);
+    (s == 0 ? Ex : Ey)[(size_t)gx * G1 + gy] = v;
+  }
 }
 
 }  // namespace dg4
