@@ -223,3 +223,64 @@ def test_bench_size_128_sampled_against_oracle():
     for gx, gy in [(0, 0), (5, 77), (127, 64), (64, 127)]:
         assert abs(rho[gx, gy] - wu @ f[gx, gy] @ wv) < 1e-13 * abs(rho[gx, gy])
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# physics on the GPU path: signs and coupling of the second space dimension, end to end
+# ---------------------------------------------------------------------------------------------
+def _landau_rate(ctx, f, dt, per, nsamp):
+    amp = []
+    for _ in range(nsamp):
+        ctx.ssprk3_run(f, dt, per, True)
+        Ex, Ey = ctx.poisson_E(ctx.density(f))
+        amp.append(float(torch.sqrt(Ex * Ex + Ey * Ey).max()))
+    amp = np.array(amp); t = dt * per * (np.arange(nsamp) + 1)
+    pk = [i for i in range(1, nsamp - 1) if amp[i] > amp[i - 1] and amp[i] > amp[i + 1]]
+    assert len(pk) >= 6
+    return np.polyfit(t[pk], np.log(amp[pk]), 1)[0], float(np.mean(np.diff(t[pk])))
+
+
+@pytest.mark.parametrize("direction", ["y", "oblique"])
+def test_landau_damping_2d2v(direction):
+    """Unmagnetised Maxwellian with a 1 % density wave of |k| = 0.5 along y, or along the diagonal of a square box: the field
+    decays at the textbook Landau rate -0.1533 with omega_r = 1.4156 (as config 1; a wrong sign of E_y or of a_v grows
+    instead), and E(0) = -(A/|k|^2) k sin(k.x) (closed form)."""
+    if direction == "y":
+        N, kx, ky = (2, 16, 8, 32), 0.0, 0.5
+        hi_xy = (4 * math.pi, 4 * math.pi)
+    else:
+        N, kx, ky = (16, 16, 32, 32), 0.5 / math.sqrt(2.0), 0.5 / math.sqrt(2.0)
+        hi_xy = (2 * math.pi / kx, 2 * math.pi / ky)
+    ctx = api().DG4Context(N, (4, 4, 4, 4), (0.0, 0.0, -6.0, -6.0), hi_xy + (6.0, 6.0), bc=(0, 0, 1, 1), omega_c=0.0, pmax=(4, 4))
+    x, y, u, v = (ctx.nodes(d) for d in range(4))
+    arg = kx * x[:, None] + ky * y[None, :]
+    maxw = np.exp(-0.5 * (u[:, None] ** 2 + v[None, :] ** 2)) / (2 * math.pi)
+    f = torch.from_numpy((1.0 + 0.01 * np.cos(arg))[:, :, None, None] * maxw[None, None]).cuda()
+    Ex, Ey = ctx.poisson_E(ctx.density(f))
+    k2 = kx * kx + ky * ky
+    assert np.max(np.abs(Ex.cpu().numpy() + 0.01 * kx / k2 * np.sin(arg))) < 2e-6
+    assert np.max(np.abs(Ey.cpu().numpy() + 0.01 * ky / k2 * np.sin(arg))) < 2e-6
+    rate, period = _landau_rate(ctx, f, 0.008, 6, 420)        # sum_d |a_d| dt / Delta_d <= 0.09 < 0.13 (n = 4 RK3 limit)
+    assert -0.165 < rate < -0.143, rate
+    assert abs(period - math.pi / 1.4156) < 0.08
+    assert ctx.last_kernel == "rhs4_tile<8>"
+    ctx.close()
+
+
+def test_cyclotron_rotation_2d2v():
+    """E = 0, uniform in x and y: f(u, v, t) = f0(u cos th + v sin th, -u sin th + v cos th), th = omega_c t (counter-clockwise,
+    reading C15): a blob at (u, v) = (1.5, 0) is at (0, 1.5) after a quarter gyration."""
+    ctx = api().DG4Context((1, 1, 16, 16), (4, 4, 4, 4), (0.0, 0.0, -6.0, -6.0), (1.0, 1.0, 6.0, 6.0), bc=(0, 0, 1, 1), omega_c=1.0)
+    u, v = ctx.nodes(2), ctx.nodes(3)
+    blob = lambda a, b: np.exp(-((a - 1.5) ** 2 + b ** 2) / (2 * 0.6 ** 2))
+    f0 = np.broadcast_to(blob(u[:, None], v[None, :]), ctx.flat_shape).copy()
+    steps = 400
+    dt = 0.5 * math.pi / steps
+    f = ctx.ssprk3_run(torch.from_numpy(f0).cuda(), dt, steps, False).cpu().numpy()
+    th = 0.5 * math.pi
+    U, V = u[:, None], v[None, :]
+    ccw = blob(U * math.cos(th) + V * math.sin(th), -U * math.sin(th) + V * math.cos(th))
+    cw = blob(U * math.cos(th) - V * math.sin(th), U * math.sin(th) + V * math.cos(th))
+    assert np.max(np.abs(f - ccw[None, None])) < 0.02
+    assert np.max(np.abs(f - cw[None, None])) > 0.5
+    ctx.close()
