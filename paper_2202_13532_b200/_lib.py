@@ -88,6 +88,7 @@ SIGNATURES = {
     "dg4_ssprk3_run": (C.c_int, [_vp, _vp, _dbl, _i32, _i32, _vp]),
     "dg4_ssprk3_run_host": (C.c_int, [_vp, _vp, _dbl, _i32, _i32]),
     "dg4_get_nodes": (C.c_int, [_vp, _i32, _dp]),
+    "dg4_max_stable_dt": (_dbl, [_vp, _dbl]),
     "dg4_set_option": (C.c_int, [_vp, _i32, _i64]),
     "dg4_get_profile": (C.c_int, [_vp, _dp, C.POINTER(_i64), _i32]),
     "dg4_launch_count": (_i64, [_vp]),

@@ -315,6 +315,9 @@ class DG4Context:
         _check(_L.dg4_get_nodes(self._h, dim, x.ctypes.data_as(C.POINTER(C.c_double))), "dg4_get_nodes")
         return x
 
+    def max_stable_dt(self, E_bound=0.0):
+        return float(_L.dg4_max_stable_dt(self._h, float(E_bound)))
+
     def set_option(self, key, value):
         _check(_L.dg4_set_option(self._h, int(key), int(value)), "dg4_set_option")
 

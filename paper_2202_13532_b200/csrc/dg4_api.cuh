@@ -412,6 +412,20 @@ extern "C" int dg4_get_nodes(const dg4_ctx* ctx, int32_t dim, double* coords) {
   return DG_OK;
 }
 
+extern "C" double dg4_max_stable_dt(const dg4_ctx* ctx, double E_bound) {
+  if (!ctx) return 0.0;
+  // per-dimension limits add: sum_d |a_d|_max / (nu_d Delta_d) * dt <= 1, nu_d = the SSP-RK3 limit of the 1-D upwind operator
+  auto vmax = [&](int d) { return std::fmax(std::fabs(ctx->desc.lo[d]), std::fabs(ctx->desc.hi[d])); };
+  const double w = std::fabs(ctx->desc.omega_c), e = std::fabs(E_bound);
+  const double amax[4] = {vmax(2), vmax(3), e + w * vmax(3), e + w * vmax(2)};
+  double sum = 0.0;
+  for (int d = 0; d < 4; ++d) {
+    const double nu = dgsetup::rk3_cfl_limit(ctx->basis[d]);
+    sum += amax[d] / (nu * (ctx->desc.hi[d] - ctx->desc.lo[d]) / ctx->N[d]);
+  }
+  return sum > 0.0 ? 1.0 / sum : INFINITY;
+}
+
 extern "C" int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_set_option: null context");
   if (key == DG4_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_kernel = (int)value; return DG_OK; }

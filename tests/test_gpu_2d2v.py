@@ -260,7 +260,8 @@ def test_landau_damping_2d2v(direction):
     k2 = kx * kx + ky * ky
     assert np.max(np.abs(Ex.cpu().numpy() + 0.01 * kx / k2 * np.sin(arg))) < 2e-6
     assert np.max(np.abs(Ey.cpu().numpy() + 0.01 * ky / k2 * np.sin(arg))) < 2e-6
-    rate, period = _landau_rate(ctx, f, 0.008, 6, 420)        # sum_d |a_d| dt / Delta_d <= 0.09 < 0.13 (n = 4 RK3 limit)
+    assert 0.008 < ctx.max_stable_dt(0.05) < 0.02             # sum_d |a_d| dt / Delta_d against the n = 4 RK3 limit 0.13
+    rate, period = _landau_rate(ctx, f, 0.008, 6, 420)
     assert -0.165 < rate < -0.143, rate
     assert abs(period - math.pi / 1.4156) < 0.08
     assert ctx.last_kernel == "rhs4_tile<8>"
