@@ -378,6 +378,27 @@ def run_config4(args, name):
 CONFIG6 = {"config6_2d2v_128^4": 32, "config6_2d2v_64^4": 16}
 
 
+def oracle_sample_2d2v(dt):
+    """Three SSP-RK3 steps of oracle.vlasov2d2v on a (4, 4, 32, 32)-element slab (4/32 of the x and y elements of the 128^4
+    grid, periodic within the slab, full velocity grid): about 10-20 s of host time."""
+    from oracle import vlasov2d2v as o4
+    import workloads as wl
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+    L = 2 * math.pi / K_WAVE
+    g = o4.make_grid((4, 4, 32, 32), (4,) * 4, (0.0, 0.0, -8.5, -8.5), (L / 8, L / 8, 8.5, 8.5), omega_c=1.0, pmax=(4, 4))
+    x, y, u, v = [c.reshape(-1) for c in g.coords]
+    f = wl.ring2d_f0(x, y, u, v, K_WAVE, K_WAVE)
+    t0 = time.perf_counter()
+    for _ in range(3):
+        f = o4.ssprk3_step(g, f, dt)
+    wall = time.perf_counter() - t0
+    return f.size * 9.0 / wall, cores, f"oracle.vlasov2d2v.ssprk3_step (NumPy), (4, 4, 32, 32) x 4^4 slab = {f.size} DOF, 3 steps"
+
+
 def run_config6(args, name):
     """2D2V: N^4 elements x 4^4 LGL nodes, ring workload in (v_x, v_y) with a seeded perturbation in x and y,
     one SSP-RK3 step with the 2-D Poisson solve at every stage (dg4_ssprk3_run)."""
@@ -424,7 +445,12 @@ def run_config6(args, name):
     for _ in range(e2e_steps):
         ctx.ssprk3_run_host(fh, dt, 1)
     e2e_s = time.perf_counter() - t0
+    cpu = None
+    if not args.no_cpu_baseline:
+        cv, cc, cd = oracle_sample_2d2v(dt)
+        cpu = {"value": cv, "unit": UNIT, "cores": cc, "kind": "oracle", "sample": cd}
     print(json.dumps({
+        "cpu_baseline": cpu,
         "metric": "FP64 phase-space DOF-updates/s per RK stage", "value": dof * 3.0 * args.steps / (ms * 1e-3), "unit": UNIT,
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
