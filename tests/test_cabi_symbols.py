@@ -42,6 +42,24 @@ def test_binding_loads_without_gpu_and_reports_errors():
     assert lib.dg_create(ctypes.byref(d), ctypes.byref(h)) == -2      # DG_ERR_UNSUPPORTED: order > 10
 
 
+def test_2d2v_argument_validation_without_gpu():
+    from paper_2202_13532_b200 import _lib
+    lib = _lib.load()
+    h = ctypes.c_void_p()
+    assert lib.dg4_create(None, ctypes.byref(h)) == -1
+    d = _lib.GridDesc4()
+    for i in range(4):
+        d.nelem[i], d.order[i], d.lo[i], d.hi[i] = 2, 4, 0.0, 1.0
+    d.order[3] = 11
+    assert lib.dg4_create(ctypes.byref(d), ctypes.byref(h)) == -2      # DG_ERR_UNSUPPORTED: order > 10
+    d.order[3] = 4
+    d.bc[2] = 2
+    assert lib.dg4_create(ctypes.byref(d), ctypes.byref(h)) == -1      # no halo boundary in the 2D2V context
+    assert b"bc" in lib.dg_last_error()
+    assert lib.dg4_workspace_bytes(None) == 0 and lib.dg4_launch_count(None) == 0
+    assert lib.dg4_rhs(None, None, None, None, None, None) == -1
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_2202_13532_b200")
     for dirpath, _, files in os.walk(pkg):
