@@ -269,8 +269,8 @@ static int launch_rhs4(dg4_ctx* ctx, const double* f, const double* fn, const do
 // Density partials of f over the (u, v) plane of every (g_x, g_y): the 1D2V density kernels with (g_x, g_y) flattened.
 static int launch_density4_partials(dg4_ctx* ctx, const double* f, int* nchunks_out, cudaStream_t st) {
   const int GXY = ctx->G[0] * ctx->G[1], G2 = ctx->G[2], G3 = ctx->G[3];
-  if (GXY > 65535) return fail(DG_ERR_UNSUPPORTED, "dg4_density: G_x G_y above 65535");
   if (!ctx->partials) return fail(DG_ERR_WORKSPACE, "dg4: set a workspace first");
+  const size_t plane = (size_t)G2 * G3;
   int nchunks, rows;
   if (G3 % 2 == 0 && ((uintptr_t)f & 15) == 0) {
     int CP = 1;
@@ -280,17 +280,26 @@ static int launch_density4_partials(dg4_ctx* ctx, const double* f, int* nchunks_
     while (rows > 8 * RL && (long long)((G2 + rows - 1) / rows) * GXY < 148LL * 16) rows /= 2;
     nchunks = (G2 + rows - 1) / rows;
     if ((size_t)nchunks * GXY <= ctx->partials_doubles) {
-      dim3 grid(nchunks, GXY);
-      dgk::density_partial_vec_kernel<8><<<grid, 256, 0, st>>>(f, ctx->d_wq[2], ctx->d_wq[3], G2, G3, rows, CP, ctx->partials);
+      for (int g0 = 0; g0 < GXY; g0 += 65535) {            // grid.y is limited to 65535 (g_x, g_y) pairs per launch
+        dim3 grid(nchunks, GXY - g0 < 65535 ? GXY - g0 : 65535);
+        dgk::density_partial_vec_kernel<8><<<grid, 256, 0, st>>>(f + g0 * plane, ctx->d_wq[2], ctx->d_wq[3], G2, G3, rows, CP,
+                                                                 ctx->partials + (size_t)g0 * nchunks);
+        int rc = check4(ctx, "density_partial_vec_kernel");
+        if (rc) return rc;
+      }
       *nchunks_out = nchunks;
-      return check4(ctx, "density_partial_vec_kernel");
+      return DG_OK;
     }
   }
   rows = G2; nchunks = 1;
-  dim3 grid(nchunks, GXY);
-  dgk::density_partial_kernel<<<grid, 256, 0, st>>>(f, ctx->d_wq[2], ctx->d_wq[3], G2, G3, rows, ctx->partials);
+  for (int g0 = 0; g0 < GXY; g0 += 65535) {
+    dim3 grid(nchunks, GXY - g0 < 65535 ? GXY - g0 : 65535);
+    dgk::density_partial_kernel<<<grid, 256, 0, st>>>(f + g0 * plane, ctx->d_wq[2], ctx->d_wq[3], G2, G3, rows, ctx->partials + g0);
+    int rc = check4(ctx, "density_partial_kernel");
+    if (rc) return rc;
+  }
   *nchunks_out = nchunks;
-  return check4(ctx, "density_partial_kernel");
+  return DG_OK;
 }
 
 static int launch_density4_finish(dg4_ctx* ctx, int nchunks, double* rho, cudaStream_t st) {

@@ -285,3 +285,14 @@ def test_cyclotron_rotation_2d2v():
     assert np.max(np.abs(f - ccw[None, None])) < 0.02
     assert np.max(np.abs(f - cw[None, None])) > 0.5
     ctx.close()
+
+
+def test_density_with_more_than_65535_space_nodes():
+    """G_x G_y = 66 564 (x, y) pairs: the density kernels run in slices of the launch grid; sampled against the definition."""
+    N, n = (43, 43, 1, 2), (6, 6, 2, 4)
+    g, ctx = make_pair(N, n)
+    dof = int(np.prod(g.flat_shape))
+    f = wl.counter_uniform_chunked(wl.SEED_CFG6_NOISE, dof).reshape(g.flat_shape)
+    rho = ctx.density(dev(f)).cpu().numpy()
+    assert relerr(rho, o4.density(g, f)) < 1e-13
+    ctx.close()
