@@ -72,7 +72,9 @@ int dg4_get_nodes(const dg4_ctx* ctx, int32_t dim, double* coords_host /*[N_d*n_
 /* Largest dt with sum_d |a_d| dt / Delta_d within the SSP-RK3 limit of this order and mass mode at |E_x|, |E_y| <= E_bound
  * (as dg_max_stable_dt). */
 double dg4_max_stable_dt(const dg4_ctx* ctx, double E_bound);
-#define DG4_OPT_RHS_KERNEL 1   /* 0 auto (tiled when all orders are 4 and N_v is even), 1 generic, 2 tiled (error if unsupported) */
+#define DG4_OPT_RHS_KERNEL 1   /* 0 auto (tiled when all orders are 4 and N_v is even; element kernel for equal orders 6 or 8;
+                                  else generic), 1 generic, 2 tiled, 3 element kernel (equal orders 4, 6, 8); 2 and 3 fail with
+                                  DG_ERR_UNSUPPORTED on other shapes */
 #define DG4_OPT_PROFILE    3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
 int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value);
 int dg4_get_profile(dg4_ctx* ctx, double* rhs_ms_total_host, int64_t* rhs_launches_host, int32_t reset);

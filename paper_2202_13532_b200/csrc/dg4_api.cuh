@@ -4,6 +4,7 @@
 #include "../../include/dgvlasov2d2v.h"
 #include "dg4_kernels.cuh"
 #include "dg4_kernels_tiled.cuh"
+#include "dg4_kernels_elem.cuh"
 
 struct dg4_ctx {
   dg4_grid_desc desc;
@@ -25,7 +26,7 @@ struct dg4_ctx {
   double* f_stage = nullptr;
   int64_t launches = 0;
   int opt_kernel = 0, opt_profile = 0;
-  bool smem_attr_done = false;
+  bool smem_attr_done = false, elem_attr_done = false;
   std::vector<cudaEvent_t> prof_events;
   double prof_ms = 0.0;
   int64_t prof_launches = 0;
@@ -37,6 +38,13 @@ static int check4(dg4_ctx* ctx, const char* what) {
   if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
   ctx->launches += 1;
   return DG_OK;
+}
+
+static int elem_order(const dg4_ctx* ctx) {     // order of the element kernel, 0 = unsupported
+  const int n = ctx->n[0];
+  for (int d = 1; d < 4; ++d) if (ctx->n[d] != n) return 0;
+  if (ctx->N[1] > 65535 || ctx->N[0] > 65535) return 0;
+  return (n == 4 || n == 6 || n == 8) ? n : 0;
 }
 
 static int tile_kv(const dg4_ctx* ctx) {       // v-elements per tile of the tiled kernel, 0 = unsupported
@@ -157,6 +165,7 @@ static size_t partials4_doubles(const dg4_ctx* ctx) {
   size_t per = 64;                                           // density_partial kernels: chunks per (g_x, g_y)
   const int kv = tile_kv(ctx);
   if (kv && (size_t)ctx->N[2] * (ctx->N[3] / kv) > per) per = (size_t)ctx->N[2] * (ctx->N[3] / kv);
+  if (elem_order(ctx) && (size_t)ctx->N[2] * ctx->N[3] > per) per = (size_t)ctx->N[2] * ctx->N[3];
   return (size_t)ctx->G[0] * ctx->G[1] * per;
 }
 
@@ -211,7 +220,7 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
   const bool aligned = (((uintptr_t)f | (uintptr_t)out | (uintptr_t)fn) & 15) == 0;
   if (ctx->opt_kernel == 2 && !(kv && aligned))
     return fail(DG_ERR_UNSUPPORTED, "dg4: the tiled kernel needs order 4 in all dimensions, an even N_v and 16-byte aligned arrays");
-  if (kv && aligned && ctx->opt_kernel != 1) {
+  if (kv && aligned && (ctx->opt_kernel == 0 || ctx->opt_kernel == 2)) {
     for (int i = 0; i < 16; ++i) p.U[i] = ctx->basis[0].ups[i];
     for (int i = 0; i < 8; ++i) p.Xi[i] = ctx->basis[0].lift[i];
     p.wqu = ctx->d_wq[2]; p.wqv = ctx->d_wq[3];
@@ -244,6 +253,31 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
     else dg4::rhs4_tile_kernel<2, 1><<<tiles, 32, smem, st>>>(p);
     ctx->last_kernel = kv == 8 ? "rhs4_tile<8>" : (kv == 4 ? "rhs4_tile<4>" : "rhs4_tile<2>");
     return check4(ctx, "rhs4_tile_kernel");
+  }
+  const int ne = elem_order(ctx);
+  if (ctx->opt_kernel == 3 && !(ne && aligned))
+    return fail(DG_ERR_UNSUPPORTED, "dg4: the element kernel needs equal orders 4, 6 or 8 and 16-byte aligned arrays");
+  if (ne && aligned && (ctx->opt_kernel == 3 || (ctx->opt_kernel == 0 && ne != 4))) {
+    for (int i = 0; i < ne * ne; ++i) p.Un[i] = ctx->basis[0].ups[i];
+    for (int i = 0; i < 2 * ne; ++i) p.Xin[i] = ctx->basis[0].lift[i];
+    p.wqu = ctx->d_wq[2]; p.wqv = ctx->d_wq[3];
+    p.chunks = ctx->N[2] * ctx->N[3];
+    if (want_partials && mode != 0 && ctx->partials && (size_t)ctx->G[0] * ctx->G[1] * p.chunks <= ctx->partials_doubles) {
+      p.partials = ctx->partials;
+      if (chunks_out) *chunks_out = p.chunks;
+    }
+    const dim3 grid(ctx->N[3] * ctx->N[2], ctx->N[1], ctx->N[0]);
+    if (ne == 8) {
+      const size_t smem = sizeof(double) * dg4::elem_smem_doubles<8>();
+      if (!ctx->elem_attr_done) {
+        CUDA_TRY(cudaFuncSetAttribute(dg4::rhs4_elem_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ctx->elem_attr_done = true;
+      }
+      dg4::rhs4_elem_kernel<8><<<grid, 512, smem, st>>>(p);
+    } else if (ne == 6) dg4::rhs4_elem_kernel<6><<<grid, 216, sizeof(double) * dg4::elem_smem_doubles<6>(), st>>>(p);
+    else dg4::rhs4_elem_kernel<4><<<grid, 64, sizeof(double) * dg4::elem_smem_doubles<4>(), st>>>(p);
+    ctx->last_kernel = ne == 8 ? "rhs4_elem<8>" : (ne == 6 ? "rhs4_elem<6>" : "rhs4_elem<4>");
+    return check4(ctx, "rhs4_elem_kernel");
   }
   long long blocks = ((long long)ctx->dof + 255) / 256;
   if (blocks > 148LL * 64) blocks = 148LL * 64;
@@ -437,7 +471,7 @@ extern "C" double dg4_max_stable_dt(const dg4_ctx* ctx, double E_bound) {
 
 extern "C" int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_set_option: null context");
-  if (key == DG4_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_kernel = (int)value; return DG_OK; }
+  if (key == DG4_OPT_RHS_KERNEL && value >= 0 && value <= 3) { ctx->opt_kernel = (int)value; return DG_OK; }
   if (key == DG4_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg4_set_option: unknown key or value");
 }

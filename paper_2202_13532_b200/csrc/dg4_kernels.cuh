@@ -12,6 +12,7 @@ struct Params {
   const double* ups[4];      // reference Upsilon [n][n] (generic kernel)
   const double* lift[4];     // reference Xi [n][2]
   double U[16], Xi[8];       // the same operators for n = 4 (tiled kernel: kernel-parameter constant bank)
+  double Un[64], Xin[16];    // ... and for the element kernel's order n <= 8: Un[j*n + k], Xin[2*j + {L,R}]
   double omega_c;
   const double* Ex;          // [G0*G1] or nullptr
   const double* Ey;

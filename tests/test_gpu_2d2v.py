@@ -45,7 +45,8 @@ def seeded_inputs(g):
 
 # (N, n): generic kernel for mixed orders, tiled kernel <2>, <4>, <8> for n = 4 (several tiles + zero-inflow / periodic edges)
 SHAPES = [((3, 2, 3, 4), (3, 4, 5, 2)), ((2, 3, 2, 3), (4, 4, 4, 4)), ((3, 2, 3, 2), (4, 4, 4, 4)), ((2, 3, 3, 4), (4, 4, 4, 4)),
-          ((3, 2, 2, 8), (4, 4, 4, 4)), ((2, 2, 3, 16), (4, 4, 4, 4)), ((2, 2, 2, 2), (6, 6, 6, 6))]
+          ((3, 2, 2, 8), (4, 4, 4, 4)), ((2, 2, 3, 16), (4, 4, 4, 4)), ((2, 2, 2, 2), (6, 6, 6, 6)), ((3, 2, 3, 2), (6, 6, 6, 6)),
+          ((2, 3, 1, 2), (8, 8, 8, 8)), ((1, 1, 2, 3), (8, 8, 8, 8)), ((2, 2, 2, 2), (5, 5, 5, 5))]
 
 
 @pytest.mark.parametrize("N,n", SHAPES)
@@ -57,8 +58,13 @@ def test_rhs_matches_oracle(N, n, bc, mode):
     r = ctx.rhs(dev(f), dev(Ex), dev(Ey)).cpu().numpy()
     ro = o4.rhs(g, f, Ex, Ey)
     assert relerr(r, ro) < 1e-12, ctx.last_kernel
-    expect_tiled = all(k == 4 for k in n) and N[3] % 2 == 0
-    assert ctx.last_kernel.startswith("rhs4_tile" if expect_tiled else "rhs4_generic")
+    if all(k == 4 for k in n) and N[3] % 2 == 0:
+        expect = "rhs4_tile"
+    elif n in ((6, 6, 6, 6), (8, 8, 8, 8)):
+        expect = "rhs4_elem"
+    else:
+        expect = "rhs4_generic"
+    assert ctx.last_kernel.startswith(expect), ctx.last_kernel
     ctx.close()
 
 
@@ -73,6 +79,30 @@ def test_tiled_equals_generic_kernel():
     assert ctx.last_kernel == "rhs4_generic"
     assert relerr(a, b) < 1e-13
     assert relerr(a, o4.rhs(g, f, Ex, Ey)) < 1e-12
+    ctx.close()
+
+
+@pytest.mark.parametrize("N,n", [((3, 2, 3, 3), (4, 4, 4, 4)), ((2, 2, 2, 8), (4, 4, 4, 4)), ((2, 2, 3, 2), (6, 6, 6, 6)), ((2, 1, 2, 2), (8, 8, 8, 8))])
+@pytest.mark.parametrize("bc", [(0, 0, 1, 1), (1, 1, 0, 0)])
+def test_element_kernel_stage_and_density(N, n, bc):
+    """rhs4_elem_kernel forced (DG4_OPT_RHS_KERNEL = 3): one Shu-Osher stage with f_n and the epilogue density, and the RHS
+    against the generic kernel on the device."""
+    g, ctx = make_pair(N, n, bc=bc)
+    ctx.set_option(api().OPT4_RHS_KERNEL, 3)
+    f, Ex, Ey = seeded_inputs(g)
+    fn = 0.5 + wl.counter_uniform_chunked(wl.SEED_CFG6_E, f.size).reshape(f.shape)
+    fd, fnd, exd, eyd = dev(f), dev(fn), dev(Ex), dev(Ey)
+    out, rho = torch.empty_like(fd), torch.empty(g.flat_shape[:2], dtype=torch.float64, device="cuda")
+    ctx.rk_stage(fd, fnd, exd, eyd, out, 1.0 / 3.0, 2.0 / 3.0, 1e-3, rho_out=rho)
+    assert ctx.last_kernel.startswith("rhs4_elem")
+    ro = o4.rhs(g, f, Ex, Ey)
+    oo = (1.0 / 3.0) * fn + (2.0 / 3.0) * (f + 1e-3 * ro)
+    assert relerr(out.cpu().numpy(), oo) < 1e-13
+    assert relerr(rho.cpu().numpy(), o4.density(g, oo)) < 1e-13
+    a = ctx.rhs(fd, exd, eyd).cpu().numpy()
+    ctx.set_option(api().OPT4_RHS_KERNEL, 1)
+    b = ctx.rhs(fd, exd, eyd).cpu().numpy()
+    assert relerr(a, ro) < 1e-12 and relerr(a, b) < 1e-13
     ctx.close()
 
 
@@ -127,7 +157,7 @@ def test_plane_wave_field_closed_form():
     ctx.close()
 
 
-@pytest.mark.parametrize("N,n", [((3, 2, 3, 8), (4, 4, 4, 4)), ((2, 2, 3, 2), (3, 4, 4, 3))])
+@pytest.mark.parametrize("N,n", [((3, 2, 3, 8), (4, 4, 4, 4)), ((2, 2, 3, 2), (3, 4, 4, 3)), ((2, 2, 2, 3), (6, 6, 6, 6)), ((1, 2, 2, 2), (8, 8, 8, 8))])
 def test_self_consistent_steps_match_oracle(N, n):
     """Ring workload, three SSP-RK3 steps with the 2-D Poisson solve at every stage (density partials from the tile epilogue)."""
     g, ctx = make_pair(N, n, omega_c=1.0, lo=(0.0, 0.0, -8.5, -8.5), hi=(20 * math.pi, 10 * math.pi, 8.5, 8.5))
