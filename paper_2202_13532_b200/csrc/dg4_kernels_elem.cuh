@@ -22,17 +22,19 @@ namespace dg4 {
 template <int n>
 constexpr int elem_pitch() { return n == 8 ? 10 : n; }            // doubles per shared-memory row
 template <int n>
-constexpr int elem_smem_doubles() { return n * n * n * elem_pitch<n>() + 5 * n * n * n + n * n * n; }
+constexpr int elem_smem_doubles() { return n * n * n * elem_pitch<n>() + 5 * n * n * elem_pitch<n>() + n * n * n + 2 * n + n * (n + 1) + (n * (n + 1)) % 2; }
 
 template <int n>
 __global__ void __launch_bounds__(n * n * n, 1) rhs4_elem_kernel(const Params p) {
   constexpr int NT = n * n * n, RP = elem_pitch<n>(), H = n / 2;
   extern __shared__ double2 esm_raw[];
   double* T = reinterpret_cast<double*>(esm_raw);                 // [n^3][RP] v lines of the element
-  double* hx = T + NT * RP;                                       // [n^2 (jy, ju)][n]
-  double* hy = hx + n * n * n;                                    // [2][n^2 (jx, ju)][n]
-  double* hu = hy + 2 * n * n * n;                                // [2][n^2 (jx, jy)][n]
-  double* red = hu + 2 * n * n * n;                               // [n^3]
+  double* hx = T + NT * RP;                                       // [n^2 (jy, ju)][RP]
+  double* hy = hx + n * n * RP;                                   // [2][n^2 (jx, ju)][RP]
+  double* hu = hy + 2 * n * n * RP;                               // [2][n^2 (jx, jy)][RP]
+  double* red = hu + 2 * n * n * RP;                              // [n^3]
+  double* Xs = red + n * n * n;                                   // [n][2] lift
+  double* Us = Xs + 2 * n;                                   // [n][n+1]: the per-thread operator rows (padded: conflict-free)
   const int tid = threadIdx.x;
   const int ju = tid % n, jy = (tid / n) % n, jx = tid / (n * n);
   const int eu = blockIdx.x / p.N[3], ev = blockIdx.x - eu * p.N[3], ey = blockIdx.y, ex = blockIdx.z;
@@ -65,17 +67,17 @@ __global__ void __launch_bounds__(n * n * n, 1) rhs4_elem_kernel(const Params p)
       if (u > 0.0) g = ex > 0 ? gx0 - 1 : (p.bc[0] == 0 ? p.G[0] - 1 : -1);
       else if (u < 0.0) g = ex < p.N[0] - 1 ? gx0 + n : (p.bc[0] == 0 ? 0 : -1);
       if (g >= 0) src = g * s0 + (gy0 + a) * s1 + (gu0 + b) * s2 + gv0;
-      dst = hx + rr * n;
+      dst = hx + rr * RP;
     } else if (which <= 2) {                                      // (jx, ju) = (a, b)
       const int g = which == 1 ? (ey > 0 ? gy0 - 1 : (p.bc[1] == 0 ? p.G[1] - 1 : -1))
                                : (ey < p.N[1] - 1 ? gy0 + n : (p.bc[1] == 0 ? 0 : -1));
       if (g >= 0) src = (gx0 + a) * s0 + g * s1 + (gu0 + b) * s2 + gv0;
-      dst = hy + ((which - 1) * n * n + rr) * n;
+      dst = hy + ((which - 1) * n * n + rr) * RP;
     } else {                                                      // (jx, jy) = (a, b)
       const int g = which == 3 ? (eu > 0 ? gu0 - 1 : (p.bc[2] == 0 ? p.G[2] - 1 : -1))
                                : (eu < p.N[2] - 1 ? gu0 + n : (p.bc[2] == 0 ? 0 : -1));
       if (g >= 0) src = (gx0 + a) * s0 + (gy0 + b) * s1 + g * s2 + gv0;
-      dst = hu + ((which - 3) * n * n + rr) * n;
+      dst = hu + ((which - 3) * n * n + rr) * RP;
     }
     double2* d2 = reinterpret_cast<double2*>(dst);
     if (src >= 0) {
@@ -103,6 +105,8 @@ __global__ void __launch_bounds__(n * n * n, 1) rhs4_elem_kernel(const Params p)
     else if (a_v < 0.0) g = ev < p.N[3] - 1 ? gv0 + n : (p.bc[3] == 0 ? 0 : -1);
     if (g >= 0) vface = __ldg(p.f + line_off - gv0 + g);
   }
+  if (tid < n * n) Us[(tid / n) * (n + 1) + tid % n] = p.Un[tid];
+  if (tid < 2 * n) Xs[tid] = p.Xin[tid];
   // own line to shared memory
   {
     double2* t2 = reinterpret_cast<double2*>(T + tid * RP);
@@ -131,12 +135,14 @@ __global__ void __launch_bounds__(n * n * n, 1) rhs4_elem_kernel(const Params p)
     const int jd = d == 2 ? ju : (d == 1 ? jy : jx);
     const int row0 = d == 2 ? tid - ju : (d == 1 ? tid - jy * n : tid - jx * n * n);
     const int rstep = d == 2 ? 1 : (d == 1 ? n : n * n);
-    double acc[n], first[n], last[n];
+    double acc[n], first[n], last[n], cf[n];
+#pragma unroll
+    for (int k = 0; k < n; ++k) cf[k] = Us[jd * (n + 1) + k];
 #pragma unroll
     for (int j = 0; j < n; ++j) acc[j] = 0.0;
 #pragma unroll
     for (int k = 0; k < n; ++k) {
-      const double c = p.Un[jd * n + k];
+      const double c = cf[k];
       const double2* t2 = reinterpret_cast<const double2*>(T + (row0 + k * rstep) * RP);
 #pragma unroll
       for (int h = 0; h < H; ++h) {
@@ -146,13 +152,19 @@ __global__ void __launch_bounds__(n * n * n, 1) rhs4_elem_kernel(const Params p)
         if (k == n - 1) { last[2 * h] = a.x; last[2 * h + 1] = a.y; }
       }
     }
-    const double xl = p.Xin[2 * jd], xr = p.Xin[2 * jd + 1];
-    const double* lo = d == 2 ? hu + (jx * n + jy) * n : (d == 1 ? hy + (jx * n + ju) * n : hx + (jy * n + ju) * n);
-    const double* hi = d == 0 ? lo : lo + n * n * n;
+    const double xl = Xs[2 * jd], xr = Xs[2 * jd + 1];
+    const double* lo = d == 2 ? hu + (jx * n + jy) * RP : (d == 1 ? hy + (jx * n + ju) * RP : hx + (jy * n + ju) * RP);
+    const double* hi = d == 0 ? lo : lo + n * n * RP;
+    double flo[n], fhi[n];
+#pragma unroll
+    for (int h = 0; h < H; ++h) {
+      const double2 a = reinterpret_cast<const double2*>(lo)[h], b = reinterpret_cast<const double2*>(hi)[h];
+      flo[2 * h] = a.x; flo[2 * h + 1] = a.y; fhi[2 * h] = b.x; fhi[2 * h + 1] = b.y;
+    }
 #pragma unroll
     for (int j = 0; j < n; ++j) {
       const double a = d == 2 ? -exf - p.omega_c * vv[j] : (d == 1 ? vv[j] : uu);
-      const double uL = a > 0.0 ? lo[j] : first[j], uR = a > 0.0 ? last[j] : hi[j];
+      const double uL = a > 0.0 ? flo[j] : first[j], uR = a > 0.0 ? last[j] : fhi[j];
       rhs[j] = fma(p.J[d] * a, acc[j] - xr * uR + xl * uL, rhs[j]);
     }
   }
