@@ -17,8 +17,19 @@
 
 namespace dg4 {
 
+// Shared-memory position of element j of v line (row) r.  n = 8: one 64-byte pad after every 8 rows (rows 8 apart -- the
+// lines of two neighbouring (x, y) nodes in the u phase -- then sit in opposite halves of a 128-byte bank line) and the 16-byte
+// chunks of a row XORed with (r / 2) mod 4 (the 8 rows a quarter-warp stores in the v phase hit 8 distinct bank groups); the
+// lanes of every other access run along j inside one row, where any permutation is conflict-free.
 template <int n>
-constexpr int elem_smem_doubles() { return 2 * n * n * n * n; }
+__device__ __forceinline__ int eaddr(int r, int j) {
+  if (n == 8) return r * 8 + (r >> 3) * 8 + ((((j >> 1) ^ (r >> 1)) & 3) << 1) + (j & 1);
+  return r * n + j;
+}
+template <int n>
+constexpr int elem_array_doubles() { return n == 8 ? n * n * n * n + n * n * n : n * n * n * n; }
+template <int n>
+constexpr int elem_smem_doubles() { return 2 * elem_array_doubles<n>(); }
 
 // Contraction + lift of one line: out[j] = s * ( sum_k U[j][k] f[k] - XiR[j] uR + XiL[j] uL ).
 template <int n>
@@ -47,7 +58,7 @@ __global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : 1)) rhs4_elem_kernel(
   constexpr int H = n / 2, n2 = n * n, n3 = n * n * n;
   extern __shared__ double2 esm_raw[];
   double* T = reinterpret_cast<double*>(esm_raw);                 // [jx][jy][ju][jv] values of f
-  double* A = T + n3 * n;                                         // the running sums, same layout
+  double* A = T + elem_array_doubles<n>();                        // the running sums, same layout
   const int tid = threadIdx.x;
   const int c0 = tid % n, c1 = (tid / n) % n, c2 = tid / n2;      // c0 fastest
   const int eu = blockIdx.x / p.N[3], ev = blockIdx.x - eu * p.N[3], ey = blockIdx.y, ex = blockIdx.z;
@@ -67,22 +78,20 @@ __global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : 1)) rhs4_elem_kernel(
     const double a = -eyf + p.omega_c * p.coord[2][gu0 + c0];
     const int g = upwind_index(p, 3, ev, n, a);
     const double ext = g >= 0 ? __ldg(p.f + line_off - gv0 + g) : 0.0;
-    double2* t2 = reinterpret_cast<double2*>(T + tid * n);
 #pragma unroll
-    for (int c = 0; c < H; ++c) t2[c] = make_double2(f[2 * c], f[2 * c + 1]);
+    for (int c = 0; c < H; ++c) *reinterpret_cast<double2*>(T + eaddr<n>(tid, 2 * c)) = make_double2(f[2 * c], f[2 * c + 1]);
     line_op<n>(p, f, a, p.J[3], ext, o);
-    double2* a2 = reinterpret_cast<double2*>(A + tid * n);
 #pragma unroll
-    for (int c = 0; c < H; ++c) a2[c] = make_double2(o[2 * c], o[2 * c + 1]);
+    for (int c = 0; c < H; ++c) *reinterpret_cast<double2*>(A + eaddr<n>(tid, 2 * c)) = make_double2(o[2 * c], o[2 * c + 1]);
   }
   __syncthreads();
 
   // ---- phase u: thread = (jx, jy, jv) = (c2, c1, c0); line over ju at stride n ---------------------------------------
   {
-    const int base = (c2 * n + c1) * n2 + c0;
+    const int row = (c2 * n + c1) * n;                                // + k
     double f[n], o[n];
 #pragma unroll
-    for (int k = 0; k < n; ++k) f[k] = T[base + k * n];
+    for (int k = 0; k < n; ++k) f[k] = T[eaddr<n>(row + k, c0)];
     const long long gxy = (long long)(gx0 + c2) * p.G[1] + gy0 + c1;
     const double exf = p.Ex ? __ldg(p.Ex + gxy) : 0.0;
     const double a = -exf - p.omega_c * p.coord[3][gv0 + c0];
@@ -90,31 +99,31 @@ __global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : 1)) rhs4_elem_kernel(
     const double ext = g >= 0 ? __ldg(p.f + elem_off - gu0 * s2 + c2 * s0 + c1 * s1 + g * s2 + c0) : 0.0;
     line_op<n>(p, f, a, p.J[2], ext, o);
 #pragma unroll
-    for (int k = 0; k < n; ++k) A[base + k * n] += o[k];
+    for (int k = 0; k < n; ++k) A[eaddr<n>(row + k, c0)] += o[k];
   }
   __syncthreads();
 
   // ---- phase y: thread = (jx, ju, jv) = (c2, c1, c0); line over jy at stride n^2 -------------------------------------
   {
-    const int base = c2 * n3 + c1 * n + c0;
+    const int row = c2 * n2 + c1;                                     // + k n
     double f[n], o[n];
 #pragma unroll
-    for (int k = 0; k < n; ++k) f[k] = T[base + k * n2];
+    for (int k = 0; k < n; ++k) f[k] = T[eaddr<n>(row + k * n, c0)];
     const double a = p.coord[3][gv0 + c0];
     const int g = upwind_index(p, 1, ey, n, a);
     const double ext = g >= 0 ? __ldg(p.f + elem_off - gy0 * s1 + c2 * s0 + g * s1 + c1 * s2 + c0) : 0.0;
     line_op<n>(p, f, a, p.J[1], ext, o);
 #pragma unroll
-    for (int k = 0; k < n; ++k) A[base + k * n2] += o[k];
+    for (int k = 0; k < n; ++k) A[eaddr<n>(row + k * n, c0)] += o[k];
   }
   __syncthreads();
 
   // ---- phase x: thread = (jy, ju, jv) = (c2, c1, c0); line over jx at stride n^3; epilogue ---------------------------
   {
-    const int base = c2 * n2 + c1 * n + c0;
+    const int row = c2 * n + c1;                                      // + k n^2
     double f[n], o[n];
 #pragma unroll
-    for (int k = 0; k < n; ++k) f[k] = T[base + k * n3];
+    for (int k = 0; k < n; ++k) f[k] = T[eaddr<n>(row + k * n2, c0)];
     const double a = p.coord[2][gu0 + c1];
     const int g = upwind_index(p, 0, ex, n, a);
     const long long node_off = elem_off + c2 * s1 + c1 * s2 + c0;          // + jx * s0
@@ -128,7 +137,7 @@ __global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : 1)) rhs4_elem_kernel(
     const double w = p.partials ? p.wqu[gu0 + c1] * p.wqv[gv0 + c0] : 0.0;
 #pragma unroll
     for (int k = 0; k < n; ++k) {
-      double r = o[k] + A[base + k * n3];
+      double r = o[k] + A[eaddr<n>(row + k * n2, c0)];
       if (p.mode != 0) {
         r = p.c1 * fma(p.dt, r, f[k]);
         if (use_fn) r = fma(p.c0, fnv[k], r);
@@ -140,11 +149,11 @@ __global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : 1)) rhs4_elem_kernel(
       // density of the element at (jx, jy): sum over (ju, jv) in a fixed order
       // (each thread overwrites the sums it has just consumed: A becomes the weighted outputs, [jx][jy][ju*n + jv])
 #pragma unroll
-      for (int k = 0; k < n; ++k) A[base + k * n3] = o[k];
+      for (int k = 0; k < n; ++k) A[eaddr<n>(row + k * n2, c0)] = o[k];
       __syncthreads();
       if (tid < n2) {
         double s = 0.0;
-        for (int i = 0; i < n2; ++i) s += A[tid * n2 + i];
+        for (int i = 0; i < n2; ++i) s += A[eaddr<n>(tid * n + i / n, i % n)];
         const int jx = tid / n, jy = tid - jx * n;
         p.partials[((long long)(gx0 + jx) * p.G[1] + gy0 + jy) * p.chunks + eu * p.N[3] + ev] = s;
       }
