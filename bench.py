@@ -408,6 +408,8 @@ def run_config6(args, name):
     N = CONFIG6[name]
     lo, hi = (0.0, 0.0, -8.5, -8.5), (2 * math.pi / K_WAVE, 2 * math.pi / K_WAVE, 8.5, 8.5)
     ctx = api.DG4Context((N,) * 4, (4,) * 4, lo, hi, bc=(0, 0, 1, 1), omega_c=1.0)
+    if args.rhs_kernel:
+        ctx.set_option(api.OPT4_RHS_KERNEL, args.rhs_kernel)
     x, y, u, v = (ctx.nodes(d) for d in range(4))
     f0 = wl.add_uniform_noise(wl.ring2d_f0(x, y, u, v, K_WAVE, K_WAVE), wl.SEED_CFG6_NOISE, 1e-4)
     f = torch.from_numpy(f0).cuda()
@@ -541,6 +543,7 @@ def main():
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "xslab", "xslab-push"],
                     help="N > 1: independent replicas (default, DESIGN.md section 9) or one problem sharded by x-slabs, with the "
                          "face planes exchanged by send/recv (xslab) or stored by the RHS kernel into peer memory (xslab-push)")
+    ap.add_argument("--rhs-kernel", type=int, default=0, help="config6 only: DG4_OPT_RHS_KERNEL (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -326,3 +326,4 @@ def test_density_with_more_than_65535_space_nodes():
     rho = ctx.density(dev(f)).cpu().numpy()
     assert relerr(rho, o4.density(g, f)) < 1e-13
     ctx.close()
+
