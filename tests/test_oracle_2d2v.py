@@ -123,3 +123,22 @@ def test_step_conserves_mass():
     m0 = np.einsum("gh,g,h->", v4.density(g, f), wx, wy)
     m1 = np.einsum("gh,g,h->", v4.density(g, f1), wx, wy)
     assert abs(m1 - m0) < 1e-13 * m0
+
+
+def test_free_streaming_exact_solution_and_convergence():
+    """omega_c = 0, E = 0, periodic x and y: f(x, y, u, v, t) = f0(x - u t, y - v t, u, v).  The nodal error of a smooth state
+    falls by more than a factor 10 when the space elements are halved at order 5 (spectral convergence of the x and y operators and of
+    the stepper together; a wrong sign or a swapped speed in the space terms gives an O(1) error)."""
+    def run(N):
+        g = v4.make_grid((N, N, 1, 1), (5, 5, 3, 3), lo=(0.0, 0.0, -1.0, -1.0), hi=(1.0, 1.0, 1.0, 1.0), bc=(0, 0, 0, 0), omega_c=0.0)
+        x, y, u, v = [c.reshape(-1) for c in g.coords]
+        def exact(t):
+            X = x[:, None, None, None] - u[None, None, :, None] * t
+            Y = y[None, :, None, None] - v[None, None, None, :] * t
+            return np.ascontiguousarray(np.broadcast_to(1.0 + 0.3 * np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Y), g.flat_shape))
+        f, dt, steps = exact(0.0), 2.5e-4, 80
+        for _ in range(steps):
+            f = v4.ssprk3_step(g, f, dt, self_consistent=False)
+        return np.max(np.abs(f - exact(dt * steps)))
+    e4, e8 = run(4), run(8)
+    assert e4 < 5e-4 and e8 < e4 / 10.0, (e4, e8)          # measured: 1.2e-4, 8.3e-6
