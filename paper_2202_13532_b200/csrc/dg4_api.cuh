@@ -244,11 +244,11 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
     const size_t smem = sizeof(double) * (kv == 8 ? dg4::tile_smem_doubles<8>(with_fn) : kv == 4 ? dg4::tile_smem_doubles<4>(with_fn)
                                                                                               : dg4::tile_smem_doubles<2>(with_fn));
     if (kv == 8 && !ctx->smem_attr_done) {
-      CUDA_TRY(cudaFuncSetAttribute(dg4::rhs4_tile_kernel<8, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+      CUDA_TRY(cudaFuncSetAttribute(dg4::rhs4_tile_kernel<8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(sizeof(double) * dg4::tile_smem_doubles<8>(true))));
       ctx->smem_attr_done = true;
     }
-    if (kv == 8) dg4::rhs4_tile_kernel<8, 3><<<tiles, 128, smem, st>>>(p);
+    if (kv == 8) dg4::rhs4_tile_kernel<8, 5><<<tiles, 128, smem, st>>>(p);
     else if (kv == 4) dg4::rhs4_tile_kernel<4, 1><<<tiles, 64, smem, st>>>(p);
     else dg4::rhs4_tile_kernel<2, 1><<<tiles, 32, smem, st>>>(p);
     ctx->last_kernel = kv == 8 ? "rhs4_tile<8>" : (kv == 4 ? "rhs4_tile<4>" : "rhs4_tile<2>");

@@ -2,11 +2,12 @@
 //
 // Tile = one (x, y, u) element x KV v-elements = 4 x 4 x 4 x (4 KV) nodes: 64 rows of R = 4 KV contiguous doubles
 // (KV = 8: 256-byte rows, 16 KB).  One CTA of 16 KV threads per tile.
-//   fill    EVERY global read of the CTA is a cp.async into shared memory issued at the top of the kernel -- the f_s tile
-//           and the f_n tile (16 bytes per request, chunk-swizzled so that both phases below are bank-conflict free), the
-//           upwind x / y face values of phase A (8 bytes per request, only the side the sign of u / v selects), both u-face
-//           rows and the two tile-edge v faces of phase B -- followed by ONE wait: a CTA pays the memory latency once and
-//           holds nothing in registers across it; 3 (stages with f_n, 66 KB) or 4 (50 KB) CTAs per SM overlap each other.
+//   fill    every global read of the CTA is issued at the top of the kernel, all but four scalars as cp.async into shared
+//           memory -- the f_s tile and the f_n tile (16 bytes per request, chunk-swizzled so that both phases below are
+//           bank-conflict free), the upwind x / y face values of phase A and the upwind u face values of phase B (8 bytes per
+//           request, only the side the sign of the speed selects) -- followed by ONE wait: a CTA pays the memory latency
+//           once.  The running sums of phase A replace f_n in its tile (c0 f_n + c1 dt (x and y parts)), so a CTA holds 44 KB
+//           and five CTAs (20 warps, 96 registers per thread) share an SM.
 //   phase A thread = (u node, v node of the tile) owns the 4 x 4 (x, y) nodes above it: x and y contractions + lifts in
 //           registers (the speeds a_x = u, a_y = v are per-thread constants), partial sums to shared memory.
 //   phase B thread = (x node, y node, v element) owns the 4 x 4 (u, v) nodes of that element: u and v contractions + lifts;
@@ -34,10 +35,10 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
 
-// Shared memory (doubles): f_s tile 64 R | partial sums 64 R | x faces 4 NT | y faces 4 NT | u faces 8 NT | v edge faces 128 |
-// f_n tile 64 R (only when the stage has an f_n).
+// Shared memory (doubles): f_s tile 64 R | f_n tile, then the running sums, 64 R | x faces 4 NT | y faces 4 NT | u faces 4 NT
+// (KV = 8: 44 KB, five CTAs per SM).
 template <int KV>
-constexpr int tile_smem_doubles(bool with_fn) { return (with_fn ? 3 : 2) * 64 * 4 * KV + 16 * (16 * KV) + 128; }
+constexpr int tile_smem_doubles(bool) { return 2 * 64 * 4 * KV + 12 * (16 * KV); }
 
 template <int KV, int MINB>
 __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p) {
@@ -47,9 +48,7 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
   double* accT = tile + ROWS * R;
   double* hXs = accT + ROWS * R;          // [jy][tid]
   double* hYs = hXs + 4 * NT;             // [jx][tid]
-  double* hUs = hYs + 4 * NT;             // double2 [lo0, lo1, hi0, hi1][tid]
-  double* eVs = hUs + 8 * NT;             // [side][row]
-  double* fnT = eVs + 128;
+  double* hUs = hYs + 4 * NT;             // [jv][tid]: the upwind u face of each of the thread's four u lines
   // grid = (N_v/KV * BX * N_u, N_y, N_x / BX), BX = 2^bx_log2 x-elements per group: consecutive CTAs walk v, then the x elements
   // of a group, then u -- the v, x and u neighbours of a tile are in flight with it and the y neighbour is N_u BX N_v/KV tiles
   // away (L2), where a row-major walk would put a whole x slab (G_y G_u G_v n doubles, more than the L2 on large grids)
@@ -103,40 +102,15 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
       px += s1; py += s0;
     }
   }
-  {
-    const int lo = eu > 0 ? gu0 - 1 : (p.bc[2] == 0 ? p.G[2] - 1 : -1);
-    const int hi = eu < p.N[2] - 1 ? gu0 + 4 : (p.bc[2] == 0 ? 0 : -1);
-    double2* h2 = reinterpret_cast<double2*>(hUs);
-    if (lo >= 0) {
-      cp_async16(h2 + tid, p.f + xy + lo * s2 + gvb);
-      cp_async16(h2 + NT + tid, p.f + xy + lo * s2 + gvb + 2);
-    } else { h2[tid] = make_double2(0.0, 0.0); h2[NT + tid] = make_double2(0.0, 0.0); }
-    if (hi >= 0) {
-      cp_async16(h2 + 2 * NT + tid, p.f + xy + hi * s2 + gvb);
-      cp_async16(h2 + 3 * NT + tid, p.f + xy + hi * s2 + gvb + 2);
-    } else { h2[2 * NT + tid] = make_double2(0.0, 0.0); h2[3 * NT + tid] = make_double2(0.0, 0.0); }
-  }
-  {
-    const int vlo = evb > 0 ? gv0 - 1 : (p.bc[3] == 0 ? p.G[3] - 1 : -1);
-    const int vhi = evb < nvb - 1 ? gv0 + R : (p.bc[3] == 0 ? 0 : -1);
-#pragma unroll
-    for (int t = tid; t < 128; t += NT) {
-      const int side = t >> 6, row = t & 63;
-      const int vv = side == 0 ? vlo : vhi;
-      if (vv >= 0) cp_async8(eVs + t, p.f + tile_off - gv0 + (row >> 4) * s0 + ((row >> 2) & 3) * s1 + (row & 3) * s2 + vv);
-      else eVs[t] = 0.0;
-    }
-  }
-  if (use_fn) {
+  if (use_fn) {                                                   // f_n lands where the running sums will live
     const double* src = p.fn + fill_off;
 #pragma unroll
     for (int jx = 0; jx < 4; ++jx) {
-      cp_async16(fnT + fill_dst + (16 * jx) * R, src);
-      cp_async16(fnT + fill_dst + (16 * jx + 8) * R, src + 2 * s1);
+      cp_async16(accT + fill_dst + (16 * jx) * R, src);
+      cp_async16(accT + fill_dst + (16 * jx + 8) * R, src + 2 * s1);
       src += s0;
     }
   }
-  asm volatile("cp.async.commit_group;" ::: "memory");
   const double exf = p.Ex ? __ldg(p.Ex + gxy) : 0.0, eyf = p.Ey ? __ldg(p.Ey + gxy) : 0.0;
   double au[4], av[4];
   {
@@ -144,6 +118,29 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
     const double2 u01 = *reinterpret_cast<const double2*>(p.coord[2] + gu0), u23 = *reinterpret_cast<const double2*>(p.coord[2] + gu0 + 2);
     au[0] = -exf - p.omega_c * v01.x; au[1] = -exf - p.omega_c * v01.y; au[2] = -exf - p.omega_c * v23.x; au[3] = -exf - p.omega_c * v23.y;
     av[0] = -eyf + p.omega_c * u01.x; av[1] = -eyf + p.omega_c * u01.y; av[2] = -eyf + p.omega_c * u23.x; av[3] = -eyf + p.omega_c * u23.y;
+  }
+  {
+    // u faces: one value per u line (fixed jv), from the row below or above the tile by the sign of a_u
+    const int lo = eu > 0 ? gu0 - 1 : (p.bc[2] == 0 ? p.G[2] - 1 : -1);
+    const int hi = eu < p.N[2] - 1 ? gu0 + 4 : (p.bc[2] == 0 ? 0 : -1);
+#pragma unroll
+    for (int jv = 0; jv < 4; ++jv) {
+      const int g = au[jv] > 0.0 ? lo : (au[jv] < 0.0 ? hi : -1);
+      if (g >= 0) cp_async8(hUs + jv * NT + tid, p.f + xy + g * s2 + gvb + jv);
+      else hUs[jv * NT + tid] = 0.0;
+    }
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  // v faces at the two tile edges: lanes ev = 0 (a_v > 0) and ev = KV-1 (a_v < 0) only, one scalar per u row
+  double eV[4] = {0.0, 0.0, 0.0, 0.0};
+  {
+    const int vlo = evb > 0 ? gv0 - 1 : (p.bc[3] == 0 ? p.G[3] - 1 : -1);
+    const int vhi = evb < nvb - 1 ? gv0 + R : (p.bc[3] == 0 ? 0 : -1);
+#pragma unroll
+    for (int ju = 0; ju < 4; ++ju) {
+      const int g = (ev == 0 && av[ju] > 0.0) ? vlo : ((ev == KV - 1 && av[ju] < 0.0) ? vhi : -1);
+      if (g >= 0) eV[ju] = __ldg(p.f + xy + (gu0 + ju) * s2 + g);
+    }
   }
   asm volatile("cp.async.wait_all;" ::: "memory");
   __syncthreads();
@@ -186,12 +183,15 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
         acc[jx][jy] = fma(sy, v, acc[jx][jy]);
       }
     }
+    // running sum: the x and y parts of the stage result, c0 f_n + c1 dt (.) (mode 0: the plain sums), in place of f_n
+    const double cs = p.mode == 0 ? 1.0 : p.c1 * p.dt;
 #pragma unroll
     for (int jx = 0; jx < 4; ++jx)
 #pragma unroll
       for (int jy = 0; jy < 4; ++jy) {
         const int row = (jx * 4 + jy) * 4 + ju_a;
-        accT[row * R + swz<KV>(row, col >> 1) * 2 + (col & 1)] = acc[jx][jy];
+        double* slot = accT + row * R + swz<KV>(row, col >> 1) * 2 + (col & 1);
+        *slot = use_fn ? fma(cs, acc[jx][jy], p.c0 * *slot) : cs * acc[jx][jy];
       }
   }
   __syncthreads();
@@ -205,17 +205,12 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
     const double2 a = *reinterpret_cast<const double2*>(tile + row * R + swz<KV>(row, 2 * ev) * 2);
     const double2 b = *reinterpret_cast<const double2*>(tile + row * R + swz<KV>(row, 2 * ev + 1) * 2);
     fb[ju][0] = a.x; fb[ju][1] = a.y; fb[ju][2] = b.x; fb[ju][3] = b.y;
-    const double2 c = *reinterpret_cast<const double2*>(accT + row * R + swz<KV>(row, 2 * ev) * 2);
-    const double2 d = *reinterpret_cast<const double2*>(accT + row * R + swz<KV>(row, 2 * ev + 1) * 2);
-    res[ju][0] = c.x; res[ju][1] = c.y; res[ju][2] = d.x; res[ju][3] = d.y;
   }
   {
-    const double2* h2 = reinterpret_cast<const double2*>(hUs);
-    const double2 l0 = h2[tid], l1 = h2[NT + tid], h0 = h2[2 * NT + tid], h1 = h2[3 * NT + tid];
-    const double hUlo[4] = {l0.x, l0.y, l1.x, l1.y}, hUhi[4] = {h0.x, h0.y, h1.x, h1.y};
 #pragma unroll
     for (int jv = 0; jv < 4; ++jv) {                                  // u lines (fixed jv)
-      const double uL = au[jv] > 0.0 ? hUlo[jv] : fb[0][jv], uR = au[jv] > 0.0 ? fb[3][jv] : hUhi[jv];
+      const double h = hUs[jv * NT + tid];
+      const double uL = au[jv] > 0.0 ? h : fb[0][jv], uR = au[jv] > 0.0 ? fb[3][jv] : h;
       const double su = p.J[2] * au[jv];
 #pragma unroll
       for (int ju = 0; ju < 4; ++ju) {
@@ -223,14 +218,14 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
         v = fma(-p.Xi[2 * ju + 1], uR, v);
 #pragma unroll
         for (int k = 0; k < 4; ++k) v = fma(p.U[ju * 4 + k], fb[k][jv], v);
-        res[ju][jv] = fma(su, v, res[ju][jv]);
+        res[ju][jv] = su * v;
       }
     }
   }
 #pragma unroll
   for (int ju = 0; ju < 4; ++ju) {                                    // v lines (fixed ju): neighbours from the adjacent lanes
     const double from_lo = __shfl_up_sync(0xffffffffu, fb[ju][3], 1), from_hi = __shfl_down_sync(0xffffffffu, fb[ju][0], 1);
-    const double nlo = ev > 0 ? from_lo : eVs[rowb + ju], nhi = ev < KV - 1 ? from_hi : eVs[64 + rowb + ju];
+    const double nlo = ev > 0 ? from_lo : eV[ju], nhi = ev < KV - 1 ? from_hi : eV[ju];
     const double uL = av[ju] > 0.0 ? nlo : fb[ju][0], uR = av[ju] > 0.0 ? fb[ju][3] : nhi;
     const double sv = p.J[3] * av[ju];
 #pragma unroll
@@ -247,20 +242,13 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
   const double2 w01 = *reinterpret_cast<const double2*>(p.wqv + gvb), w23 = *reinterpret_cast<const double2*>(p.wqv + gvb + 2);
 #pragma unroll
   for (int ju = 0; ju < 4; ++ju) {
-    double o[4];
-    if (p.mode == 0) {
+    // running sum of phase A (x and y parts, already scaled, + c0 f_n) + the u and v parts
+    const int row = rowb + ju;
+    const double2 sa = *reinterpret_cast<const double2*>(accT + row * R + swz<KV>(row, 2 * ev) * 2);
+    const double2 sb = *reinterpret_cast<const double2*>(accT + row * R + swz<KV>(row, 2 * ev + 1) * 2);
+    double o[4] = {sa.x, sa.y, sb.x, sb.y};
 #pragma unroll
-      for (int jv = 0; jv < 4; ++jv) o[jv] = res[ju][jv];
-    } else {
-#pragma unroll
-      for (int jv = 0; jv < 4; ++jv) o[jv] = p.c1 * fma(p.dt, res[ju][jv], fb[ju][jv]);
-      if (use_fn) {
-        const int row = rowb + ju;
-        const double2 a = *reinterpret_cast<const double2*>(fnT + row * R + swz<KV>(row, 2 * ev) * 2);
-        const double2 b = *reinterpret_cast<const double2*>(fnT + row * R + swz<KV>(row, 2 * ev + 1) * 2);
-        o[0] = fma(p.c0, a.x, o[0]); o[1] = fma(p.c0, a.y, o[1]); o[2] = fma(p.c0, b.x, o[2]); o[3] = fma(p.c0, b.y, o[3]);
-      }
-    }
+    for (int jv = 0; jv < 4; ++jv) o[jv] += p.mode == 0 ? res[ju][jv] : p.c1 * fma(p.dt, res[ju][jv], fb[ju][jv]);
     __stcs(q, make_double2(o[0], o[1]));
     __stcs(q + 1, make_double2(o[2], o[3]));
     q += s2 / 2;
