@@ -54,7 +54,7 @@ __device__ __forceinline__ int upwind_index(const Params& p, int d, int e, int n
 }
 
 template <int n>
-__global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : 1)) rhs4_elem_kernel(const Params p) {
+__global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : (n == 6 ? 4 : 8))) rhs4_elem_kernel(const Params p) {
   constexpr int H = n / 2, n2 = n * n;
   extern __shared__ double2 esm_raw[];
   double* T = reinterpret_cast<double*>(esm_raw);                 // [jx][jy][ju][jv] values of f
