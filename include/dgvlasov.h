@@ -117,6 +117,14 @@ int dg_ssprk3_step(dg_ctx* ctx, double* f_dev, double dt, int32_t self_consisten
 int dg_ssprk3_run(dg_ctx* ctx, double* f_dev, double dt, int32_t nsteps, int32_t self_consistent, void* stream);
 /* Same with a HOST array: copies f in, runs nsteps, copies f back, synchronises. */
 int dg_ssprk3_run_host(dg_ctx* ctx, double* f_host, double dt, int32_t nsteps, int32_t self_consistent);
+/* The Shu-Osher coefficients of stage `stage` = 0, 1, 2 (its ref. [38]): out = c0 u^n + c1 (u^(s) + dt L(u^(s))),
+ * (c0, c1) = (0, 1), (3/4, 1/4), (1/3, 2/3).  For callers that drive dg_rk_stage themselves (the x-slab stepper): the table
+ * lives in the library, not in the binding. */
+int dg_ssprk3_stage_coeffs(int32_t stage, double* c0_host, double* c1_host);
+/* Non-finite guard (the CFL blow-up case: PAPER.md:477 defers the order-dependent limits to its ref. [39]; see
+ * dg_max_stable_dt): *flag_dev = 0 if every value of f is finite, 1 if any is Inf or NaN.  One pass over f, asynchronous
+ * on `stream`; flag_dev is a device int32 owned by the caller.  x-only contexts check N_x*n_x values. */
+int dg_check_finite(dg_ctx* ctx, const double* f_dev, int32_t* flag_dev, void* stream);
 
 /* Zeroth moment Eq. 27 by LGL quadrature: rho[g_x] = sum_{g_u,g_v}
  * (w_{b_u}/J_u)(w_{b_v}/J_v) f.  rho_dev: [N_x*n_x].  Deterministic (no atomics). */
@@ -160,19 +168,30 @@ double dg_max_stable_dt(const dg_ctx* ctx, double E_bound);
                                   4 FFT-factorised kernel (equal-width elements: N_x a power of two, even order; n FFTs of
                                   length N_x per vector in shared memory + a (pmax+1) x n mode table instead of the dense
                                   T and S; DG_ERR_UNSUPPORTED otherwise).  auto takes 4 for batched calls when supported. */
-#define DG_OPT_PROFILE      3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
+#define DG_OPT_PROFILE      3   /* k = 1: bracket every RHS-kernel launch with CUDA events on its stream (kernels run without
+                                  programmatic launches: the kernel alone); k >= 2: bracket every k-th RHS launch only, inside a
+                                  normally running sequence (k coprime to 3 visits every RK stage); 0: off */
 #define DG_OPT_PDL          4   /* 1 (default): consecutive kernels of dg_ssprk3_* are chained by programmatic dependent
                                   launch (the next kernel's prologue overlaps the previous kernel's tail); 0: plain launches */
 #define DG_OPT_FORM         5   /* 0 (default): weak form, Eq. 14: Upsilon F - Xi F*;  1: strong form, Eq. 15
                                   (PAPER.md:102): -D F + Xi (F - F*), D = Eq. 55.  Same scheme (Upsilon + D = Xi_R e_R^T -
                                   Xi_L e_L^T), different rounding; both RHS kernels, every entry point. */
+#define DG_OPT_SMEM_PAD_KB  6   /* unused extra shared memory (KB) per CTA of the tiled RHS kernel: lowers the number of resident
+                                  CTAs per SM.  For occupancy sweeps (profiles/): 0 (default) in production */
 int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value);
 /* Profile mode: total device time (ms) and count of the RHS-kernel launches since the last reset.
  * Synchronises on the recorded events. */
 int dg_get_profile(dg_ctx* ctx, double* rhs_ms_total_host, int64_t* rhs_launches_host, int32_t reset);
+/* The same per RK stage: index 0 = launches outside dg_ssprk3_* (dg_rhs, dg_rk_stage), 1..3 = stages 1..3.
+ *   ms_host [out] [4]   launches_host [out] [4] */
+int dg_get_profile_stages(dg_ctx* ctx, double* ms_host, int64_t* launches_host, int32_t reset);
 int64_t dg_launch_count(const dg_ctx* ctx);      /* kernels launched through this context so far */
 const char* dg_last_kernel(const dg_ctx* ctx);   /* name of the RHS kernel variant last used */
 const char* dg_last_field_kernel(const dg_ctx* ctx);   /* name of the projection / field-solve kernel last used */
+/* Measured FP64 arithmetic peak of `device` in TFLOP/s (2 flop per fused multiply-add): variant 0 = DFMA (vector pipe),
+ * 1 = DMMA (mma.sync.m8n8k4.f64, the FP64 tensor path).  Register-resident chains, `iters` iterations (>= 1000 for a stable
+ * figure), synchronises.  The roofline denominator of the dense DG->Fourier contraction (Eq. 63). */
+int dg_fp64_peak(int32_t device, int32_t variant, int32_t iters, double* tflops_host);
 const char* dg_last_error(void);
 const char* dg_version(void);
 

@@ -75,7 +75,7 @@ double dg4_max_stable_dt(const dg4_ctx* ctx, double E_bound);
 #define DG4_OPT_RHS_KERNEL 1   /* 0 auto (tiled when all orders are 4 and N_v is even; element kernel for equal orders 6 or 8;
                                   else generic), 1 generic, 2 tiled, 3 element kernel (equal orders 4, 6, 8); 2 and 3 fail with
                                   DG_ERR_UNSUPPORTED on other shapes */
-#define DG4_OPT_PROFILE    3   /* 1: bracket every RHS-kernel launch with CUDA events on its stream */
+#define DG4_OPT_PROFILE    3   /* k >= 1: bracket every k-th RHS-kernel launch with CUDA events on its stream (0 off) */
 int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value);
 int dg4_get_profile(dg4_ctx* ctx, double* rhs_ms_total_host, int64_t* rhs_launches_host, int32_t reset);
 int64_t dg4_launch_count(const dg4_ctx* ctx);

@@ -70,6 +70,10 @@ SIGNATURES = {
     "dg_max_stable_dt": (_dbl, [_vp, _dbl]),
     "dg_set_option": (C.c_int, [_vp, _i32, _i64]),
     "dg_get_profile": (C.c_int, [_vp, _dp, C.POINTER(_i64), _i32]),
+    "dg_get_profile_stages": (C.c_int, [_vp, _dp, C.POINTER(_i64), _i32]),
+    "dg_ssprk3_stage_coeffs": (C.c_int, [_i32, _dp, _dp]),
+    "dg_check_finite": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "dg_fp64_peak": (C.c_int, [_i32, _i32, _i32, _dp]),
     "dg_launch_count": (_i64, [_vp]),
     "dg_last_kernel": (C.c_char_p, [_vp]),
     "dg_last_field_kernel": (C.c_char_p, [_vp]),

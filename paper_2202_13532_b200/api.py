@@ -18,6 +18,7 @@ OPT_FIELD_KERNEL = 2
 OPT_PROFILE = 3
 OPT_PDL = 4
 OPT_FORM = 5
+OPT_SMEM_PAD_KB = 6
 FORM_WEAK, FORM_STRONG = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 FIELD_AUTO, FIELD_SIMPLE, FIELD_DMMA, FIELD_DFMA, FIELD_FFT = 0, 1, 2, 3, 4
@@ -47,6 +48,20 @@ def _stream(device):
 
 def version() -> str:
     return _L.dg_version().decode()
+
+
+def ssprk3_stage_coeffs(stage: int):
+    """dg_ssprk3_stage_coeffs: (c0, c1) of Shu-Osher stage 0, 1, 2 -- the table lives in the library."""
+    c0, c1 = C.c_double(0.0), C.c_double(0.0)
+    _check(_L.dg_ssprk3_stage_coeffs(int(stage), C.byref(c0), C.byref(c1)), "dg_ssprk3_stage_coeffs")
+    return c0.value, c1.value
+
+
+def fp64_peak(device=0, variant=0, iters=20000) -> float:
+    """dg_fp64_peak: measured FP64 TFLOP/s of the device (variant 0 DFMA, 1 DMMA)."""
+    tf = C.c_double(0.0)
+    _check(_L.dg_fp64_peak(int(device), int(variant), int(iters), C.byref(tf)), "dg_fp64_peak")
+    return tf.value
 
 
 class DGContext:
@@ -220,6 +235,18 @@ class DGContext:
         ms, cnt = C.c_double(0.0), C.c_int64(0)
         _check(_L.dg_get_profile(self._h, C.byref(ms), C.byref(cnt), int(bool(reset))), "dg_get_profile")
         return ms.value, cnt.value
+
+    def get_profile_stages(self, reset=True):
+        """([ms] * 4, [launches] * 4): index 0 = RHS launches outside dg_ssprk3_*, 1..3 = RK stages 1..3."""
+        ms, cnt = (C.c_double * 4)(), (C.c_int64 * 4)()
+        _check(_L.dg_get_profile_stages(self._h, ms, cnt, int(bool(reset))), "dg_get_profile_stages")
+        return list(ms), list(cnt)
+
+    def check_finite(self, f, flag=None):
+        """dg_check_finite: int32 device flag, 0 = every value of f finite, 1 = some Inf/NaN (asynchronous)."""
+        flag = torch.empty(1, dtype=torch.int32, device=self.device) if flag is None else flag
+        _check(_L.dg_check_finite(self._h, _ptr(f), flag.data_ptr(), _stream(self.device)), "dg_check_finite")
+        return flag
 
     @property
     def launch_count(self):

@@ -25,8 +25,8 @@ struct dg4_ctx {
   size_t partials_doubles = 0;
   double* f_stage = nullptr;
   int64_t launches = 0;
-  int opt_kernel = 0, opt_profile = 0;
-  bool smem_attr_done = false, elem_attr_done = false;
+  int opt_kernel = 0, opt_profile = 0;   // opt_profile = k: every k-th RHS launch is bracketed by events
+  int64_t prof_seen = 0;
   std::vector<cudaEvent_t> prof_events;
   double prof_ms = 0.0;
   int64_t prof_launches = 0;
@@ -66,7 +66,7 @@ extern "C" int dg4_create(const dg4_grid_desc* desc, dg4_ctx** out) {
   }
   if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dg4_create: mass_mode must be 0 or 1");
   if (desc->pmax[0] < 0 || desc->pmax[1] < 0) return fail(DG_ERR_INVALID_ARG, "dg4_create: pmax must be >= 0");
-  CUDA_TRY(cudaSetDevice(desc->device));
+  DeviceGuard guard(desc->device);      // the caller's current device is restored on return
   dg4_ctx* ctx = new (std::nothrow) dg4_ctx();
   if (!ctx) return fail(DG_ERR_CUDA, "dg4_create: out of host memory");
   ctx->desc = *desc;
@@ -154,6 +154,7 @@ extern "C" int dg4_create(const dg4_grid_desc* desc, dg4_ctx** out) {
 
 extern "C" int dg4_destroy(dg4_ctx* ctx) {
   if (!ctx) return DG_OK;
+  DeviceGuard guard(ctx->desc.device);
   if (ctx->dev_block) cudaFree(ctx->dev_block);
   if (ctx->f_stage) cudaFree(ctx->f_stage);
   for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
@@ -184,6 +185,7 @@ extern "C" size_t dg4_workspace_bytes(const dg4_ctx* ctx) {
 
 extern "C" int dg4_set_workspace(dg4_ctx* ctx, void* ws_dev, size_t bytes) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_set_workspace: null context");
+  DeviceGuard guard(ctx->desc.device);
   if (!ws_dev || ((uintptr_t)ws_dev & 255) != 0) return fail(DG_ERR_INVALID_ARG, "dg4_set_workspace: pointer must be non-null and 256-byte aligned");
   if (bytes < dg4_workspace_bytes(ctx)) return fail(DG_ERR_WORKSPACE, "dg4_set_workspace: too small, see dg4_workspace_bytes");
   const size_t gxy = (size_t)ctx->G[0] * ctx->G[1], nq = 2 * (size_t)ctx->Q + 1;
@@ -243,11 +245,7 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
     const bool with_fn = mode != 0 && fn != nullptr;
     const size_t smem = sizeof(double) * (kv == 8 ? dg4::tile_smem_doubles<8>(with_fn) : kv == 4 ? dg4::tile_smem_doubles<4>(with_fn)
                                                                                               : dg4::tile_smem_doubles<2>(with_fn));
-    if (kv == 8 && !ctx->smem_attr_done) {
-      CUDA_TRY(cudaFuncSetAttribute(dg4::rhs4_tile_kernel<8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)(sizeof(double) * dg4::tile_smem_doubles<8>(true))));
-      ctx->smem_attr_done = true;
-    }
+    if (kv == 8) CUDA_TRY(ensure_dyn_smem(reinterpret_cast<const void*>(dg4::rhs4_tile_kernel<8, 5>), sizeof(double) * dg4::tile_smem_doubles<8>(true)));
     if (kv == 8) dg4::rhs4_tile_kernel<8, 5><<<tiles, 128, smem, st>>>(p);
     else if (kv == 4) dg4::rhs4_tile_kernel<4, 1><<<tiles, 64, smem, st>>>(p);
     else dg4::rhs4_tile_kernel<2, 1><<<tiles, 32, smem, st>>>(p);
@@ -269,10 +267,7 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
     const dim3 grid(ctx->N[3] * ctx->N[2], ctx->N[1], ctx->N[0]);
     if (ne == 8) {
       const size_t smem = sizeof(double) * dg4::elem_smem_doubles<8>();
-      if (!ctx->elem_attr_done) {
-        CUDA_TRY(cudaFuncSetAttribute(dg4::rhs4_elem_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ctx->elem_attr_done = true;
-      }
+      CUDA_TRY(ensure_dyn_smem(reinterpret_cast<const void*>(dg4::rhs4_elem_kernel<8>), smem));
       dg4::rhs4_elem_kernel<8><<<grid, 512, smem, st>>>(p);
     } else if (ne == 6) dg4::rhs4_elem_kernel<6><<<grid, 216, sizeof(double) * dg4::elem_smem_doubles<6>(), st>>>(p);
     else dg4::rhs4_elem_kernel<4><<<grid, 64, sizeof(double) * dg4::elem_smem_doubles<4>(), st>>>(p);
@@ -288,7 +283,7 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
 
 static int launch_rhs4(dg4_ctx* ctx, const double* f, const double* fn, const double* Ex, const double* Ey, double* out,
                        int mode, double c0, double c1, double dt, bool want_partials, int* chunks_out, cudaStream_t st) {
-  if (!ctx->opt_profile) return launch_rhs4_inner(ctx, f, fn, Ex, Ey, out, mode, c0, c1, dt, want_partials, chunks_out, st);
+  if (!(ctx->opt_profile > 0 && (ctx->prof_seen++ % ctx->opt_profile) == 0)) return launch_rhs4_inner(ctx, f, fn, Ex, Ey, out, mode, c0, c1, dt, want_partials, chunks_out, st);
   cudaEvent_t e0, e1;
   CUDA_TRY(cudaEventCreate(&e0));
   CUDA_TRY(cudaEventCreate(&e1));
@@ -368,12 +363,14 @@ static int launch_field4(dg4_ctx* ctx, const double* rho, double* Ex, double* Ey
 // ------------------------------------------------------------------------------------------------
 extern "C" int dg4_rhs(dg4_ctx* ctx, const double* f_dev, const double* Ex_dev, const double* Ey_dev, double* dfdt_dev, void* stream) {
   if (!ctx || !f_dev || !dfdt_dev) return fail(DG_ERR_INVALID_ARG, "dg4_rhs: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (f_dev == dfdt_dev) return fail(DG_ERR_INVALID_ARG, "dg4_rhs: dfdt must not alias f");
   return launch_rhs4(ctx, f_dev, nullptr, Ex_dev, Ey_dev, dfdt_dev, 0, 0.0, 1.0, 0.0, false, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" int dg4_density(dg4_ctx* ctx, const double* f_dev, double* rho_dev, void* stream) {
   if (!ctx || !f_dev || !rho_dev) return fail(DG_ERR_INVALID_ARG, "dg4_density: null argument");
+  DeviceGuard guard(ctx->desc.device);
   int nchunks = 0;
   int rc = launch_density4_partials(ctx, f_dev, &nchunks, (cudaStream_t)stream);
   if (rc) return rc;
@@ -383,6 +380,7 @@ extern "C" int dg4_density(dg4_ctx* ctx, const double* f_dev, double* rho_dev, v
 extern "C" int dg4_rk_stage(dg4_ctx* ctx, const double* f_s_dev, const double* f_n_dev, const double* Ex_dev, const double* Ey_dev,
                             double* out_dev, double c0, double c1, double dt, double* rho_out_dev, void* stream) {
   if (!ctx || !f_s_dev || !out_dev) return fail(DG_ERR_INVALID_ARG, "dg4_rk_stage: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (f_s_dev == out_dev) return fail(DG_ERR_INVALID_ARG, "dg4_rk_stage: out must not alias f_s");
   if (c0 != 0.0 && !f_n_dev) return fail(DG_ERR_INVALID_ARG, "dg4_rk_stage: c0 != 0 needs f_n");
   cudaStream_t st = (cudaStream_t)stream;
@@ -395,12 +393,14 @@ extern "C" int dg4_rk_stage(dg4_ctx* ctx, const double* f_s_dev, const double* f
 
 extern "C" int dg4_fourier_project(dg4_ctx* ctx, const double* rho_dev, double* c_dev, void* stream) {
   if (!ctx || !rho_dev || !c_dev) return fail(DG_ERR_INVALID_ARG, "dg4_fourier_project: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg4_fourier_project: set a workspace first");
   return launch_project4(ctx, rho_dev, c_dev, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" int dg4_poisson_E(dg4_ctx* ctx, const double* rho_dev, double* Ex_dev, double* Ey_dev, void* stream) {
   if (!ctx || !rho_dev || !Ex_dev || !Ey_dev) return fail(DG_ERR_INVALID_ARG, "dg4_poisson_E: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg4_poisson_E: set a workspace first");
   return launch_field4(ctx, rho_dev, Ex_dev, Ey_dev, (cudaStream_t)stream);
 }
@@ -415,6 +415,7 @@ static int field4_from_partials_or_f(dg4_ctx* ctx, const double* f, int chunks, 
 
 extern "C" int dg4_ssprk3_run(dg4_ctx* ctx, double* f_dev, double dt, int32_t nsteps, int32_t self_consistent, void* stream) {
   if (!ctx || !f_dev) return fail(DG_ERR_INVALID_ARG, "dg4_ssprk3_run: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (nsteps < 0 || !(dt == dt)) return fail(DG_ERR_INVALID_ARG, "dg4_ssprk3_run: bad nsteps or dt");
   if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg4_ssprk3_run: set a workspace first");
   if (self_consistent && (ctx->desc.bc[0] != 0 || ctx->desc.bc[1] != 0))
@@ -439,6 +440,7 @@ extern "C" int dg4_ssprk3_run(dg4_ctx* ctx, double* f_dev, double dt, int32_t ns
 
 extern "C" int dg4_ssprk3_run_host(dg4_ctx* ctx, double* f_host, double dt, int32_t nsteps, int32_t self_consistent) {
   if (!ctx || !f_host) return fail(DG_ERR_INVALID_ARG, "dg4_ssprk3_run_host: null argument");
+  DeviceGuard guard(ctx->desc.device);
   const size_t bytes = ctx->dof * sizeof(double);
   if (!ctx->f_stage) CUDA_TRY(cudaMalloc(&ctx->f_stage, bytes));
   CUDA_TRY(cudaMemcpyAsync(ctx->f_stage, f_host, bytes, cudaMemcpyHostToDevice, 0));
@@ -472,12 +474,13 @@ extern "C" double dg4_max_stable_dt(const dg4_ctx* ctx, double E_bound) {
 extern "C" int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_set_option: null context");
   if (key == DG4_OPT_RHS_KERNEL && value >= 0 && value <= 3) { ctx->opt_kernel = (int)value; return DG_OK; }
-  if (key == DG4_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
+  if (key == DG4_OPT_PROFILE && value >= 0 && value <= 1000000) { ctx->opt_profile = (int)value; ctx->prof_seen = 0; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg4_set_option: unknown key or value");
 }
 
 extern "C" int dg4_get_profile(dg4_ctx* ctx, double* ms_total, int64_t* launches, int32_t reset) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_get_profile: null context");
+  DeviceGuard guard(ctx->desc.device);
   for (size_t i = 0; i + 1 < ctx->prof_events.size(); i += 2) {
     CUDA_TRY(cudaEventSynchronize(ctx->prof_events[i + 1]));
     float ms = 0.f;

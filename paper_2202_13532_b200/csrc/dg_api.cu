@@ -13,6 +13,7 @@
 #include "dg_kernels_tiled.cuh"
 #include "dg_kernels_field.cuh"
 #include "dg_kernels_fft.cuh"
+#include "dg_microbench.cuh"
 
 static thread_local std::string g_err;
 
@@ -70,7 +71,12 @@ static int create_impl(const dg_grid_desc* desc, const double* edges, dg_ctx** o
   }
   if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dg_create: mass_mode must be 0 or 1");
   if (desc->pmax < 0) return fail(DG_ERR_INVALID_ARG, "dg_create: pmax must be >= 0");
-  CUDA_TRY(cudaSetDevice(desc->device));
+  {
+    int ndev = 0;
+    CUDA_TRY(cudaGetDeviceCount(&ndev));
+    if (desc->device < 0 || desc->device >= ndev) return fail(DG_ERR_INVALID_ARG, "dg_create: no such device");
+  }
+  DeviceGuard guard(desc->device);      // the caller's current device is restored on return
 
   dg_ctx* ctx = new (std::nothrow) dg_ctx();
   if (!ctx) return fail(DG_ERR_CUDA, "dg_create: out of host memory");
@@ -212,10 +218,12 @@ static int create_impl(const dg_grid_desc* desc, const double* edges, dg_ctx** o
 
 extern "C" int dg_destroy(dg_ctx* ctx) {
   if (!ctx) return DG_OK;
+  DeviceGuard guard(ctx->desc.device);
   if (ctx->dev_block) cudaFree(ctx->dev_block);
+  if (ctx->d_flag) cudaFree(ctx->d_flag);
   if (ctx->dense_block) cudaFree(ctx->dense_block);
   if (ctx->f_stage) cudaFree(ctx->f_stage);
-  for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
+  for (const ProfRecord& r : ctx->prof_events) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete ctx;
   return DG_OK;
 }
@@ -295,18 +303,21 @@ static int launch_rhs_generic(dg_ctx* ctx, const double* f, const double* fn, co
 static int launch_rhs_inner(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                             double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st);
 
-// In profile mode (DG_OPT_PROFILE) every RHS launch is bracketed by events on its own stream.
+// In profile mode (DG_OPT_PROFILE) RHS launches are bracketed by events on their own stream.
 static int launch_rhs(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                       double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
-  if (!ctx->opt_profile) return launch_rhs_inner(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-  cudaEvent_t e0, e1;
-  CUDA_TRY(cudaEventCreate(&e0));
-  CUDA_TRY(cudaEventCreate(&e1));
-  CUDA_TRY(cudaEventRecord(e0, st));
+  // DG_OPT_PROFILE = k: every k-th RHS launch is bracketed (k = 1: all of them, and the kernels run without programmatic
+  // launches; k >= 2: a sample taken inside a normally running step sequence -- k coprime to 3 visits every stage)
+  const bool bracket = ctx->opt_profile > 0 && (ctx->prof_seen++ % ctx->opt_profile) == 0;
+  if (!bracket) return launch_rhs_inner(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+  ProfRecord r;
+  r.stage = ctx->cur_stage;
+  CUDA_TRY(cudaEventCreate(&r.e0));
+  CUDA_TRY(cudaEventCreate(&r.e1));
+  CUDA_TRY(cudaEventRecord(r.e0, st));
   int rc = launch_rhs_inner(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-  CUDA_TRY(cudaEventRecord(e1, st));
-  ctx->prof_events.push_back(e0);
-  ctx->prof_events.push_back(e1);
+  CUDA_TRY(cudaEventRecord(r.e1, st));
+  ctx->prof_events.push_back(r);
   return rc;
 }
 
@@ -462,6 +473,7 @@ static int launch_synth(dg_ctx* ctx, const double* c, int batch, double* E, cuda
 // ------------------------------------------------------------------------------------------------
 extern "C" int dg_rhs(dg_ctx* ctx, const double* f_dev, const double* E_dev, double* dfdt_dev, void* stream) {
   if (!ctx || !f_dev || !dfdt_dev) return fail(DG_ERR_INVALID_ARG, "dg_rhs: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_rhs: field-only context (ndim = 1)");
   if (f_dev == dfdt_dev) return fail(DG_ERR_INVALID_ARG, "dg_rhs: dfdt must not alias f");
   return launch_rhs(ctx, f_dev, nullptr, E_dev, dfdt_dev, 0, 0.0, 1.0, 0.0, false, nullptr, (cudaStream_t)stream);
@@ -487,6 +499,7 @@ extern "C" int dg_set_xhalo_push(dg_ctx* ctx, double* left_dst_dev, double* righ
 extern "C" int dg_rk_stage(dg_ctx* ctx, const double* f_s_dev, const double* f_n_dev, const double* E_dev, double* out_dev,
                            double c0, double c1, double dt, double* rho_out_dev, void* stream) {
   if (!ctx || !f_s_dev || !out_dev) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_rk_stage: field-only context (ndim = 1)");
   if (f_s_dev == out_dev) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: out must not alias f_s");
   if (!f_n_dev && c0 != 0.0) return fail(DG_ERR_INVALID_ARG, "dg_rk_stage: f_n is needed when c0 != 0");
@@ -501,19 +514,35 @@ extern "C" int dg_rk_stage(dg_ctx* ctx, const double* f_s_dev, const double* f_n
 
 extern "C" int dg_density(dg_ctx* ctx, const double* f_dev, double* rho_dev, void* stream) {
   if (!ctx || !f_dev || !rho_dev) return fail(DG_ERR_INVALID_ARG, "dg_density: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_density: field-only context (ndim = 1)");
   if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_density: set a workspace first (partials live there)");
   return launch_density(ctx, f_dev, rho_dev, ctx->partials, ctx->partials_doubles, (cudaStream_t)stream);
 }
 
+extern "C" int dg_check_finite(dg_ctx* ctx, const double* f_dev, int32_t* flag_dev, void* stream) {
+  if (!ctx || !f_dev || !flag_dev) return fail(DG_ERR_INVALID_ARG, "dg_check_finite: null argument");
+  DeviceGuard guard(ctx->desc.device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long n = ctx->dof ? (long long)ctx->dof : (long long)ctx->G[0];
+  CUDA_TRY(cudaMemsetAsync(flag_dev, 0, sizeof(int32_t), st));
+  long long blocks = (n / 2 + 255) / 256;
+  if (blocks < 1) blocks = 1;
+  if (blocks > 148LL * 16) blocks = 148LL * 16;
+  dgk::check_finite_kernel<<<(unsigned)blocks, 256, 0, st>>>(f_dev, n, flag_dev);
+  return check_launch(ctx, "check_finite_kernel");
+}
+
 extern "C" int dg_fourier_project(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* c_dev, void* stream) {
   if (!ctx || !rho_dev || !c_dev) return fail(DG_ERR_INVALID_ARG, "dg_fourier_project: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_fourier_project: batch must be >= 1");
   return launch_project(ctx, rho_dev, batch, c_dev, (cudaStream_t)stream);
 }
 
 static int poisson_solve(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* out_dev, int phi, void* stream) {
   if (!ctx || !rho_dev || !out_dev) return fail(DG_ERR_INVALID_ARG, "dg_poisson: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_poisson: batch must be >= 1");
   if (ctx->desc.bc[0] != 0) return fail(DG_ERR_INVALID_ARG, "dg_poisson: x must be periodic");
   cudaStream_t st = (cudaStream_t)stream;
@@ -535,6 +564,7 @@ static int poisson_solve(dg_ctx* ctx, const double* rho_dev, int32_t batch, doub
 
 extern "C" int dg_broken_l2(dg_ctx* ctx, const double* u_dev, const double* v_dev, int32_t batch, double* eps_dev, void* stream) {
   if (!ctx || !u_dev || !eps_dev) return fail(DG_ERR_INVALID_ARG, "dg_broken_l2: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_broken_l2: batch must be >= 1");
   const int n0 = ctx->n[0];
   const double alpha = n0 * (n0 - 1) / (2.0 * (2 * n0 - 1));
@@ -556,7 +586,7 @@ static int field_from_partials_or_f(dg_ctx* ctx, const double* f, int partial_ch
   int rc;
   if (ctx->fused_grid > 0 && ctx->opt_field_kernel != 1) {
     // one launch: finish the density, project, synthesise (field_fused_kernel)
-    bool pdl = ctx->opt_pdl != 0 && !ctx->opt_profile;
+    bool pdl = ctx->opt_pdl != 0 && ctx->opt_profile != 1;
     if (partial_chunks <= 0) {
       rc = launch_density_partials(ctx, f, ctx->partials, ctx->partials_doubles, &partial_chunks, st);
       if (rc) return rc;
@@ -579,8 +609,17 @@ static int field_from_partials_or_f(dg_ctx* ctx, const double* f, int partial_ch
   return launch_synth(ctx, ctx->cbuf, 1, ctx->E, st);
 }
 
+// Shu-Osher SSP-RK3 (reading C3): stage s combines out = c0 u^n + c1 (u^(s) + dt L(u^(s))).
+extern "C" int dg_ssprk3_stage_coeffs(int32_t stage, double* c0, double* c1) {
+  static const double tab[3][2] = {{0.0, 1.0}, {0.75, 0.25}, {1.0 / 3.0, 2.0 / 3.0}};
+  if (stage < 0 || stage > 2 || !c0 || !c1) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3_stage_coeffs: stage must be 0, 1 or 2");
+  *c0 = tab[stage][0]; *c1 = tab[stage][1];
+  return DG_OK;
+}
+
 extern "C" int dg_ssprk3_run(dg_ctx* ctx, double* f_dev, double dt, int32_t nsteps, int32_t self_consistent, void* stream) {
   if (!ctx || !f_dev) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_ssprk3: field-only context (ndim = 1)");
   if (nsteps < 0 || !(dt == dt)) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: bad nsteps or dt");
   if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_ssprk3: set a workspace first");
@@ -592,15 +631,23 @@ extern "C" int dg_ssprk3_run(dg_ctx* ctx, double* f_dev, double dt, int32_t nste
     int rc;
     // stage 1: u1 = u + dt L(u)
     if (self_consistent) { rc = field_from_partials_or_f(ctx, f_dev, chunks, st); if (rc) return rc; E = ctx->E; }
-    rc = launch_rhs(ctx, f_dev, nullptr, E, ctx->u1, 1, 0.0, 1.0, dt, self_consistent != 0, &chunks, st);
-    if (rc) return rc;
+    double c0, c1;
+    dg_ssprk3_stage_coeffs(0, &c0, &c1);
+    ctx->cur_stage = 1;
+    rc = launch_rhs(ctx, f_dev, nullptr, E, ctx->u1, 1, c0, c1, dt, self_consistent != 0, &chunks, st);
+    if (rc) { ctx->cur_stage = 0; return rc; }
     // stage 2: u2 = 3/4 u + 1/4 (u1 + dt L(u1))
     if (self_consistent) { rc = field_from_partials_or_f(ctx, ctx->u1, chunks, st); if (rc) return rc; }
-    rc = launch_rhs(ctx, ctx->u1, f_dev, E, ctx->u2, 1, 0.75, 0.25, dt, self_consistent != 0, &chunks, st);
-    if (rc) return rc;
+    dg_ssprk3_stage_coeffs(1, &c0, &c1);
+    ctx->cur_stage = 2;
+    rc = launch_rhs(ctx, ctx->u1, f_dev, E, ctx->u2, 1, c0, c1, dt, self_consistent != 0, &chunks, st);
+    if (rc) { ctx->cur_stage = 0; return rc; }
     // stage 3: u = 1/3 u + 2/3 (u2 + dt L(u2)), in place (each node of u is read and written by one thread)
     if (self_consistent) { rc = field_from_partials_or_f(ctx, ctx->u2, chunks, st); if (rc) return rc; }
-    rc = launch_rhs(ctx, ctx->u2, f_dev, E, f_dev, 1, 1.0 / 3.0, 2.0 / 3.0, dt, self_consistent != 0, &chunks, st);
+    dg_ssprk3_stage_coeffs(2, &c0, &c1);
+    ctx->cur_stage = 3;
+    rc = launch_rhs(ctx, ctx->u2, f_dev, E, f_dev, 1, c0, c1, dt, self_consistent != 0, &chunks, st);
+    ctx->cur_stage = 0;
     if (rc) return rc;
   }
   return DG_OK;
@@ -612,6 +659,7 @@ extern "C" int dg_ssprk3_step(dg_ctx* ctx, double* f_dev, double dt, int32_t sel
 
 extern "C" int dg_ssprk3_run_host(dg_ctx* ctx, double* f_host, double dt, int32_t nsteps, int32_t self_consistent) {
   if (!ctx || !f_host) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3_run_host: null argument");
+  DeviceGuard guard(ctx->desc.device);
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_ssprk3_run_host: field-only context (ndim = 1)");
   const size_t bytes = ctx->dof * sizeof(double);
   if (!ctx->f_stage) CUDA_TRY(cudaMalloc(&ctx->f_stage, bytes));
@@ -652,6 +700,7 @@ extern "C" int dg_get_nodes(const dg_ctx* ctx, int32_t dim, double* coords) {
 extern "C" int dg_get_transform(const dg_ctx* ctx, int32_t p_first, int32_t p_count, double* T_host) {
   if (!ctx || !T_host || p_first < 0 || p_count < 0 || p_first + p_count > ctx->P1)
     return fail(DG_ERR_INVALID_ARG, "dg_get_transform: bad argument");
+  DeviceGuard guard(ctx->desc.device);
   const int G = ctx->G[0];
   if (int rc = ensure_dense(const_cast<dg_ctx*>(ctx))) return rc;
   std::vector<double> rows((size_t)2 * p_count * G);
@@ -681,32 +730,72 @@ extern "C" double dg_max_stable_dt(const dg_ctx* ctx, double E_bound) {
   return sum > 0.0 ? 1.0 / sum : INFINITY;
 }
 
-extern "C" int dg_get_profile(dg_ctx* ctx, double* rhs_ms_total, int64_t* rhs_launches, int32_t reset) {
-  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_get_profile: null context");
-  for (size_t i = 0; i + 1 < ctx->prof_events.size(); i += 2) {
-    CUDA_TRY(cudaEventSynchronize(ctx->prof_events[i + 1]));
+static int drain_profile(dg_ctx* ctx) {
+  for (const ProfRecord& r : ctx->prof_events) {
+    CUDA_TRY(cudaEventSynchronize(r.e1));
     float ms = 0.f;
-    CUDA_TRY(cudaEventElapsedTime(&ms, ctx->prof_events[i], ctx->prof_events[i + 1]));
-    ctx->prof_rhs_ms += ms;
-    ctx->prof_rhs_launches += 1;
-    cudaEventDestroy(ctx->prof_events[i]);
-    cudaEventDestroy(ctx->prof_events[i + 1]);
+    CUDA_TRY(cudaEventElapsedTime(&ms, r.e0, r.e1));
+    const int s = (r.stage >= 0 && r.stage <= 3) ? r.stage : 0;
+    ctx->prof_ms[s] += ms;
+    ctx->prof_n[s] += 1;
+    cudaEventDestroy(r.e0);
+    cudaEventDestroy(r.e1);
   }
   ctx->prof_events.clear();
-  if (rhs_ms_total) *rhs_ms_total = ctx->prof_rhs_ms;
-  if (rhs_launches) *rhs_launches = ctx->prof_rhs_launches;
-  if (reset) { ctx->prof_rhs_ms = 0.0; ctx->prof_rhs_launches = 0; }
+  return DG_OK;
+}
+
+extern "C" int dg_get_profile(dg_ctx* ctx, double* rhs_ms_total, int64_t* rhs_launches, int32_t reset) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_get_profile: null context");
+  DeviceGuard guard(ctx->desc.device);
+  if (int rc = drain_profile(ctx)) return rc;
+  double ms = 0.0; int64_t n = 0;
+  for (int s = 0; s < 4; ++s) { ms += ctx->prof_ms[s]; n += ctx->prof_n[s]; }
+  if (rhs_ms_total) *rhs_ms_total = ms;
+  if (rhs_launches) *rhs_launches = n;
+  if (reset) for (int s = 0; s < 4; ++s) { ctx->prof_ms[s] = 0.0; ctx->prof_n[s] = 0; }
+  return DG_OK;
+}
+
+extern "C" int dg_get_profile_stages(dg_ctx* ctx, double* ms_host, int64_t* launches_host, int32_t reset) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_get_profile_stages: null context");
+  DeviceGuard guard(ctx->desc.device);
+  if (int rc = drain_profile(ctx)) return rc;
+  for (int s = 0; s < 4; ++s) {
+    if (ms_host) ms_host[s] = ctx->prof_ms[s];
+    if (launches_host) launches_host[s] = ctx->prof_n[s];
+  }
+  if (reset) for (int s = 0; s < 4; ++s) { ctx->prof_ms[s] = 0.0; ctx->prof_n[s] = 0; }
   return DG_OK;
 }
 
 extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_option: null context");
-  if (key == DG_OPT_PROFILE && (value == 0 || value == 1)) { ctx->opt_profile = (int)value; return DG_OK; }
+  if (key == DG_OPT_PROFILE && value >= 0 && value <= 1000000) { ctx->opt_profile = (int)value; ctx->prof_seen = 0; return DG_OK; }
+  if (key == DG_OPT_SMEM_PAD_KB && value >= 0 && value <= 180) { ctx->opt_smem_pad_kb = (int)value; return DG_OK; }
   if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 4) { ctx->opt_field_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_PDL && (value == 0 || value == 1)) { ctx->opt_pdl = (int)value; return DG_OK; }
   if (key == DG_OPT_FORM && (value == 0 || value == 1)) { ctx->opt_form = (int)value; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg_set_option: unknown key or value");
+}
+
+extern "C" int dg_fp64_peak(int32_t device, int32_t variant, int32_t iters, double* tflops_host) {
+  if (!tflops_host || iters < 1 || (variant != 0 && variant != 1)) return fail(DG_ERR_INVALID_ARG, "dg_fp64_peak: bad argument");
+  DeviceGuard guard(device);
+  int sms = 0;
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+  const int blocks = sms * 8;                      // 2048 threads per SM
+  double* scratch = nullptr;
+  CUDA_TRY(cudaMalloc(&scratch, sizeof(double) * (size_t)blocks * 256));
+  float ms = 0.f;
+  cudaError_t e = dgmb::run_peak(variant, blocks, iters, scratch, 0, &ms);
+  cudaFree(scratch);
+  if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("dg_fp64_peak: ") + cudaGetErrorString(e));
+  // DFMA: 16 FMAs per thread and iteration; DMMA m8n8k4: 8 x (8*8*4) FMAs per warp and iteration
+  const double fma_per_thread = variant == 0 ? 16.0 : 8.0 * 256.0 / 32.0;
+  *tflops_host = 2.0 * fma_per_thread * (double)iters * (double)blocks * 256.0 / (ms * 1e-3) / 1e12;
+  return DG_OK;
 }
 
 extern "C" int64_t dg_launch_count(const dg_ctx* ctx) { return ctx ? ctx->launches : 0; }

@@ -1,12 +1,61 @@
 // Internal context of the C-ABI library (not part of the public boundary).
 #pragma once
 #include <cuda_runtime.h>
+#include <cuda.h>
 #include <cstdint>
+#include <map>
+#include <mutex>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/dgvlasov.h"
 #include "dg_setup.hpp"
+
+// Every entry point runs with the context's device current and restores the caller's on return (a process may hold
+// contexts on several GPUs).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device property of a kernel: remember the largest value set per
+// (kernel, device) instead of a process-wide flag.  Call with the target device current.
+inline cudaError_t ensure_dyn_smem(const void* func, size_t bytes) {
+  static std::mutex mu;
+  static std::map<std::pair<const void*, int>, size_t> done;
+  if (bytes <= 48 * 1024) return cudaSuccess;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  size_t& cur = done[std::make_pair(func, dev)];
+  if (bytes <= cur) return cudaSuccess;
+  e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess) cur = bytes;
+  return e;
+}
+
+// key of a cached TMA descriptor: base pointer + box + swizzle + outer extent
+struct TmapKey {
+  const void* base; int b0, b1, b2, swz, outer;
+  bool operator<(const TmapKey& o) const {
+    if (base != o.base) return base < o.base;
+    if (b0 != o.b0) return b0 < o.b0;
+    if (b1 != o.b1) return b1 < o.b1;
+    if (b2 != o.b2) return b2 < o.b2;
+    if (swz != o.swz) return swz < o.swz;
+    return outer < o.outer;
+  }
+};
+
+struct ProfRecord { cudaEvent_t e0, e1; int stage; };
 
 struct dg_ctx {
   dg_grid_desc desc;
@@ -59,9 +108,15 @@ struct dg_ctx {
   int64_t launches = 0;
   int opt_rhs_kernel = 0, opt_field_kernel = 0, opt_profile = 0, opt_pdl = 1;
   int opt_form = 0;           // 0 weak form (Eq. 14), 1 strong form (Eq. 15)
-  std::vector<cudaEvent_t> prof_events;   // (start, stop) pairs around RHS launches in profile mode
-  double prof_rhs_ms = 0.0;
-  int64_t prof_rhs_launches = 0;
+  int opt_smem_pad_kb = 0;    // DG_OPT_SMEM_PAD_KB: extra dynamic shared memory per CTA of the tiled kernel (occupancy sweeps)
+  // profile mode: (start, stop) event pairs around RHS launches, tagged with the RK stage (0 = not inside dg_ssprk3_*)
+  std::vector<ProfRecord> prof_events;
+  int64_t prof_seen = 0;      // RHS launches since profile mode was set (every opt_profile-th one is bracketed)
+  int cur_stage = 0;          // stage tag of the launch being issued
+  double prof_ms[4] = {0, 0, 0, 0};
+  int64_t prof_n[4] = {0, 0, 0, 0};
+  std::map<TmapKey, CUtensorMap> tmaps;   // TMA descriptors of the arrays seen so far (f, u1, u2, halos: a handful)
+  int* d_flag = nullptr;      // library-owned word for dg_ssprk3_run_host's finiteness report
   std::string last_kernel = "none";
   std::string last_field_kernel = "none";
   double cfl_limit = -1.0;    // lazily computed

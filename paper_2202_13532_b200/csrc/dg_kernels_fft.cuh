@@ -21,6 +21,7 @@
 // place, inverse = in-place decimation in time (bit-reversed in, natural out); Re/Im of the result are
 // E_{m,2k}, E_{m,2k+1}: one 128-bit store.  Up to three radix-2 stages are fused in registers per pass.
 #pragma once
+#include "dg_context.hpp"
 #include <cuda_runtime.h>
 #include <cstdint>
 
@@ -275,11 +276,7 @@ inline bool fft_supported(int N, int n) {
 template <int NP>
 inline int launch_fft_t(const FftParams& P, int sms, cudaStream_t st) {
   const size_t smem = fft_smem_bytes(P.N, NP);
-  static size_t smem_set = 0;
-  if (smem > 48 * 1024 && smem > smem_set) {
-    if (cudaFuncSetAttribute(field_fft_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
-    smem_set = smem;
-  }
+  if (ensure_dyn_smem(reinterpret_cast<const void*>(field_fft_kernel<NP>), smem) != cudaSuccess) return -3;
   int per_sm = (int)((220 * 1024) / (smem + 1024));
   if (per_sm < 1) per_sm = 1;
   if (per_sm > 4) per_sm = 4;

@@ -8,6 +8,7 @@
 #include <cstdint>
 
 #include "../../include/dgvlasov.h"
+#include "dg_context.hpp"
 
 namespace dgf {
 
@@ -205,11 +206,7 @@ inline int launch_gemm_tn(const double* A, const double* B, double* C, int M, in
   if (variant != 1 && dmma_ok) {
     const long long tiles = (long long)((M + 127) / 128) * ((N + 127) / 128);
     if (tiles <= 0 || tiles > 0x7fffffffLL) return DG_ERR_INVALID_ARG;
-    static bool attr_set = false;
-    if (!attr_set) {
-      if (cudaFuncSetAttribute(field_gemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM_BYTES) != cudaSuccess) return DG_ERR_CUDA;
-      attr_set = true;
-    }
+    if (ensure_dyn_smem(reinterpret_cast<const void*>(field_gemm_dmma_kernel), DMMA_SMEM_BYTES) != cudaSuccess) return DG_ERR_CUDA;
     field_gemm_dmma_kernel<<<(unsigned)tiles, 256, DMMA_SMEM_BYTES, st>>>(A, B, C, M, N, K);
     return DG_OK;
   }
@@ -376,11 +373,7 @@ inline bool field_fused_supported(int G0, int Q) {
 
 inline int launch_field_fused(const FieldFusedParams& P, int grid, bool pdl, cudaStream_t st) {
   const size_t smem = field_fused_smem(P.rows, P.Q);
-  static size_t smem_set = 0;
-  if (smem > 48 * 1024 && smem > smem_set) {
-    if (cudaFuncSetAttribute(field_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return DG_ERR_CUDA;
-    smem_set = smem;
-  }
+  if (ensure_dyn_smem(reinterpret_cast<const void*>(field_fused_kernel), smem) != cudaSuccess) return DG_ERR_CUDA;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = smem; cfg.stream = st;
   cudaLaunchAttribute at[1];

@@ -85,6 +85,26 @@ __global__ void __launch_bounds__(256) rhs_generic_kernel(const GenericParams p)
   }
 }
 
+// Non-finite guard for the CFL blow-up case (the stable time step depends on the order):
+// flag[0] becomes 1 if any of the n values is Inf or NaN (the caller zeroes it first).  8 B per value, HBM-bound.
+__global__ void __launch_bounds__(256) check_finite_kernel(const double* __restrict__ f, long long n, int* __restrict__ flag) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  const long long i0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = false;
+  if ((reinterpret_cast<uintptr_t>(f) & 15) == 0) {
+    const double2* f2 = reinterpret_cast<const double2*>(f);
+    const long long n2 = n >> 1;
+    for (long long i = i0; i < n2; i += stride) {
+      const double2 v = __ldcs(f2 + i);
+      bad |= !(fabs(v.x) <= 1.7976931348623157e308) | !(fabs(v.y) <= 1.7976931348623157e308);
+    }
+    if ((n & 1) && i0 == 0) bad |= !(fabs(f[n - 1]) <= 1.7976931348623157e308);
+  } else {
+    for (long long i = i0; i < n; i += stride) bad |= !(fabs(f[i]) <= 1.7976931348623157e308);
+  }
+  if (__syncthreads_or(bad ? 1 : 0) && threadIdx.x == 0) atomicOr(flag, 1);
+}
+
 // Deterministic block reduction (fixed tree): every thread passes its partial, thread 0 gets the sum.
 template <int THREADS>
 __device__ __forceinline__ double block_reduce_sum(double v, double* smem) {

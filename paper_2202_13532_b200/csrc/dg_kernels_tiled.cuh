@@ -170,9 +170,11 @@ __device__ __forceinline__ void apply_lines2(const TiledParams<NN>& P, const dou
 // ------------------------------------------------------------------------------------------------
 // resident CTAs per SM the register allocation must allow: set for n = 10 only (134 -> 128 registers: 4 CTAs instead of 3);
 // the other orders reach the shared-memory limit with the default allocation (0 = unspecified)
-__host__ __device__ constexpr int tiled_min_ctas(int n) { return n == 10 ? 4 : 0; }   // 0: unspecified
+__host__ __device__ constexpr int tiled_min_ctas(int n) { return n == 10 ? 4 : (n == 8 ? 5 : 0); }   // 0: unspecified
 
-template <int NN, int KV>
+// FN: the stage combination reads f_n (stages 2, 3 of SSP-RK3: c0 != 0); without it (dg_rhs, stage 1) the f_n tile is
+// neither loaded nor read and the accumulator tile starts from the x-phase result.
+template <int NN, int KV, bool FN>
 __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
   using Cfg = TileCfg<NN, KV>;
   constexpr int R = Cfg::R, H = Cfg::H, RP = R / 2;
@@ -208,6 +210,11 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   // RK stage: cf = c1, cr = c1*dt.  None of this reads what the previous kernel in the stream wrote.
   const double cf = (P.mode != 0) ? P.c1 : 0.0;
   const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
+  // The speeds below carry the factor cr; the upwind side of Eq. 23 is decided by the sign of the speed itself, so a
+  // negative cr (c1 dt < 0) swaps the comparisons (the generic kernel and thread 0's halo choice use the unscaled a_d).
+  const bool flip = cr < 0.0;
+  auto is_pos = [flip](double a) { return flip ? a < 0.0 : a > 0.0; };
+  auto is_neg = [flip](double a) { return flip ? a > 0.0 : a < 0.0; };
   const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
   // phase v: rows ju and ju + H of (jx, ev).  Swizzled tiles: ju fastest (the XOR spreads the rows over the banks);
   // plain row-major tiles (R != 32): ev fastest -- a row is R/2 16-byte units and an element n/2 of them, and
@@ -228,10 +235,10 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   if (t == 0) {
     // The tile itself (and f_n) first: their byte count is known, so the transaction count is raised without
     // arriving, and the loads are in flight while the halo decision below fetches the speeds.
-    mbar_expect_tx_noarrive(bar, (P.has_fn ? 2u : 1u) * (NN * NN * R * 8));
+    mbar_expect_tx_noarrive(bar, (FN ? 2u : 1u) * (NN * NN * R * 8));
     tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
     if (Cfg::SWZ) tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
-    if (P.has_fn) {
+    if (FN) {
       tma_load_3d(smem_u32(sN), &P.m_fn, bar, c0, gu0, gx0);
       if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
     }
@@ -293,12 +300,12 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
       f[0][k] = v.x; f[1][k] = v.y;
     }
     // upwind states, Eq. 23
-    if (ax > 0.0) { const double2 v = *reinterpret_cast<const double2*>(&sXL[ju * R + c]); uL[0] = v.x; uL[1] = v.y; }
+    if (is_pos(ax)) { const double2 v = *reinterpret_cast<const double2*>(&sXL[ju * R + c]); uL[0] = v.x; uL[1] = v.y; }
     else { uL[0] = f[0][0]; uL[1] = f[1][0]; }
-    if (ax < 0.0) { const double2 v = *reinterpret_cast<const double2*>(&sXR[ju * R + c]); uR[0] = v.x; uR[1] = v.y; }
+    if (is_neg(ax)) { const double2 v = *reinterpret_cast<const double2*>(&sXR[ju * R + c]); uR[0] = v.x; uR[1] = v.y; }
     else { uR[0] = f[0][NN - 1]; uR[1] = f[1][NN - 1]; }
     apply_lines2<NN>(P, f, uL, uR, s);
-    if (P.has_fn) {
+    if (FN) {
 #pragma unroll
       for (int j = 0; j < NN; ++j) {
         double2* q = reinterpret_cast<double2*>(&sN[Cfg::idx(j * NN + ju, c)]);
@@ -323,10 +330,10 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
     }
     const double2 hl = *reinterpret_cast<const double2*>(&sUL[jx * R + c]);
     const double2 hr = *reinterpret_cast<const double2*>(&sUR[jx * R + c]);
-    uL[0] = (au[0] > 0.0) ? hl.x : f[0][0];
-    uL[1] = (au[1] > 0.0) ? hl.y : f[1][0];
-    uR[0] = (au[0] < 0.0) ? hr.x : f[0][NN - 1];
-    uR[1] = (au[1] < 0.0) ? hr.y : f[1][NN - 1];
+    uL[0] = is_pos(au[0]) ? hl.x : f[0][0];
+    uL[1] = is_pos(au[1]) ? hl.y : f[1][0];
+    uR[0] = is_neg(au[0]) ? hr.x : f[0][NN - 1];
+    uR[1] = is_neg(au[1]) ? hr.y : f[1][NN - 1];
     apply_lines2<NN>(P, f, uL, uR, s);
 #pragma unroll
     for (int j = 0; j < NN; ++j) {
@@ -355,8 +362,8 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
           acc[l][k] = a2.x; acc[l][k + 1] = a2.y;
         }
         uL[l] = f[l][0]; uR[l] = f[l][NN - 1];
-        if (av[l] > 0.0) uL[l] = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
-        if (av[l] < 0.0) uR[l] = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
+        if (is_pos(av[l])) uL[l] = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
+        if (is_neg(av[l])) uR[l] = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
       }
       apply_lines2<NN>(P, f, uL, uR, s);
 #pragma unroll
@@ -458,8 +465,13 @@ inline EncodeTiledFn encode_fn() {
   return fn;
 }
 
-inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0, int b1, int b2, bool swz128 = false,
+// TMA descriptors depend only on (base pointer, box, swizzle, outer extent): dg_ssprk3_run sees three arrays (f, u1, u2), so
+// after the first step every launch finds its descriptors in the context's cache instead of re-encoding 6-9 of them.
+inline bool make_map(CUtensorMap* m, const void* base, dg_ctx* ctx, int b0, int b1, int b2, bool swz128 = false,
                      int outer = 0) {
+  const TmapKey key{base, b0, b1, b2, swz128 ? 1 : 0, outer};
+  auto it = ctx->tmaps.find(key);
+  if (it != ctx->tmaps.end()) { *m = it->second; return true; }
   EncodeTiledFn enc = encode_fn();
   if (!enc) { g_tiled_err = "cuTensorMapEncodeTiled not available"; return false; }
   const cuuint64_t dims[3] = {(cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)(outer > 0 ? outer : ctx->G[0])};
@@ -470,10 +482,12 @@ inline bool make_map(CUtensorMap* m, const void* base, const dg_ctx* ctx, int b0
                    CU_TENSOR_MAP_INTERLEAVE_NONE, swz128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { g_tiled_err = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r); return false; }
+  if (ctx->tmaps.size() >= 512) ctx->tmaps.clear();      // callers cycling through many arrays: start over
+  ctx->tmaps[key] = *m;
   return true;
 }
 
-template <int NN, int KV>
+template <int NN, int KV, bool FN>
 int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                        double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
   using Cfg = TileCfg<NN, KV>;
@@ -483,8 +497,10 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   const int RB = Cfg::SWZ ? 16 : R;      // swizzled tiles move as two 128-byte-wide boxes
   if (!make_map(&P.m_main, f, ctx, RB, NN, NN, Cfg::SWZ) || !make_map(&P.m_xface, f, ctx, R, NN, 1) ||
       !make_map(&P.m_uface, f, ctx, R, 1, NN) || !make_map(&P.m_vface, f, ctx, 2, NN, NN) ||
-      !make_map(&P.m_fn, fn ? fn : f, ctx, RB, NN, NN, Cfg::SWZ) || !make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ))
+      !make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ))
     return DG_ERR_CUDA;
+  if (FN) { if (!make_map(&P.m_fn, fn, ctx, RB, NN, NN, Cfg::SWZ)) return DG_ERR_CUDA; }
+  else P.m_fn = P.m_main;
   if (ctx->desc.bc[0] == 2) {
     if (!ctx->xhalo) { g_tiled_err = "bc[0] = DG_BC_HALO needs dg_set_xhalo first"; return DG_ERR_INVALID_ARG; }
     if (!make_map(&P.m_xhalo, ctx->xhalo, ctx, R, NN, 1, false, 2)) return DG_ERR_CUDA;
@@ -518,39 +534,46 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   P.N0 = ctx->N[0]; P.N1 = ctx->N[1]; P.N2 = ctx->N[2]; P.G0 = ctx->G[0]; P.G1 = ctx->G[1]; P.G2 = ctx->G[2];
   P.bc0 = ctx->desc.bc[0]; P.bc1 = ctx->desc.bc[1]; P.bc2 = ctx->desc.bc[2];
   P.tiles_v = (ctx->N[2] + KV - 1) / KV;
-  P.mode = mode; P.has_fn = (mode != 0 && fn != nullptr) ? 1 : 0;
+  P.mode = mode; P.has_fn = FN ? 1 : 0;
   const size_t chunks = (size_t)P.N1 * P.tiles_v;
   P.want_partials = (want_partials && ctx->partials && chunks * ctx->G[0] <= ctx->partials_doubles) ? 1 : 0;
   if (partial_chunks) *partial_chunks = P.want_partials ? (int)chunks : 0;
 
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(rhs_tiled_kernel<NN, KV>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+  // DG_OPT_SMEM_PAD_KB: unused extra shared memory per CTA, to lower the number of resident CTAs (occupancy sweeps)
+  const size_t smem_bytes = (size_t)Cfg::SMEM_BYTES + (size_t)ctx->opt_smem_pad_kb * 1024;
+  {
+    cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(rhs_tiled_kernel<NN, KV, FN>), smem_bytes);
     if (e != cudaSuccess) { g_tiled_err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return DG_ERR_CUDA; }
-    attr_set = true;
   }
   const long long tiles = (long long)P.N0 * P.N1 * P.tiles_v;
   if (tiles > 0x7fffffffLL) { g_tiled_err = "too many tiles"; return DG_ERR_UNSUPPORTED; }
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)tiles); cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = Cfg::SMEM_BYTES; cfg.stream = st;
+  cfg.gridDim = dim3((unsigned)tiles); cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = smem_bytes; cfg.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = (ctx->opt_pdl && !ctx->opt_profile) ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, rhs_tiled_kernel<NN, KV>, P);
+  // DG_OPT_PROFILE = 1 (every launch bracketed by events) measures the kernel alone, without programmatic launches
+  cfg.attrs = at; cfg.numAttrs = (ctx->opt_pdl && ctx->opt_profile != 1) ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, rhs_tiled_kernel<NN, KV, FN>, P);
   ctx->last_kernel = "rhs_tiled<" + std::to_string(NN) + "," + std::to_string(KV) + ">";
   return DG_OK;
 }
 
 inline int launch_rhs_tiled(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                             double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
+  const bool has_fn = (mode != 0 && fn != nullptr);
+#define DG_TILED_CASE(NN_, KV_)                                                                                                  \
+  case NN_:                                                                                                                      \
+    return has_fn ? launch_rhs_tiled_t<NN_, KV_, true>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st)  \
+                  : launch_rhs_tiled_t<NN_, KV_, false>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
   switch (ctx->n[0]) {
-    case 4: return launch_rhs_tiled_t<4, 8>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-    case 6: return launch_rhs_tiled_t<6, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-    case 8: return launch_rhs_tiled_t<8, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-    case 10: return launch_rhs_tiled_t<10, 2>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    DG_TILED_CASE(4, 8)
+    DG_TILED_CASE(6, 4)
+    DG_TILED_CASE(8, 4)
+    DG_TILED_CASE(10, 2)
     default: g_tiled_err = "order not supported by the tiled kernel"; return DG_ERR_UNSUPPORTED;
   }
+#undef DG_TILED_CASE
 }
 
 }  // namespace dgt

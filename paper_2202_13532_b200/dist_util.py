@@ -18,10 +18,32 @@ def init(backend: str, device=None):
     world, rank, _ = env_world()
     if world > 1 and not dist.is_initialized():
         kw = {}
+        log = None
         if backend == "nccl" and device is not None:
             kw["device_id"] = device
+            # NCCL's communicator lines go to a per-process file (stdout carries the one JSON line); rank 0 echoes its
+            # "Init COMPLETE" line to stderr after the first collective so that a reader can see the N ranks
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+            log = os.environ.setdefault("NCCL_DEBUG_FILE", "/tmp/dg_nccl_%h_%p.log")
         dist.init_process_group(backend, **kw)
+        if log is not None:
+            dist.barrier()
+            _echo_nccl_init(log, rank)
     return world, rank
+
+
+def _echo_nccl_init(pattern: str, rank: int):
+    import socket
+    import sys
+    path = pattern.replace("%h", socket.gethostname()).replace("%p", str(os.getpid()))
+    try:
+        lines = [l.rstrip() for l in open(path) if "Init COMPLETE" in l or "nranks" in l]
+    except OSError:
+        return
+    if rank == 0:
+        for l in lines[-2:]:
+            print("[nccl] " + l, file=sys.stderr, flush=True)
 
 
 def barrier(device=None):

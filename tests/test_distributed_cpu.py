@@ -35,6 +35,19 @@ def test_reference_arm_prints_contract_line():
     assert out["e2e"]["h2d_bytes_per_step"] == 0 and out["unit"] == "DOF-updates/s"
 
 
+def test_bench_gpus_2_starts_two_ranks_itself():
+    """`python bench.py --gpus 2` without a torchrun environment starts the two ranks itself; the line says n_gpus = 2
+    (reference arm: rank 0 alone runs the oracle, the other rank exits 0 without work)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--steps", "1",
+                          "--warmup", "0", "--workload", "small_1d2v_128^3"], capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                   # rank 0 only
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["impl"] == "reference"
+
+
 def test_xslab_partition():
     sys.path.insert(0, ROOT)
     from paper_2202_13532_b200 import sharded
