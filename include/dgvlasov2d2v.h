@@ -72,8 +72,9 @@ int dg4_get_nodes(const dg4_ctx* ctx, int32_t dim, double* coords_host /*[N_d*n_
 /* Largest dt with sum_d |a_d| dt / Delta_d within the SSP-RK3 limit of this order and mass mode at |E_x|, |E_y| <= E_bound
  * (as dg_max_stable_dt). */
 double dg4_max_stable_dt(const dg4_ctx* ctx, double E_bound);
-#define DG4_OPT_RHS_KERNEL 1   /* 0 auto (tiled when all orders are 4 and N_v is even; element kernel for equal orders 6 or 8;
-                                  else generic), 1 generic, 2 tiled, 3 element kernel (equal orders 4, 6, 8); 2 and 3 fail with
+#define DG4_OPT_RHS_KERNEL 1   /* 0 auto (tiled when all orders are 4 and N_v is even; TMA line kernel for order 8 in all
+                                  dimensions; element kernel for equal orders 6; else generic), 1 generic, 2 tiled, 3 element
+                                  kernel (equal orders 4, 6, 8), 4 line kernel (order 8); 2, 3 and 4 fail with
                                   DG_ERR_UNSUPPORTED on other shapes */
 #define DG4_OPT_PROFILE    3   /* k >= 1: bracket every k-th RHS-kernel launch with CUDA events on its stream (0 off) */
 int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value);

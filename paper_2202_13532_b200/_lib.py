@@ -8,7 +8,8 @@ import ctypes as C
 import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libdgvlasov.so")
+# DGVLASOV_LIB: another build of the same library (kernel A/B comparisons); default: the in-tree build
+LIB_PATH = os.environ.get("DGVLASOV_LIB") or os.path.join(HERE, "libdgvlasov.so")
 
 
 class GridDesc(C.Structure):

@@ -262,7 +262,7 @@ class DGContext:
 
 
 OPT4_RHS_KERNEL, OPT4_PROFILE = 1, 3
-KERNEL4_AUTO, KERNEL4_GENERIC, KERNEL4_TILED, KERNEL4_ELEMENT = 0, 1, 2, 3
+KERNEL4_AUTO, KERNEL4_GENERIC, KERNEL4_TILED, KERNEL4_ELEMENT, KERNEL4_LINE = 0, 1, 2, 3, 4
 
 
 class DG4Context:

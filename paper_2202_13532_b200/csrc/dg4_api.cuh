@@ -5,6 +5,7 @@
 #include "dg4_kernels.cuh"
 #include "dg4_kernels_tiled.cuh"
 #include "dg4_kernels_elem.cuh"
+#include "dg4_kernels_line.cuh"
 
 struct dg4_ctx {
   dg4_grid_desc desc;
@@ -31,6 +32,7 @@ struct dg4_ctx {
   double prof_ms = 0.0;
   int64_t prof_launches = 0;
   std::string last_kernel = "none";
+  std::map<TmapKey, CUtensorMap> tmaps;   // TMA descriptors of the arrays seen so far (line kernel)
 };
 
 static int check4(dg4_ctx* ctx, const char* what) {
@@ -206,6 +208,82 @@ extern "C" int dg4_set_workspace(dg4_ctx* ctx, void* ws_dev, size_t bytes) {
 // ------------------------------------------------------------------------------------------------
 // launches
 // ------------------------------------------------------------------------------------------------
+// 4-D TMA descriptor of an array f[G0][G1][G2][G3] with box (b0 = v, b1 = u, b2 = y, b3 = x); cached per (base, box).
+static bool make_map4(CUtensorMap* m, const void* base, dg4_ctx* ctx, int b0, int b1, int b2, int b3, bool swz64) {
+  const TmapKey key{base, b0, b1, b2 * 16 + b3, swz64 ? 2 : 0, 4};
+  auto it = ctx->tmaps.find(key);
+  if (it != ctx->tmaps.end()) { *m = it->second; return true; }
+  dgt::EncodeTiledFn enc = dgt::encode_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)ctx->G[3], (cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)ctx->G[0]};
+  const cuuint64_t strides[3] = {(cuuint64_t)ctx->G[3] * 8, (cuuint64_t)ctx->G[3] * ctx->G[2] * 8,
+                                 (cuuint64_t)ctx->G[3] * ctx->G[2] * ctx->G[1] * 8};
+  const cuuint32_t box[4] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, swz64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  if (ctx->tmaps.size() >= 512) ctx->tmaps.clear();
+  ctx->tmaps[key] = *m;
+  return true;
+}
+
+// n = 8 in all four dimensions, G_v*8 a multiple of 16 bytes (always), arrays 16-byte aligned: the TMA line kernel
+static bool line_supported(const dg4_ctx* ctx) {
+  for (int d = 0; d < 4; ++d) if (ctx->n[d] != 8) return false;
+  return true;
+}
+
+static int launch_rhs4_line(dg4_ctx* ctx, const double* f, const double* fn, const double* Ex, const double* Ey, double* out,
+                            int mode, double c0, double c1, double dt, bool want_partials, int* chunks_out, cudaStream_t st) {
+  dg4l::LineParams P;
+  memset(&P, 0, sizeof(P));
+  const bool with_fn = mode != 0 && fn != nullptr;
+  bool ok = make_map4(&P.m_main, f, ctx, 8, 8, 8, 8, true) && make_map4(&P.m_out, out, ctx, 8, 8, 8, 8, true) &&
+            make_map4(&P.m_xface, f, ctx, 8, 8, 8, 1, false) && make_map4(&P.m_yface, f, ctx, 8, 8, 1, 8, false) &&
+            make_map4(&P.m_uface, f, ctx, 8, 1, 8, 8, false) && make_map4(&P.m_vface, f, ctx, 2, 8, 8, 8, false);
+  if (ok && with_fn) ok = make_map4(&P.m_fn, fn, ctx, 8, 8, 8, 8, true);
+  else P.m_fn = P.m_main;
+  if (!ok) return fail(DG_ERR_CUDA, "dg4: cuTensorMapEncodeTiled failed");
+  const dgsetup::Basis1D& b = ctx->basis[0];
+  for (int j = 0; j < 4; ++j) {
+    for (int k = 0; k < 4; ++k) {
+      P.pe[j * 4 + k] = 0.5 * (b.ups[j * 8 + k] + b.ups[j * 8 + 7 - k]);
+      P.qo[j * 4 + k] = 0.5 * (b.ups[j * 8 + k] - b.ups[j * 8 + 7 - k]);
+    }
+    P.la[j] = 0.5 * (b.lift[2 * j] - b.lift[2 * j + 1]);
+    P.lb[j] = 0.5 * (b.lift[2 * j] + b.lift[2 * j + 1]);
+  }
+  for (int j = 0; j < 8; ++j) P.wref[j] = b.w[j];
+  P.cu = ctx->d_coord[2]; P.cv = ctx->d_coord[3]; P.Ex = Ex; P.Ey = Ey;
+  P.Jx = ctx->J[0]; P.Jy = ctx->J[1]; P.Ju = ctx->J[2]; P.Jv = ctx->J[3]; P.omega_c = ctx->desc.omega_c;
+  P.wscale = 1.0 / (ctx->J[2] * ctx->J[3]);
+  P.c0 = c0; P.c1 = c1; P.dt = dt; P.mode = mode; P.strong = 0;
+  for (int d = 0; d < 4; ++d) { P.N[d] = ctx->N[d]; P.G[d] = ctx->G[d]; P.bc[d] = ctx->desc.bc[d]; }
+  P.chunks = ctx->N[2] * ctx->N[3];
+  if (want_partials && mode != 0 && ctx->partials && (size_t)ctx->G[0] * ctx->G[1] * P.chunks <= ctx->partials_doubles) {
+    P.partials = ctx->partials; P.want_partials = 1;
+    if (chunks_out) *chunks_out = P.chunks;
+  }
+  // x-elements per rasterisation group (as the n = 4 tiled kernel): a power of two <= 8 dividing N_x, grown while the tiles
+  // between a tile and its y neighbour (three 32 KB tiles each) stay within ~32 MB, a quarter of the L2
+  int bxl = 0;
+  while (bxl < 3 && ctx->N[0] % (2 << bxl) == 0 && (double)ctx->N[2] * ctx->N[3] * (2 << bxl) * 3.0 * 32768.0 <= 32e6) ++bxl;
+  P.bx_log2 = bxl;
+  const long long tiles = (long long)ctx->N[0] * ctx->N[1] * ctx->N[2] * ctx->N[3];
+  if (tiles > 0x7fffffffLL) return fail(DG_ERR_UNSUPPORTED, "dg4: too many tiles");
+  if (with_fn) {
+    CUDA_TRY(ensure_dyn_smem(reinterpret_cast<const void*>(dg4l::rhs4_line_kernel<true>), dg4l::SMEM_BYTES));
+    dg4l::rhs4_line_kernel<true><<<(unsigned)tiles, dg4l::NT, dg4l::SMEM_BYTES, st>>>(P);
+  } else {
+    CUDA_TRY(ensure_dyn_smem(reinterpret_cast<const void*>(dg4l::rhs4_line_kernel<false>), dg4l::SMEM_BYTES));
+    dg4l::rhs4_line_kernel<false><<<(unsigned)tiles, dg4l::NT, dg4l::SMEM_BYTES, st>>>(P);
+  }
+  ctx->last_kernel = "rhs4_line<8>";
+  return check4(ctx, "rhs4_line_kernel");
+}
+
 static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, const double* Ex, const double* Ey, double* out,
                              int mode, double c0, double c1, double dt, bool want_partials, int* chunks_out, cudaStream_t st) {
   if (chunks_out) *chunks_out = 0;
@@ -252,6 +330,10 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
     ctx->last_kernel = kv == 8 ? "rhs4_tile<8>" : (kv == 4 ? "rhs4_tile<4>" : "rhs4_tile<2>");
     return check4(ctx, "rhs4_tile_kernel");
   }
+  if (ctx->opt_kernel == 4 && !(line_supported(ctx) && aligned))
+    return fail(DG_ERR_UNSUPPORTED, "dg4: the line kernel needs order 8 in all dimensions and 16-byte aligned arrays");
+  if (line_supported(ctx) && aligned && (ctx->opt_kernel == 0 || ctx->opt_kernel == 4))
+    return launch_rhs4_line(ctx, f, fn, Ex, Ey, out, mode, c0, c1, dt, want_partials, chunks_out, st);
   const int ne = elem_order(ctx);
   if (ctx->opt_kernel == 3 && !(ne && aligned))
     return fail(DG_ERR_UNSUPPORTED, "dg4: the element kernel needs equal orders 4, 6 or 8 and 16-byte aligned arrays");
@@ -473,7 +555,7 @@ extern "C" double dg4_max_stable_dt(const dg4_ctx* ctx, double E_bound) {
 
 extern "C" int dg4_set_option(dg4_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_set_option: null context");
-  if (key == DG4_OPT_RHS_KERNEL && value >= 0 && value <= 3) { ctx->opt_kernel = (int)value; return DG_OK; }
+  if (key == DG4_OPT_RHS_KERNEL && value >= 0 && value <= 4) { ctx->opt_kernel = (int)value; return DG_OK; }
   if (key == DG4_OPT_PROFILE && value >= 0 && value <= 1000000) { ctx->opt_profile = (int)value; ctx->prof_seen = 0; return DG_OK; }
   return fail(DG_ERR_INVALID_ARG, "dg4_set_option: unknown key or value");
 }

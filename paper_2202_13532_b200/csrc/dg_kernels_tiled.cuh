@@ -133,8 +133,9 @@ struct TileCfg {
 
 // Two lines at once (the operator coefficients are fetched once for both):
 // s[l][j] = (Ups f_l - Xi_R uR_l + Xi_L uL_l)_j, reference element (Eq. 14 / 20 / 21).
-template <int NN>
-__device__ __forceinline__ void apply_lines2(const TiledParams<NN>& P, const double (&f)[2][NN], const double (&uL)[2],
+// PT: any parameter block with members pe, qo, la, lb, strong (TiledParams here, LineParams of the 2D2V line kernel).
+template <int NN, class PT>
+__device__ __forceinline__ void apply_lines2(const PT& P, const double (&f)[2][NN], const double (&uL)[2],
                                              const double (&uR)[2], double (&s)[2][NN]) {
   constexpr int H = NN / 2;
   double e[2][H], o[2][H], sp[2], dm[2];
@@ -170,12 +171,16 @@ __device__ __forceinline__ void apply_lines2(const TiledParams<NN>& P, const dou
 // ------------------------------------------------------------------------------------------------
 // resident CTAs per SM the register allocation must allow: set for n = 10 only (134 -> 128 registers: 4 CTAs instead of 3);
 // the other orders reach the shared-memory limit with the default allocation (0 = unspecified)
-__host__ __device__ constexpr int tiled_min_ctas(int n) { return n == 10 ? 4 : (n == 8 ? 5 : 0); }   // 0: unspecified
+// (n = 8 must NOT be given a minimum: ptxas reaches 96 registers, five CTAs, without spills on its own, and spills 44 bytes per
+// thread when asked for five -- measured 1.51 -> 1.65 ms per step at 512^3)
+__host__ __device__ constexpr int tiled_min_ctas(int n) { return n == 10 ? 4 : 0; }   // 0: unspecified
 
-// FN: the stage combination reads f_n (stages 2, 3 of SSP-RK3: c0 != 0); without it (dg_rhs, stage 1) the f_n tile is
-// neither loaded nor read and the accumulator tile starts from the x-phase result.
-template <int NN, int KV, bool FN>
+// has_fn: the stage combination reads f_n (stages 2, 3 of SSP-RK3: c0 != 0); without it (dg_rhs, stage 1) the f_n tile is
+// neither loaded nor read and the accumulator tile starts from the x-phase result.  (A compile-time flag instead of this
+// CTA-uniform branch costs 6 registers at n = 8 -- 102 instead of 96, four CTAs per SM instead of five: measured, dropped.)
+template <int NN, int KV>
 __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
+  const bool FN = P.has_fn != 0;
   using Cfg = TileCfg<NN, KV>;
   constexpr int R = Cfg::R, H = Cfg::H, RP = R / 2;
   extern __shared__ __align__(1024) unsigned char smem[];
@@ -487,7 +492,7 @@ inline bool make_map(CUtensorMap* m, const void* base, dg_ctx* ctx, int b0, int 
   return true;
 }
 
-template <int NN, int KV, bool FN>
+template <int NN, int KV>
 int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                        double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
   using Cfg = TileCfg<NN, KV>;
@@ -499,7 +504,8 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
       !make_map(&P.m_uface, f, ctx, R, 1, NN) || !make_map(&P.m_vface, f, ctx, 2, NN, NN) ||
       !make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ))
     return DG_ERR_CUDA;
-  if (FN) { if (!make_map(&P.m_fn, fn, ctx, RB, NN, NN, Cfg::SWZ)) return DG_ERR_CUDA; }
+  const bool has_fn = (mode != 0 && fn != nullptr);
+  if (has_fn) { if (!make_map(&P.m_fn, fn, ctx, RB, NN, NN, Cfg::SWZ)) return DG_ERR_CUDA; }
   else P.m_fn = P.m_main;
   if (ctx->desc.bc[0] == 2) {
     if (!ctx->xhalo) { g_tiled_err = "bc[0] = DG_BC_HALO needs dg_set_xhalo first"; return DG_ERR_INVALID_ARG; }
@@ -534,7 +540,7 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   P.N0 = ctx->N[0]; P.N1 = ctx->N[1]; P.N2 = ctx->N[2]; P.G0 = ctx->G[0]; P.G1 = ctx->G[1]; P.G2 = ctx->G[2];
   P.bc0 = ctx->desc.bc[0]; P.bc1 = ctx->desc.bc[1]; P.bc2 = ctx->desc.bc[2];
   P.tiles_v = (ctx->N[2] + KV - 1) / KV;
-  P.mode = mode; P.has_fn = FN ? 1 : 0;
+  P.mode = mode; P.has_fn = has_fn ? 1 : 0;
   const size_t chunks = (size_t)P.N1 * P.tiles_v;
   P.want_partials = (want_partials && ctx->partials && chunks * ctx->G[0] <= ctx->partials_doubles) ? 1 : 0;
   if (partial_chunks) *partial_chunks = P.want_partials ? (int)chunks : 0;
@@ -542,7 +548,7 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   // DG_OPT_SMEM_PAD_KB: unused extra shared memory per CTA, to lower the number of resident CTAs (occupancy sweeps)
   const size_t smem_bytes = (size_t)Cfg::SMEM_BYTES + (size_t)ctx->opt_smem_pad_kb * 1024;
   {
-    cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(rhs_tiled_kernel<NN, KV, FN>), smem_bytes);
+    cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(rhs_tiled_kernel<NN, KV>), smem_bytes);
     if (e != cudaSuccess) { g_tiled_err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return DG_ERR_CUDA; }
   }
   const long long tiles = (long long)P.N0 * P.N1 * P.tiles_v;
@@ -554,26 +560,20 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   at[0].val.programmaticStreamSerializationAllowed = 1;
   // DG_OPT_PROFILE = 1 (every launch bracketed by events) measures the kernel alone, without programmatic launches
   cfg.attrs = at; cfg.numAttrs = (ctx->opt_pdl && ctx->opt_profile != 1) ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, rhs_tiled_kernel<NN, KV, FN>, P);
+  cudaLaunchKernelEx(&cfg, rhs_tiled_kernel<NN, KV>, P);
   ctx->last_kernel = "rhs_tiled<" + std::to_string(NN) + "," + std::to_string(KV) + ">";
   return DG_OK;
 }
 
 inline int launch_rhs_tiled(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                             double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
-  const bool has_fn = (mode != 0 && fn != nullptr);
-#define DG_TILED_CASE(NN_, KV_)                                                                                                  \
-  case NN_:                                                                                                                      \
-    return has_fn ? launch_rhs_tiled_t<NN_, KV_, true>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st)  \
-                  : launch_rhs_tiled_t<NN_, KV_, false>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
   switch (ctx->n[0]) {
-    DG_TILED_CASE(4, 8)
-    DG_TILED_CASE(6, 4)
-    DG_TILED_CASE(8, 4)
-    DG_TILED_CASE(10, 2)
+    case 4: return launch_rhs_tiled_t<4, 8>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 6: return launch_rhs_tiled_t<6, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 8: return launch_rhs_tiled_t<8, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 10: return launch_rhs_tiled_t<10, 2>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
     default: g_tiled_err = "order not supported by the tiled kernel"; return DG_ERR_UNSUPPORTED;
   }
-#undef DG_TILED_CASE
 }
 
 }  // namespace dgt

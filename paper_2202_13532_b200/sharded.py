@@ -20,7 +20,7 @@ NVLink, symmetric-memory allocation), into the buffer of the other parity than t
 all-gather of step 2 is then the only thing that orders the ranks between two stages.
 
 This module is host plumbing only: which planes go where, and in what order the C-ABI calls and the
-torch.distributed calls are issued.  The arithmetic runs behind the `backend` object -- `CudaBackend`
+torch.distributed calls are issued (the stage coefficients too come from the backend: dg_ssprk3_stage_coeffs).  The arithmetic runs behind the `backend` object -- `CudaBackend`
 (libdgvlasov kernels) in the product; there is no CPU backend here, and constructing `CudaBackend`
 without a CUDA device raises.  The CPU tests drive the same plumbing over gloo with a backend of their
 own (tests/_xslab_worker.py).
@@ -29,9 +29,6 @@ from __future__ import annotations
 
 import torch
 import torch.distributed as dist
-
-SSPRK3 = ((0.0, 1.0), (0.75, 0.25), (1.0 / 3.0, 2.0 / 3.0))      # (c0, c1) per stage, Shu-Osher form (PAPER.md:477)
-
 
 def slab_partition(n_elem_x: int, world: int):
     """[(e0, e1)] per rank: contiguous, sizes differ by at most one element, every rank non-empty."""
@@ -160,6 +157,10 @@ class CudaBackend:
     def set_push(self, left_dst, right_dst):
         self.slab.set_xhalo_push(left_dst, right_dst)
 
+    def stage_coeffs(self, stage):
+        """(c0, c1) of Shu-Osher stage 0, 1, 2: the table lives in the library (dg_ssprk3_stage_coeffs)."""
+        return self.api.ssprk3_stage_coeffs(stage)
+
     def close(self):
         self.slab.close(); self.field.close()
 
@@ -230,7 +231,7 @@ class XSlabStepper:
     def step(self, f, dt, self_consistent=True, rho_known=False):
         """u1 = u + dt L(u); u2 = 3/4 u + 1/4 (u1 + dt L(u1)); u <- 1/3 u + 2/3 (u2 + dt L(u2)), in place.
         rho_known is for run(): a lone step cannot know whether the caller touched f since the last one."""
-        (a0, b0), (a1, b1), (a2, b2) = SSPRK3
+        (a0, b0), (a1, b1), (a2, b2) = (self.be.stage_coeffs(s) for s in range(3))     # method arithmetic stays behind the backend
         self.stage(f, f, self.u1, a0, b0, dt, self_consistent, rho_known)
         self.stage(self.u1, f, self.u2, a1, b1, dt, self_consistent, True)
         self.stage(self.u2, f, f, a2, b2, dt, self_consistent, True)

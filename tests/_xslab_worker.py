@@ -53,6 +53,10 @@ class OracleSlabBackend:
     def set_halo(self, halo):
         self.halo = halo
 
+    def stage_coeffs(self, stage):
+        """Shu-Osher table as oracle.vlasov.ssprk3_step writes it out (reading C3)."""
+        return ((0.0, 1.0), (0.75, 0.25), (1.0 / 3.0, 2.0 / 3.0))[stage]
+
     def rk_stage(self, f_s, f_n, E_loc, out, c0, c1, dt, rho_out=None):
         n = self.n
         fs = f_s.numpy()

@@ -60,7 +60,9 @@ def test_rhs_matches_oracle(N, n, bc, mode):
     assert relerr(r, ro) < 1e-12, ctx.last_kernel
     if all(k == 4 for k in n) and N[3] % 2 == 0:
         expect = "rhs4_tile"
-    elif n in ((6, 6, 6, 6), (8, 8, 8, 8)):
+    elif n == (8, 8, 8, 8):
+        expect = "rhs4_line"
+    elif n == (6, 6, 6, 6):
         expect = "rhs4_elem"
     else:
         expect = "rhs4_generic"
@@ -103,6 +105,45 @@ def test_element_kernel_stage_and_density(N, n, bc):
     ctx.set_option(api().OPT4_RHS_KERNEL, 1)
     b = ctx.rhs(fd, exd, eyd).cpu().numpy()
     assert relerr(a, ro) < 1e-12 and relerr(a, b) < 1e-13
+    ctx.close()
+
+
+@pytest.mark.parametrize("N", [(2, 1, 2, 2), (1, 2, 3, 2), (3, 2, 1, 1), (4, 2, 2, 3)])
+@pytest.mark.parametrize("bc", [(0, 0, 1, 1), (1, 1, 0, 0), (0, 0, 0, 0)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_line_kernel_stage_and_density(N, bc, mode):
+    """rhs4_line_kernel (n = 8, TMA): what `auto` takes at the paper's order.  One Shu-Osher stage with f_n and the epilogue
+    density, a stage without f_n, the plain RHS against the oracle and against the generic and element kernels on the device
+    (the mirrored u lines of the odd-jy threads and the x-rasterisation groups are both exercised by N_x = 4, N_y = 2)."""
+    n = (8, 8, 8, 8)
+    g, ctx = make_pair(N, n, bc=bc, mass_mode=mode)
+    f, Ex, Ey = seeded_inputs(g)
+    fn = 0.5 + wl.counter_uniform_chunked(wl.SEED_CFG6_E, f.size).reshape(f.shape)
+    fd, fnd, exd, eyd = dev(f), dev(fn), dev(Ex), dev(Ey)
+    out, rho = torch.empty_like(fd), torch.empty(g.flat_shape[:2], dtype=torch.float64, device="cuda")
+    ctx.rk_stage(fd, fnd, exd, eyd, out, 1.0 / 3.0, 2.0 / 3.0, 1e-3, rho_out=rho)
+    assert ctx.last_kernel == "rhs4_line<8>"
+    ro = o4.rhs(g, f, Ex, Ey)
+    oo = (1.0 / 3.0) * fn + (2.0 / 3.0) * (f + 1e-3 * ro)
+    assert relerr(out.cpu().numpy(), oo) < 1e-13
+    assert relerr(rho.cpu().numpy(), o4.density(g, oo)) < 1e-13
+    # in place on f_n (stage 3 of dg4_ssprk3_run) and without f_n (stage 1), negative dt (upwind side from the unscaled speed)
+    inpl = fnd.clone()
+    ctx.rk_stage(fd, inpl, exd, eyd, inpl, 1.0 / 3.0, 2.0 / 3.0, 1e-3)
+    assert torch.equal(inpl, out)
+    ctx.rk_stage(fd, None, exd, eyd, out, 0.0, 1.0, -2e-3)
+    assert np.max(np.abs(out.cpu().numpy() - (f - 2e-3 * ro))) <= 1e-12 * 2e-3 * np.max(np.abs(ro))
+    a = ctx.rhs(fd, exd, eyd).cpu().numpy()
+    assert ctx.last_kernel == "rhs4_line<8>"
+    ctx.set_option(api().OPT4_RHS_KERNEL, 1)
+    b = ctx.rhs(fd, exd, eyd).cpu().numpy()
+    ctx.set_option(api().OPT4_RHS_KERNEL, 3)
+    c = ctx.rhs(fd, exd, eyd).cpu().numpy()
+    assert ctx.last_kernel.startswith("rhs4_elem")
+    assert relerr(a, ro) < 1e-12 and relerr(a, b) < 1e-13 and relerr(a, c) < 1e-13
+    # E = NULL
+    ctx.set_option(api().OPT4_RHS_KERNEL, 0)
+    assert relerr(ctx.rhs(fd).cpu().numpy(), o4.rhs(g, f)) < 1e-12
     ctx.close()
 
 
