@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
     else { uL[0] = f[0][0]; uL[1] = f[1][0]; }
     if (is_neg(ax)) { const double2 v = *reinterpret_cast<const double2*>(&sXR[rbase * NN + c2]); uR[0] = v.x; uR[1] = v.y; }
     else { uR[0] = f[0][NN - 1]; uR[1] = f[1][NN - 1]; }
-    dgt::apply_lines2<NN>(P, f, uL, uR, s);
+    dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
 #pragma unroll
     for (int j = 0; j < NN; ++j) {
       double2* q = reinterpret_cast<double2*>(&sN[chunk_off(j * 64 + rbase, cv)]);
@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
     uL[1] = is_pos(ay1) ? hl.y : f[1][0];
     uR[0] = is_neg(ay0) ? hr.x : f[0][NN - 1];
     uR[1] = is_neg(ay1) ? hr.y : f[1][NN - 1];
-    dgt::apply_lines2<NN>(P, f, uL, uR, s);
+    dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
 #pragma unroll
     for (int j = 0; j < NN; ++j) {
       double2* q = reinterpret_cast<double2*>(&sN[chunk_off(rbase + j * NN, cv)]);
@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
     uL[1] = is_pos(au1) ? hl.y : f[1][0];
     uR[0] = is_neg(au0) ? hr.x : f[0][NN - 1];
     uR[1] = is_neg(au1) ? hr.y : f[1][NN - 1];
-    dgt::apply_lines2<NN>(P, f, uL, uR, s);
+    dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
 #pragma unroll
     for (int i = 0; i < NN; ++i) {
       double2* q = reinterpret_cast<double2*>(&sN[chunk_off(rbase + (i ^ urev), cv)]);
@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
       if (is_pos(avl[l])) uL[l] = sVL[row * 2 + 1];
       if (is_neg(avl[l])) uR[l] = sVR[row * 2];
     }
-    dgt::apply_lines2<NN>(P, f, uL, uR, s);
+    dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
     double psum[2] = {0.0, 0.0};
 #pragma unroll
     for (int l = 0; l < 2; ++l) {

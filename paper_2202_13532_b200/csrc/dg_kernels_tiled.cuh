@@ -5,8 +5,8 @@
 //
 // One CTA owns a tile of 1 x-element x 1 u-element x KV v-elements: NN x NN x (KV*NN) nodes, rows of
 // KV*NN contiguous doubles.  TMA (cp.async.bulk.tensor.3d) brings the tile, its upwind face halos and
-// the f_n tile into shared memory on one mbarrier; three phases contract along x, u and v with one
-// thread per line (operators come from the kernel-parameter constant bank); the result goes back
+// the f_n tile into shared memory on one mbarrier; three phases contract along x, u and v with two
+// lines per thread (operators come from the kernel-parameter constant bank); the result goes back
 // through shared memory and one TMA store.  Several CTAs per SM overlap load / compute / store.
 #pragma once
 #include <cuda.h>
@@ -58,7 +58,6 @@ __device__ __forceinline__ void tma_store_commit_and_wait_read() {
   asm volatile("cp.async.bulk.commit_group;" ::: "memory");
   asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
-
 // ------------------------------------------------------------------------------------------------
 // parameters
 // ------------------------------------------------------------------------------------------------
@@ -76,8 +75,8 @@ struct alignas(64) TiledParams {
   CUtensorMap m_uface;   // f_s, box (R, 1, NN)
   CUtensorMap m_vface;   // f_s, box (2, NN, NN)
   CUtensorMap m_fn;      // f_n, box as m_main
-  CUtensorMap m_out;     // output, box as m_main
   CUtensorMap m_xhalo;   // exterior x-face planes [2][G1][G2] of an x-slab (bc0 = 2), box (R, NN, 1)
+  CUtensorMap m_out;     // output, box as m_main
   CUtensorMap m_pushL;   // plane [G1][G2] in the LEFT x-neighbour's halo buffer: receives this slab's first x plane of out
   CUtensorMap m_pushR;   // plane [G1][G2] in the RIGHT x-neighbour's halo buffer: receives this slab's last x plane of out
   double pe[NN * NN / 4];
@@ -89,15 +88,14 @@ struct alignas(64) TiledParams {
   const double* vy;      // node coordinates of dim 2 (v = v_y)
   const double* E;       // [G0] or nullptr
   double* partials;      // [G0][N1*tiles_v] density partials of the output (want_partials)
+  double* push_r_ptr;    // the same plane as m_pushR, for tiles whose last row block is not 128-byte aligned in shared memory
   double Jx, Ju, Jv, omega_c;
   double wscale;         // 1/(J_u J_v): quadrature weight of node (b_u, b_v) = wref[b_u] wref[b_v] wscale
   double c0, c1, dt;     // out = c0*fn + c1*(f + dt*rhs)  (mode 1);  out = rhs (mode 0)
-  int N0, N1, N2, G0, G1, G2;
+  int N2, G0, G1, G2;    // N0 = gridDim.z, N1 = gridDim.y, tiles along v = gridDim.x
   int bc0, bc1, bc2;
-  int tiles_v, mode, has_fn, want_partials;
-  double* push_r_ptr;    // the same plane as m_pushR, for tiles whose last row block is not 128-byte aligned in shared memory
+  int mode, has_fn, want_partials;
   int push_l, push_r;    // x-slab face push (dg_set_xhalo_push): store the boundary planes of out into the neighbours' halos
-  int strong;            // 1: strong form Eq. 15 -- pe/qo are built from -D and the lift acts on (upwind state - own face value)
 };
 
 template <int NN, int KV>
@@ -116,6 +114,12 @@ struct TileCfg {
   __host__ __device__ static constexpr int idx(int row, int c) {
     return SWZ ? ((c >> 4) * (ROWS * 16) + row * 16 + (((((c & 15) >> 1) ^ (row & 7))) << 1) + (c & 1)) : (row * R + c);
   }
+  // phase v: byte offset of the first 16-byte chunk of the line (row, columns cl .. cl+NN-1), and of its chunk q = k/2.
+  // Swizzled tiles: cl is a multiple of NN, so the chunk index of column cl + 2q is that of cl with q XORed in.
+  __device__ static __forceinline__ uint32_t vline(int row, int cl) {
+    return SWZ ? (uint32_t)((cl >> 4) * (ROWS * 128) + row * 128 + ((((cl & 15) >> 1) ^ (row & 7)) << 4)) : (uint32_t)((row * R + cl) * 8);
+  }
+  __device__ static __forceinline__ uint32_t vchunk(uint32_t line, int q) { return SWZ ? (line ^ (uint32_t)(q << 4)) : (line + (uint32_t)(q << 4)); }
   static constexpr int SZ_FACE = a1k(NN * R * 8);
   static constexpr int SZ_V = a1k(NN * NN * 2 * 8);
   static constexpr int OFF_F = 0;
@@ -127,15 +131,16 @@ struct TileCfg {
   static constexpr int OFF_VL = OFF_UR + SZ_FACE;
   static constexpr int OFF_VR = OFF_VL + SZ_V;
   static constexpr int OFF_RED = OFF_VR + SZ_V;
-  static constexpr int OFF_BAR = OFF_RED + a1k(NT * 8);
+  static constexpr int OFF_BAR = OFF_RED + (SHFL_RED ? 0 : a1k(NT * 8));
   static constexpr int SMEM_BYTES = OFF_BAR + 128;
 };
 
 // Two lines at once (the operator coefficients are fetched once for both):
 // s[l][j] = (Ups f_l - Xi_R uR_l + Xi_L uL_l)_j, reference element (Eq. 14 / 20 / 21).
-// PT: any parameter block with members pe, qo, la, lb, strong (TiledParams here, LineParams of the 2D2V line kernel).
+// PT: any parameter block with members pe, qo, la, lb (TiledParams here, LineParams of the 2D2V line kernel).
+// strong: Eq. 15 -- pe/qo are built from -D and the lift acts on (upwind state - own face value).
 template <int NN, class PT>
-__device__ __forceinline__ void apply_lines2(const PT& P, const double (&f)[2][NN], const double (&uL)[2],
+__device__ __forceinline__ void apply_lines2(const PT& P, const bool strong, const double (&f)[2][NN], const double (&uL)[2],
                                              const double (&uR)[2], double (&s)[2][NN]) {
   constexpr int H = NN / 2;
   double e[2][H], o[2][H], sp[2], dm[2];
@@ -146,7 +151,7 @@ __device__ __forceinline__ void apply_lines2(const PT& P, const double (&f)[2][N
     sp[l] = uL[l] + uR[l];
     dm[l] = uL[l] - uR[l];
     // strong form (Eq. 15): (uL - f_0) +- (uR - f_{n-1})
-    if (P.strong) { sp[l] -= e[l][0]; dm[l] -= o[l][0]; }
+    if (strong) { sp[l] -= e[l][0]; dm[l] -= o[l][0]; }
   }
 #pragma unroll
   for (int j = 0; j < H; ++j) {
@@ -171,36 +176,38 @@ __device__ __forceinline__ void apply_lines2(const PT& P, const double (&f)[2][N
 // ------------------------------------------------------------------------------------------------
 // resident CTAs per SM the register allocation must allow: set for n = 10 only (134 -> 128 registers: 4 CTAs instead of 3);
 // the other orders reach the shared-memory limit with the default allocation (0 = unspecified)
-// (n = 8 must NOT be given a minimum: ptxas reaches 96 registers, five CTAs, without spills on its own, and spills 44 bytes per
-// thread when asked for five -- measured 1.51 -> 1.65 ms per step at 512^3)
 __host__ __device__ constexpr int tiled_min_ctas(int n) { return n == 10 ? 4 : 0; }   // 0: unspecified
 
+// Upwind side of a line from the sign of its speed (Eq. 23): bit 0 = a > 0 (the left neighbour's face state enters at the
+// left face), bit 1 = a < 0 (the right neighbour's at the right face); a = 0: neither (zero flux, reading C12).  The speeds
+// the threads hold carry the factor cr = c1 dt; `flip` (cr < 0) swaps the bits so that they describe a itself.
+__device__ __forceinline__ int upwind_bits(double a_scaled, bool flip) {
+  const int p = a_scaled > 0.0 ? 1 : 0, n = a_scaled < 0.0 ? 1 : 0;
+  return flip ? (n | (p << 1)) : (p | (n << 1));
+}
+
 // has_fn: the stage combination reads f_n (stages 2, 3 of SSP-RK3: c0 != 0); without it (dg_rhs, stage 1) the f_n tile is
-// neither loaded nor read and the accumulator tile starts from the x-phase result.  (A compile-time flag instead of this
-// CTA-uniform branch costs 6 registers at n = 8 -- 102 instead of 96, four CTAs per SM instead of five: measured, dropped.)
-template <int NN, int KV>
+// neither loaded nor read and the accumulator tile starts from the x-phase result (a CTA-uniform branch).
+// Grid = (tiles along v, N1, N0): v fastest, then u, then x -- neighbouring CTAs share halos through L2.
+template <int NN, int KV, bool STRONG>
 __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tiled_kernel(const __grid_constant__ TiledParams<NN> P) {
   const bool FN = P.has_fn != 0;
   using Cfg = TileCfg<NN, KV>;
   constexpr int R = Cfg::R, H = Cfg::H, RP = R / 2;
   extern __shared__ __align__(1024) unsigned char smem[];
   double* sF = reinterpret_cast<double*>(smem + Cfg::OFF_F);    // stage input tile
-  double* sN = reinterpret_cast<double*>(smem + Cfg::OFF_N);    // f_n tile -> accumulator -> output tile
+  double* sN = reinterpret_cast<double*>(smem + Cfg::OFF_N);    // f_n tile -> running sum -> output tile
   double* sXL = reinterpret_cast<double*>(smem + Cfg::OFF_XL);
   double* sXR = reinterpret_cast<double*>(smem + Cfg::OFF_XR);
   double* sUL = reinterpret_cast<double*>(smem + Cfg::OFF_UL);
   double* sUR = reinterpret_cast<double*>(smem + Cfg::OFF_UR);
   double* sVL = reinterpret_cast<double*>(smem + Cfg::OFF_VL);
   double* sVR = reinterpret_cast<double*>(smem + Cfg::OFF_VR);
-  double* sRed = reinterpret_cast<double*>(smem + Cfg::OFF_RED);
   const uint32_t bar = smem_u32(smem + Cfg::OFF_BAR);
 
   const int t = threadIdx.x;
-  // tile coordinates: v fastest, then u, then x (neighbouring CTAs share halos through L2)
-  int bid = blockIdx.x;
-  const int tv = bid % P.tiles_v; bid /= P.tiles_v;
-  const int eu = bid % P.N1;
-  const int ex = bid / P.N1;
+  const int tv = blockIdx.x, eu = blockIdx.y, ex = blockIdx.z;
+  const int N1 = gridDim.y, N0 = gridDim.z, tiles_v = gridDim.x;
   const int ev0 = tv * KV;
   const int kvalid = min(KV, P.N2 - ev0);             // v-elements of this tile inside the grid
   const int gx0 = ex * NN, gu0 = eu * NN, c0 = ev0 * NN;
@@ -215,11 +222,7 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   // RK stage: cf = c1, cr = c1*dt.  None of this reads what the previous kernel in the stream wrote.
   const double cf = (P.mode != 0) ? P.c1 : 0.0;
   const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
-  // The speeds below carry the factor cr; the upwind side of Eq. 23 is decided by the sign of the speed itself, so a
-  // negative cr (c1 dt < 0) swaps the comparisons (the generic kernel and thread 0's halo choice use the unscaled a_d).
   const bool flip = cr < 0.0;
-  auto is_pos = [flip](double a) { return flip ? a < 0.0 : a > 0.0; };
-  auto is_neg = [flip](double a) { return flip ? a > 0.0 : a < 0.0; };
   const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
   // phase v: rows ju and ju + H of (jx, ev).  Swizzled tiles: ju fastest (the XOR spreads the rows over the banks);
   // plain row-major tiles (R != 32): ev fastest -- a row is R/2 16-byte units and an element n/2 of them, and
@@ -238,8 +241,8 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
   if (t == 0) {
-    // The tile itself (and f_n) first: their byte count is known, so the transaction count is raised without
-    // arriving, and the loads are in flight while the halo decision below fetches the speeds.
+    // the tile itself (and f_n): their byte count is known, so the transaction count is raised without arriving and the
+    // loads are in flight while the threads work out which halos the signs of their speeds need
     mbar_expect_tx_noarrive(bar, (FN ? 2u : 1u) * (NN * NN * R * 8));
     tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
     if (Cfg::SWZ) tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
@@ -247,19 +250,28 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
       tma_load_3d(smem_u32(sN), &P.m_fn, bar, c0, gu0, gx0);
       if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
     }
-    // which upwind halos can be needed at all (signs of the speeds over the tile, Eq. 28)
-    const double vx_lo = P.vx[gu0], vx_hi = P.vx[gu0 + NN - 1];
-    const bool ax_pos = vx_hi > 0.0, ax_neg = vx_lo < 0.0;
-    const double w_lo = P.omega_c * vx_lo, w_hi = P.omega_c * vx_hi;
-    const bool av_pos = fmax(w_lo, w_hi) > 0.0, av_neg = fmin(w_lo, w_hi) < 0.0;
-    double e_min = 0.0, e_max = 0.0;
-    if (P.E) {
-      e_min = e_max = P.E[gx0];
-      for (int j = 1; j < NN; ++j) { const double e = P.E[gx0 + j]; e_min = fmin(e_min, e); e_max = fmax(e_max, e); }
-    }
-    const double y_lo = -P.omega_c * P.vy[c0], y_hi = -P.omega_c * P.vy[c0 + kvalid * NN - 1];
-    const bool au_pos = (-e_min + fmax(y_lo, y_hi)) > 0.0, au_neg = (-e_max + fmin(y_lo, y_hi)) < 0.0;
-
+  }
+  // a_u = -E - omega_c v  (E = -Phi', reading C15)
+  const double Ex = P.E ? P.E[gx0 + xu_hi] : 0.0;
+#pragma unroll
+  for (int l = 0; l < 2; ++l) au[l] = cr * P.Ju * (-Ex - au[l]);
+  // upwind sides of this thread's lines: bits 0-1 x, 2-3 / 4-5 u (lines 0, 1), 6-7 / 8-9 v (lines 0, 1)
+  const int um = upwind_bits(ax, flip) | (upwind_bits(au[0], flip) << 2) | (upwind_bits(au[1], flip) << 4) |
+                 (upwind_bits(av[0], flip) << 6) | (upwind_bits(av[1], flip) << 8);
+  // The threads' lines cover the tile in every phase, so the OR over the CTA says exactly which face halos are read at
+  // all; the barrier also makes the mbarrier initialisation visible to the waiters.
+  int* sAny = reinterpret_cast<int*>(smem + Cfg::OFF_BAR + 64);      // one word per warp
+  {
+    const int w_or = __reduce_or_sync(__activemask(), um);      // NT need not be a multiple of 32
+    if ((t & 31) == 0) sAny[t >> 5] = w_or;
+  }
+  __syncthreads();
+  if (t == 0) {
+    int any = 0;
+#pragma unroll
+    for (int w = 0; w < (Cfg::NT + 31) / 32; ++w) any |= sAny[w];
+    const bool ax_pos = any & 1, ax_neg = any & 2, au_pos = any & (4 | 16), au_neg = any & (8 | 32);
+    const bool av_pos = any & (64 | 256), av_neg = any & (128 | 512);
     uint32_t bytes = 0;
     if (ax_pos) bytes += NN * R * 8;
     if (ax_neg) bytes += NN * R * 8;
@@ -276,23 +288,17 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
       else tma_load_3d(smem_u32(sXL), &P.m_xface, bar, c0, gu0, (ex > 0) ? gx0 - 1 : (P.bc0 == 0 ? P.G0 - 1 : -1));
     }
     if (ax_neg) {
-      if (P.bc0 == 2 && ex == P.N0 - 1) tma_load_3d(smem_u32(sXR), &P.m_xhalo, bar, c0, gu0, 1);
-      else tma_load_3d(smem_u32(sXR), &P.m_xface, bar, c0, gu0, (ex < P.N0 - 1) ? gx0 + NN : (P.bc0 == 0 ? 0 : P.G0));
+      if (P.bc0 == 2 && ex == N0 - 1) tma_load_3d(smem_u32(sXR), &P.m_xhalo, bar, c0, gu0, 1);
+      else tma_load_3d(smem_u32(sXR), &P.m_xface, bar, c0, gu0, (ex < N0 - 1) ? gx0 + NN : (P.bc0 == 0 ? 0 : P.G0));
     }
     if (au_pos) tma_load_3d(smem_u32(sUL), &P.m_uface, bar, c0, (eu > 0) ? gu0 - 1 : (P.bc1 == 0 ? P.G1 - 1 : -1), gx0);
-    if (au_neg) tma_load_3d(smem_u32(sUR), &P.m_uface, bar, c0, (eu < P.N1 - 1) ? gu0 + NN : (P.bc1 == 0 ? 0 : P.G1), gx0);
+    if (au_neg) tma_load_3d(smem_u32(sUR), &P.m_uface, bar, c0, (eu < N1 - 1) ? gu0 + NN : (P.bc1 == 0 ? 0 : P.G1), gx0);
     if (av_pos) tma_load_3d(smem_u32(sVL), &P.m_vface, bar, (ev0 > 0) ? c0 - 2 : (P.bc2 == 0 ? P.G2 - 2 : -2), gu0, gx0);
     if (av_neg) {
       const int cend = c0 + kvalid * NN;
       tma_load_3d(smem_u32(sVR), &P.m_vface, bar, (cend < P.G2) ? cend : (P.bc2 == 0 ? 0 : P.G2), gu0, gx0);
     }
   }
-  // a_u = -E - omega_c v  (E = -Phi', reading C15), fetched while the TMA loads are in flight
-  const double Ex = P.E ? P.E[gx0 + xu_hi] : 0.0;
-#pragma unroll
-  for (int l = 0; l < 2; ++l) au[l] = cr * P.Ju * (-Ex - au[l]);
-
-  __syncthreads();           // barrier init visible to all waiters
   mbar_wait(bar, 0);
 
   // ---------------- phase x: thread = (ju, c..c+1), lines over jx ----------------
@@ -305,11 +311,11 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
       f[0][k] = v.x; f[1][k] = v.y;
     }
     // upwind states, Eq. 23
-    if (is_pos(ax)) { const double2 v = *reinterpret_cast<const double2*>(&sXL[ju * R + c]); uL[0] = v.x; uL[1] = v.y; }
+    if (um & 1) { const double2 v = *reinterpret_cast<const double2*>(&sXL[ju * R + c]); uL[0] = v.x; uL[1] = v.y; }
     else { uL[0] = f[0][0]; uL[1] = f[1][0]; }
-    if (is_neg(ax)) { const double2 v = *reinterpret_cast<const double2*>(&sXR[ju * R + c]); uR[0] = v.x; uR[1] = v.y; }
+    if (um & 2) { const double2 v = *reinterpret_cast<const double2*>(&sXR[ju * R + c]); uR[0] = v.x; uR[1] = v.y; }
     else { uR[0] = f[0][NN - 1]; uR[1] = f[1][NN - 1]; }
-    apply_lines2<NN>(P, f, uL, uR, s);
+    apply_lines2<NN>(P, STRONG, f, uL, uR, s);
     if (FN) {
 #pragma unroll
       for (int j = 0; j < NN; ++j) {
@@ -333,13 +339,18 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
       const double2 v = *reinterpret_cast<const double2*>(&sF[Cfg::idx(jx * NN + k, c)]);
       f[0][k] = v.x; f[1][k] = v.y;
     }
-    const double2 hl = *reinterpret_cast<const double2*>(&sUL[jx * R + c]);
-    const double2 hr = *reinterpret_cast<const double2*>(&sUR[jx * R + c]);
-    uL[0] = is_pos(au[0]) ? hl.x : f[0][0];
-    uL[1] = is_pos(au[1]) ? hl.y : f[1][0];
-    uR[0] = is_neg(au[0]) ? hr.x : f[0][NN - 1];
-    uR[1] = is_neg(au[1]) ? hr.y : f[1][NN - 1];
-    apply_lines2<NN>(P, f, uL, uR, s);
+    uL[0] = f[0][0]; uL[1] = f[1][0]; uR[0] = f[0][NN - 1]; uR[1] = f[1][NN - 1];
+    if (um & (4 | 16)) {
+      const double2 hl = *reinterpret_cast<const double2*>(&sUL[jx * R + c]);
+      if (um & 4) uL[0] = hl.x;
+      if (um & 16) uL[1] = hl.y;
+    }
+    if (um & (8 | 32)) {
+      const double2 hr = *reinterpret_cast<const double2*>(&sUR[jx * R + c]);
+      if (um & 8) uR[0] = hr.x;
+      if (um & 32) uR[1] = hr.y;
+    }
+    apply_lines2<NN>(P, STRONG, f, uL, uR, s);
 #pragma unroll
     for (int j = 0; j < NN; ++j) {
       double2* q = reinterpret_cast<double2*>(&sN[Cfg::idx(jx * NN + j, c)]);
@@ -356,29 +367,31 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
     if (ev < kvalid) {
       const int cl = ev * NN;
       double f[2][NN], s[2][NN], acc[2][NN], uL[2], uR[2];
+      uint32_t line[2];
 #pragma unroll
       for (int l = 0; l < 2; ++l) {
         const int row = jx * NN + v_ju + l * H;
+        line[l] = Cfg::vline(row, cl);
 #pragma unroll
         for (int k = 0; k < NN; k += 2) {
-          const double2 v2 = *reinterpret_cast<const double2*>(&sF[Cfg::idx(row, cl + k)]);
+          const uint32_t o = Cfg::vchunk(line[l], k >> 1);
+          const double2 v2 = *reinterpret_cast<const double2*>(smem + Cfg::OFF_F + o);
           f[l][k] = v2.x; f[l][k + 1] = v2.y;
-          const double2 a2 = *reinterpret_cast<const double2*>(&sN[Cfg::idx(row, cl + k)]);
+          const double2 a2 = *reinterpret_cast<const double2*>(smem + Cfg::OFF_N + o);
           acc[l][k] = a2.x; acc[l][k + 1] = a2.y;
         }
         uL[l] = f[l][0]; uR[l] = f[l][NN - 1];
-        if (is_pos(av[l])) uL[l] = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
-        if (is_neg(av[l])) uR[l] = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
+        if (um & (64 << (2 * l))) uL[l] = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
+        if (um & (128 << (2 * l))) uR[l] = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
       }
-      apply_lines2<NN>(P, f, uL, uR, s);
+      apply_lines2<NN>(P, STRONG, f, uL, uR, s);
 #pragma unroll
       for (int l = 0; l < 2; ++l) {
-        const int row = jx * NN + v_ju + l * H;
 #pragma unroll
         for (int j = 0; j < NN; ++j) acc[l][j] = fma(cf, f[l][j], fma(av[l], s[l][j], acc[l][j]));
 #pragma unroll
         for (int k = 0; k < NN; k += 2)
-          *reinterpret_cast<double2*>(&sN[Cfg::idx(row, cl + k)]) = make_double2(acc[l][k], acc[l][k + 1]);
+          *reinterpret_cast<double2*>(smem + Cfg::OFF_N + Cfg::vchunk(line[l], k >> 1)) = make_double2(acc[l][k], acc[l][k + 1]);
       }
       if (P.want_partials) {
         // Eq. 27: LGL quadrature of the stage output over this thread's two v lines
@@ -393,9 +406,9 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
         // the H*KV = 16 threads of x node jx are one aligned half-warp: fixed butterfly, deterministic
 #pragma unroll
         for (int off = 8; off > 0; off >>= 1) psum += __shfl_xor_sync(0xffffffffu, psum, off);
-        if ((t & 15) == 0) P.partials[(size_t)(gx0 + v_jx) * (P.N1 * P.tiles_v) + (eu * P.tiles_v + tv)] = psum;
+        if ((t & 15) == 0) P.partials[(size_t)(gx0 + v_jx) * (N1 * tiles_v) + (eu * tiles_v + tv)] = psum;
       } else {
-        sRed[t] = psum;
+        reinterpret_cast<double*>(smem + Cfg::OFF_RED)[t] = psum;
       }
     }
   }
@@ -403,7 +416,7 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   __syncthreads();
   constexpr int ROFF = (NN - 1) * NN * (Cfg::SWZ ? 16 : R);          // last x-node row block of the tile
   constexpr bool PUSHR_TMA = (ROFF * 8) % 128 == 0;                  // a TMA store needs a 128-byte aligned source
-  if (!PUSHR_TMA && P.push_r && ex == P.N0 - 1) {
+  if (!PUSHR_TMA && P.push_r && ex == N0 - 1) {
     // n = 10 (R = 20): the block starts at 14 400 B; the NN x R doubles leave by plain stores instead
     for (int i = t; i < NN * R; i += Cfg::NT) {
       const int row = i / R, c = i - row * R;
@@ -420,7 +433,7 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
       tma_store_3d(&P.m_pushL, smem_u32(sN), c0, gu0, 0);
       if (Cfg::SWZ) tma_store_3d(&P.m_pushL, smem_u32(sN + Cfg::ROWS * 16), c0 + 16, gu0, 0);
     }
-    if (PUSHR_TMA && P.push_r && ex == P.N0 - 1) {
+    if (PUSHR_TMA && P.push_r && ex == N0 - 1) {
       tma_store_3d(&P.m_pushR, smem_u32(sN + ROFF), c0, gu0, 0);
       if (Cfg::SWZ) tma_store_3d(&P.m_pushR, smem_u32(sN + Cfg::ROWS * 16 + ROFF), c0 + 16, gu0, 0);
     }
@@ -428,10 +441,11 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   }
   if (!Cfg::SHFL_RED && P.want_partials && t >= 32 && t < 32 + NN) {
     // fixed-order sum over the (ev, ju) threads of x node jx: deterministic
+    const double* sRed = reinterpret_cast<const double*>(smem + Cfg::OFF_RED);
     const int jx = t - 32;
     double sum = 0.0;
     for (int i = 0; i < H * KV; ++i) sum += sRed[jx * H * KV + i];
-    P.partials[(size_t)(gx0 + jx) * (P.N1 * P.tiles_v) + (eu * P.tiles_v + tv)] = sum;
+    P.partials[(size_t)(gx0 + jx) * (N1 * tiles_v) + (eu * tiles_v + tv)] = sum;
   }
 }
 
@@ -492,7 +506,7 @@ inline bool make_map(CUtensorMap* m, const void* base, dg_ctx* ctx, int b0, int 
   return true;
 }
 
-template <int NN, int KV>
+template <int NN, int KV, bool STRONG>
 int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
                        double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
   using Cfg = TileCfg<NN, KV>;
@@ -501,8 +515,7 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   if (((uintptr_t)f & 15) || ((uintptr_t)out & 15) || (fn && ((uintptr_t)fn & 15))) { g_tiled_err = "arrays must be 16-byte aligned"; return DG_ERR_INVALID_ARG; }
   const int RB = Cfg::SWZ ? 16 : R;      // swizzled tiles move as two 128-byte-wide boxes
   if (!make_map(&P.m_main, f, ctx, RB, NN, NN, Cfg::SWZ) || !make_map(&P.m_xface, f, ctx, R, NN, 1) ||
-      !make_map(&P.m_uface, f, ctx, R, 1, NN) || !make_map(&P.m_vface, f, ctx, 2, NN, NN) ||
-      !make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ))
+      !make_map(&P.m_uface, f, ctx, R, 1, NN) || !make_map(&P.m_vface, f, ctx, 2, NN, NN))
     return DG_ERR_CUDA;
   const bool has_fn = (mode != 0 && fn != nullptr);
   if (has_fn) { if (!make_map(&P.m_fn, fn, ctx, RB, NN, NN, Cfg::SWZ)) return DG_ERR_CUDA; }
@@ -513,6 +526,7 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   } else {
     P.m_xhalo = P.m_xface;
   }
+  if (!make_map(&P.m_out, out, ctx, RB, NN, NN, Cfg::SWZ)) return DG_ERR_CUDA;
   P.push_l = (mode != 0 && ctx->push_left) ? 1 : 0;
   P.push_r = (mode != 0 && ctx->push_right) ? 1 : 0;
   P.m_pushL = P.m_out; P.m_pushR = P.m_out; P.push_r_ptr = ctx->push_right;
@@ -520,9 +534,8 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   if (P.push_r && !make_map(&P.m_pushR, ctx->push_right, ctx, RB, NN, 1, Cfg::SWZ, 1)) return DG_ERR_CUDA;
   const dgsetup::Basis1D& b = ctx->basis[0];
   constexpr int H = NN / 2;
-  P.strong = ctx->opt_form;
   // volume operator: Upsilon (weak form, Eq. 14) or -D (strong form, Eq. 15); both are centro-antisymmetric
-  auto vol = [&](int j, int k) { return ctx->opt_form ? -b.dmat[j * NN + k] : b.ups[j * NN + k]; };
+  auto vol = [&](int j, int k) { return STRONG ? -b.dmat[j * NN + k] : b.ups[j * NN + k]; };
   for (int j = 0; j < H; ++j) {
     for (int k = 0; k < H; ++k) {
       P.pe[j * H + k] = 0.5 * (vol(j, k) + vol(j, NN - 1 - k));
@@ -537,43 +550,50 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   P.Jx = ctx->J[0]; P.Ju = ctx->J[1]; P.Jv = ctx->J[2]; P.omega_c = ctx->desc.omega_c;
   P.wscale = 1.0 / (ctx->J[1] * ctx->J[2]);
   P.c0 = c0; P.c1 = c1; P.dt = dt;
-  P.N0 = ctx->N[0]; P.N1 = ctx->N[1]; P.N2 = ctx->N[2]; P.G0 = ctx->G[0]; P.G1 = ctx->G[1]; P.G2 = ctx->G[2];
+  P.N2 = ctx->N[2]; P.G0 = ctx->G[0]; P.G1 = ctx->G[1]; P.G2 = ctx->G[2];
   P.bc0 = ctx->desc.bc[0]; P.bc1 = ctx->desc.bc[1]; P.bc2 = ctx->desc.bc[2];
-  P.tiles_v = (ctx->N[2] + KV - 1) / KV;
+  const int tiles_v = (ctx->N[2] + KV - 1) / KV;
   P.mode = mode; P.has_fn = has_fn ? 1 : 0;
-  const size_t chunks = (size_t)P.N1 * P.tiles_v;
+  const size_t chunks = (size_t)ctx->N[1] * tiles_v;
   P.want_partials = (want_partials && ctx->partials && chunks * ctx->G[0] <= ctx->partials_doubles) ? 1 : 0;
   if (partial_chunks) *partial_chunks = P.want_partials ? (int)chunks : 0;
 
   // DG_OPT_SMEM_PAD_KB: unused extra shared memory per CTA, to lower the number of resident CTAs (occupancy sweeps)
   const size_t smem_bytes = (size_t)Cfg::SMEM_BYTES + (size_t)ctx->opt_smem_pad_kb * 1024;
   {
-    cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(rhs_tiled_kernel<NN, KV>), smem_bytes);
+    cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(rhs_tiled_kernel<NN, KV, STRONG>), smem_bytes);
     if (e != cudaSuccess) { g_tiled_err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return DG_ERR_CUDA; }
   }
-  const long long tiles = (long long)P.N0 * P.N1 * P.tiles_v;
-  if (tiles > 0x7fffffffLL) { g_tiled_err = "too many tiles"; return DG_ERR_UNSUPPORTED; }
+  if (ctx->N[1] > 65535 || ctx->N[0] > 65535) { g_tiled_err = "more than 65535 elements along x or v_x"; return DG_ERR_UNSUPPORTED; }
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)tiles); cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = smem_bytes; cfg.stream = st;
+  cfg.gridDim = dim3((unsigned)tiles_v, (unsigned)ctx->N[1], (unsigned)ctx->N[0]);
+  cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = smem_bytes; cfg.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   // DG_OPT_PROFILE = 1 (every launch bracketed by events) measures the kernel alone, without programmatic launches
   cfg.attrs = at; cfg.numAttrs = (ctx->opt_pdl && ctx->opt_profile != 1) ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, rhs_tiled_kernel<NN, KV>, P);
+  cudaLaunchKernelEx(&cfg, rhs_tiled_kernel<NN, KV, STRONG>, P);
   ctx->last_kernel = "rhs_tiled<" + std::to_string(NN) + "," + std::to_string(KV) + ">";
   return DG_OK;
 }
 
-inline int launch_rhs_tiled(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
-                            double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
+template <bool STRONG>
+inline int launch_rhs_tiled_f(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
+                              double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
   switch (ctx->n[0]) {
-    case 4: return launch_rhs_tiled_t<4, 8>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-    case 6: return launch_rhs_tiled_t<6, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-    case 8: return launch_rhs_tiled_t<8, 4>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
-    case 10: return launch_rhs_tiled_t<10, 2>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 4: return launch_rhs_tiled_t<4, 8, STRONG>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 6: return launch_rhs_tiled_t<6, 4, STRONG>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 8: return launch_rhs_tiled_t<8, 4, STRONG>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
+    case 10: return launch_rhs_tiled_t<10, 2, STRONG>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
     default: g_tiled_err = "order not supported by the tiled kernel"; return DG_ERR_UNSUPPORTED;
   }
+}
+
+inline int launch_rhs_tiled(dg_ctx* ctx, const double* f, const double* fn, const double* E, double* out, int mode,
+                            double c0, double c1, double dt, bool want_partials, int* partial_chunks, cudaStream_t st) {
+  return ctx->opt_form ? launch_rhs_tiled_f<true>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st)
+                       : launch_rhs_tiled_f<false>(ctx, f, fn, E, out, mode, c0, c1, dt, want_partials, partial_chunks, st);
 }
 
 }  // namespace dgt
