@@ -217,32 +217,13 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
     mbar_init(bar, 1);
     fence_mbar_init();
   }
-  // Thread <-> line maps of the three phases and the E-independent speeds (Eq. 28), scaled by the Jacobian
-  // J_d = 2/Delta_d (Eq. 61) and by cr.  out = c0*fn + cf*f + cr*rhs:  plain RHS (mode 0): cf = 0, cr = 1;
-  // RK stage: cf = c1, cr = c1*dt.  None of this reads what the previous kernel in the stream wrote.
-  const double cf = (P.mode != 0) ? P.c1 : 0.0;
-  const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
-  const bool flip = cr < 0.0;
-  const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
-  // phase v: rows ju and ju + H of (jx, ev).  Swizzled tiles: ju fastest (the XOR spreads the rows over the banks);
-  // plain row-major tiles (R != 32): ev fastest -- a row is R/2 16-byte units and an element n/2 of them, and
-  // (n/2) ev + (R/2) ju hits 8 different bank groups over 8 lanes for (n, KV) = (6, 4), (10, 2), (10, 3)
-  const int v_ju = Cfg::SWZ ? t % H : (t / KV) % H, v_ev = Cfg::SWZ ? (t / H) % KV : t % KV, v_jx = t / (KV * H);
-  const double ax = cr * P.Jx * P.vx[gu0 + xu_hi];                                         // a_x = u
-  double au[2], av[2];
-#pragma unroll
-  for (int l = 0; l < 2; ++l) {
-    au[l] = P.omega_c * P.vy[min(c0 + xu_c + l, P.G2 - 1)];
-    av[l] = cr * P.Jv * (P.omega_c * P.vx[gu0 + v_ju + l * H]);                            // a_v = omega_c u
-  }
   // Programmatic dependent launch: let the next kernel of the stream start its prologue, then wait until the
   // previous kernel (the field solve that wrote E, and through it the stage that wrote f_s) has completed.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
-
   if (t == 0) {
-    // the tile itself (and f_n): their byte count is known, so the transaction count is raised without arriving and the
-    // loads are in flight while the threads work out which halos the signs of their speeds need
+    // The tile itself (and f_n) first: their byte count is known, so the transaction count is raised without arriving and
+    // the loads are in flight while the threads fetch their speeds and work out which halos the signs need.
     mbar_expect_tx_noarrive(bar, (FN ? 2u : 1u) * (NN * NN * R * 8));
     tma_load_3d(smem_u32(sF), &P.m_main, bar, c0, gu0, gx0);
     if (Cfg::SWZ) tma_load_3d(smem_u32(sF + Cfg::ROWS * 16), &P.m_main, bar, c0 + 16, gu0, gx0);
@@ -251,10 +232,27 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
       if (Cfg::SWZ) tma_load_3d(smem_u32(sN + Cfg::ROWS * 16), &P.m_fn, bar, c0 + 16, gu0, gx0);
     }
   }
-  // a_u = -E - omega_c v  (E = -Phi', reading C15)
+  // Thread <-> line maps of the three phases and the speeds (Eq. 28), scaled by the Jacobian J_d = 2/Delta_d (Eq. 61)
+  // and by cr.  out = c0*fn + cf*f + cr*rhs:  plain RHS (mode 0): cf = 0, cr = 1;  RK stage: cf = c1, cr = c1*dt.
+  const double cf = (P.mode != 0) ? P.c1 : 0.0;
+  const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
+  const bool flip = cr < 0.0;
+  const int xu_hi = t / RP, xu_c = 2 * (t - xu_hi * RP);            // phase x: (ju, c, c+1);  phase u: (jx, c, c+1)
+  // phase v: rows ju and ju + H of (jx, ev).  Swizzled tiles: ju fastest (the XOR spreads the rows over the banks);
+  // plain row-major tiles (R != 32): ev fastest -- a row is R/2 16-byte units and an element n/2 of them, and
+  // (n/2) ev + (R/2) ju hits 8 different bank groups over 8 lanes for (n, KV) = (6, 4), (10, 2), (10, 3)
+  const int v_ju = Cfg::SWZ ? t % H : (t / KV) % H, v_ev = Cfg::SWZ ? (t / H) % KV : t % KV, v_jx = t / (KV * H);
+  // all global reads of the thread in one batch: a_x = u, a_u = -E - omega_c v (E = -Phi', reading C15), a_v = omega_c u
+  const double vx_x = P.vx[gu0 + xu_hi];
+  const double vy_0 = P.vy[min(c0 + xu_c, P.G2 - 1)], vy_1 = P.vy[min(c0 + xu_c + 1, P.G2 - 1)];
+  const double vx_0 = P.vx[gu0 + v_ju], vx_1 = P.vx[gu0 + v_ju + H];
   const double Ex = P.E ? P.E[gx0 + xu_hi] : 0.0;
-#pragma unroll
-  for (int l = 0; l < 2; ++l) au[l] = cr * P.Ju * (-Ex - au[l]);
+  const double ax = cr * P.Jx * vx_x;
+  double au[2], av[2];
+  au[0] = cr * P.Ju * (-Ex - P.omega_c * vy_0);
+  au[1] = cr * P.Ju * (-Ex - P.omega_c * vy_1);
+  av[0] = cr * P.Jv * (P.omega_c * vx_0);
+  av[1] = cr * P.Jv * (P.omega_c * vx_1);
   // upwind sides of this thread's lines: bits 0-1 x, 2-3 / 4-5 u (lines 0, 1), 6-7 / 8-9 v (lines 0, 1)
   const int um = upwind_bits(ax, flip) | (upwind_bits(au[0], flip) << 2) | (upwind_bits(au[1], flip) << 4) |
                  (upwind_bits(av[0], flip) << 6) | (upwind_bits(av[1], flip) << 8);
@@ -380,9 +378,12 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
           const double2 a2 = *reinterpret_cast<const double2*>(smem + Cfg::OFF_N + o);
           acc[l][k] = a2.x; acc[l][k + 1] = a2.y;
         }
-        uL[l] = f[l][0]; uR[l] = f[l][NN - 1];
-        if (um & (64 << (2 * l))) uL[l] = (ev > 0) ? sF[Cfg::idx(row, cl - 1)] : sVL[row * 2 + 1];
-        if (um & (128 << (2 * l))) uR[l] = (ev < kvalid - 1) ? sF[Cfg::idx(row, cl + NN)] : sVR[row * 2];
+        // upwind states (Eq. 23): the neighbour element's face node inside the tile, the halo at the tile's v edges; both
+        // candidates are fetched unconditionally (a halo that was not loaded is never selected)
+        const double hL = *((ev > 0) ? &sF[Cfg::idx(row, cl - 1)] : &sVL[row * 2 + 1]);
+        const double hR = *((ev < kvalid - 1) ? &sF[Cfg::idx(row, cl + NN)] : &sVR[row * 2]);
+        uL[l] = (um & (64 << (2 * l))) ? hL : f[l][0];
+        uR[l] = (um & (128 << (2 * l))) ? hR : f[l][NN - 1];
       }
       apply_lines2<NN>(P, STRONG, f, uL, uR, s);
 #pragma unroll
