@@ -1,6 +1,6 @@
 """End-to-end physics on the GPU path: the cyclotron-harmonic instability of the paper's Section 6.1 on a scaled grid.
 
-Simulation A (PAPER.md:479-483): ring distribution j = 6 (Eq. 31), omega_p/omega_c = 10 (B_ext = 0.1), perturbed by the
+Simulation A (PAPER.md:481-483): ring distribution j = 6 (Eq. 31), omega_p/omega_c = 10 (B_ext = 0.1), perturbed by the
 eigenmode of Eq. 35-36 at (k, omega) = (0.886 / r_L, 0.349i omega_c), domain length 2 pi / k, velocity box +-8.5.  Linear
 theory (Eq. 30 / 34) and Fig. 10a of the paper: the field energy grows as exp(2 * 0.349 omega_c t).  Here: (16, 32, 32)
 elements x 8^3 nodes instead of (25, 50, 50) (a few seconds of GPU time), self-consistent SSP-RK3 through dg_ssprk3_run,
@@ -46,7 +46,7 @@ def _run(k_larmor, omega, t_end, t_diag, nelem, amp=2e-4, sense=-1):
 
 
 def test_simulation_A_growth_rate():
-    """Purely growing mode: energy growth rate 2 * 0.349 omega_c (PAPER.md:248, Fig. 10a) from t = 0, within 2 %."""
+    """Purely growing mode: energy growth rate 2 * 0.349 omega_c (PAPER.md:251, Fig. 10a) from t = 0, within 2 %."""
     ts, W, dmass, wc = _run(0.886, 0.349j, 60.0, 2.0, (16, 32, 32))
     m = ts >= 10.0
     gamma = np.polyfit(ts[m], np.log(W[m]), 1)[0] / 2.0 / wc
@@ -65,7 +65,7 @@ def test_eq36_as_printed_is_the_other_handedness():
 
 
 def test_simulation_B_growth_rate_and_frequency():
-    """Mode with a real frequency (PAPER.md:479): (k, omega) = (1.4, 1.182 + 0.131i); field energy ~ exp(2 * 0.131 omega_c t)
+    """Mode with a real frequency (PAPER.md:481): (k, omega) = (1.4, 1.182 + 0.131i); field energy ~ exp(2 * 0.131 omega_c t)
     (Fig. 10b).  The energy of a travelling eigenmode grows without oscillating; tolerance 5 % (three-digit root, and
     the slower mode is contaminated longer by the stable harmonics the truncated series leaves behind)."""
     ts, W, dmass, wc = _run(1.4, 1.182 + 0.131j, 150.0, 5.0, (16, 32, 32))

@@ -210,3 +210,26 @@ def test_two_slab_emulation_steps_match_unsharded_oracle(push):
     assert relerr(got, fo) <= 1e-12
     for be in bes:
         be.close()
+
+
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two GPUs: the x-slab exchange over NCCL / peer memory has only been run on one device (DESIGN.md section 9)")
+@pytest.mark.parametrize("mode", ["sendrecv", "push"])
+def test_two_gpu_xslab_matches_unsharded_oracle(mode):
+    """World-size-2 run of the sharded step (one rank per GPU, torchrun): plain NCCL send/recv of the face planes, and
+    the fused push of the faces into the neighbours' symmetric-memory halo buffers; against the unsharded oracle."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(root, "tests", "_xslab_gpu_worker.py"), mode]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=root)
+    assert res.returncode == 0, res.stderr[-3000:]
+    out = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])
+    assert out["world"] == 2
+    for k, v in out.items():
+        if k.startswith("err_"):
+            assert v <= 1e-11, (k, v)
