@@ -26,7 +26,8 @@ typedef struct {
   int32_t order[4];    /* LGL nodes per element per dimension, 2..DG_MAX_ORDER (tiled kernel: all four equal to 4) */
   double  lo[4];
   double  hi[4];
-  int32_t bc[4];       /* 0 periodic, 1 zero-inflow; bc[0], bc[1] must be 0 when the Poisson solve is used */
+  int32_t bc[4];       /* 0 periodic, 1 zero-inflow; bc[0] may be DG_BC_HALO (an x-slab of a larger grid, dg4_set_xhalo);
+                          bc[0], bc[1] must be 0 for the self-consistent dg4_ssprk3_run (the Poisson solve is global) */
   double  omega_c;     /* B_ext of Eq. 28 */
   int32_t pmax[2];     /* Fourier modes kept: |p| <= pmax[0] in x, |q| <= pmax[1] in y; 0 -> N_x, N_y */
   int32_t mass_mode;   /* 0 exact LGL mass (Eq. 51/53/54), 1 lumped */
@@ -50,6 +51,16 @@ int dg4_rhs(dg4_ctx* ctx, const double* f_dev, const double* Ex_dev, const doubl
  * partials (tiled kernel and a workspace) or by a density pass. */
 int dg4_rk_stage(dg4_ctx* ctx, const double* f_s_dev, const double* f_n_dev, const double* Ex_dev, const double* Ey_dev,
                  double* out_dev, double c0, double c1, double dt, double* rho_out_dev, void* stream);
+
+/* x-slab sharding (SURVEY.md 8(e) carried to 2D2V; the contract of dg_set_xhalo): a context created with bc[0] = DG_BC_HALO
+ * is a slab of x-elements of a larger grid (y, u, v stay whole, so the density is local).  The upwind flux of Eq. 23
+ * at the slab's first / last x face reads the left neighbour's LAST x-node plane / the right neighbour's
+ * FIRST one from
+ *   halo_dev [in] [2][G_y][G_u][G_v]: plane 0 = exterior state below the slab, plane 1 = above it (zeros for zero inflow);
+ * device memory, 16-byte aligned, owned by the caller, read by every later dg4_rhs / dg4_rk_stage until replaced.
+ * DG_ERR_INVALID_ARG if the context is not a halo context or the pointer is null or misaligned; dg4_rhs / dg4_rk_stage on a
+ * halo context without a halo buffer fail the same way. */
+int dg4_set_xhalo(dg4_ctx* ctx, const double* halo_dev);
 
 /* rho[g_x][g_y] = sum_{g_u,g_v} (w_{b_u}/J_u)(w_{b_v}/J_v) f  (Eq. 27).  Deterministic.  Needs a workspace. */
 int dg4_density(dg4_ctx* ctx, const double* f_dev, double* rho_dev, void* stream);

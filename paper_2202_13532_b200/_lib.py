@@ -87,6 +87,7 @@ SIGNATURES = {
     "dg4_set_workspace": (C.c_int, [_vp, _vp, C.c_size_t]),
     "dg4_rhs": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "dg4_rk_stage": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _dbl, _vp, _vp]),
+    "dg4_set_xhalo": (C.c_int, [_vp, _vp]),
     "dg4_density": (C.c_int, [_vp, _vp, _vp, _vp]),
     "dg4_fourier_project": (C.c_int, [_vp, _vp, _vp, _vp]),
     "dg4_poisson_E": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),

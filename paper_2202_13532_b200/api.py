@@ -313,6 +313,11 @@ class DG4Context:
                                _ptr(rho_out), _stream(self.device)), "dg4_rk_stage")
         return out
 
+    def set_xhalo(self, halo):
+        """halo: [2][G_y][G_u][G_v] exterior x-face planes of an x-slab context (bc[0] = BC_HALO); kept alive here."""
+        self._xhalo = halo
+        _check(_L.dg4_set_xhalo(self._h, _ptr(halo)), "dg4_set_xhalo")
+
     def density(self, f, out=None):
         out = self._field() if out is None else out
         _check(_L.dg4_density(self._h, _ptr(f), _ptr(out), _stream(self.device)), "dg4_density")

@@ -33,6 +33,7 @@ struct dg4_ctx {
   int64_t prof_launches = 0;
   std::string last_kernel = "none";
   std::map<TmapKey, CUtensorMap> tmaps;   // TMA descriptors of the arrays seen so far (line kernel)
+  const double* xhalo = nullptr;          // caller-owned exterior x-face planes (bc[0] = DG_BC_HALO)
 };
 
 static int check4(dg4_ctx* ctx, const char* what) {
@@ -64,7 +65,8 @@ extern "C" int dg4_create(const dg4_grid_desc* desc, dg4_ctx** out) {
     if (desc->nelem[d] < 1) return fail(DG_ERR_INVALID_ARG, "dg4_create: nelem must be >= 1");
     if (desc->order[d] < 2 || desc->order[d] > DG_MAX_ORDER) return fail(DG_ERR_UNSUPPORTED, "dg4_create: order must be 2..10");
     if (!(desc->hi[d] > desc->lo[d])) return fail(DG_ERR_INVALID_ARG, "dg4_create: hi must exceed lo");
-    if (desc->bc[d] != 0 && desc->bc[d] != 1) return fail(DG_ERR_INVALID_ARG, "dg4_create: bc must be 0 or 1");
+    if (desc->bc[d] != 0 && desc->bc[d] != 1 && !(d == 0 && desc->bc[d] == DG_BC_HALO))
+      return fail(DG_ERR_INVALID_ARG, "dg4_create: bc must be 0 or 1 (bc[0] may be DG_BC_HALO)");
   }
   if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dg4_create: mass_mode must be 0 or 1");
   if (desc->pmax[0] < 0 || desc->pmax[1] < 0) return fail(DG_ERR_INVALID_ARG, "dg4_create: pmax must be >= 0");
@@ -209,13 +211,13 @@ extern "C" int dg4_set_workspace(dg4_ctx* ctx, void* ws_dev, size_t bytes) {
 // launches
 // ------------------------------------------------------------------------------------------------
 // 4-D TMA descriptor of an array f[G0][G1][G2][G3] with box (b0 = v, b1 = u, b2 = y, b3 = x); cached per (base, box).
-static bool make_map4(CUtensorMap* m, const void* base, dg4_ctx* ctx, int b0, int b1, int b2, int b3, bool swz64) {
-  const TmapKey key{base, b0, b1, b2 * 16 + b3, swz64 ? 2 : 0, 4};
+static bool make_map4(CUtensorMap* m, const void* base, dg4_ctx* ctx, int b0, int b1, int b2, int b3, bool swz64, int outer = 0) {
+  const TmapKey key{base, b0, b1, b2 * 16 + b3, swz64 ? 2 : 0, 4 + 16 * outer};
   auto it = ctx->tmaps.find(key);
   if (it != ctx->tmaps.end()) { *m = it->second; return true; }
   dgt::EncodeTiledFn enc = dgt::encode_fn();
   if (!enc) return false;
-  const cuuint64_t dims[4] = {(cuuint64_t)ctx->G[3], (cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)ctx->G[0]};
+  const cuuint64_t dims[4] = {(cuuint64_t)ctx->G[3], (cuuint64_t)ctx->G[2], (cuuint64_t)ctx->G[1], (cuuint64_t)(outer > 0 ? outer : ctx->G[0])};
   const cuuint64_t strides[3] = {(cuuint64_t)ctx->G[3] * 8, (cuuint64_t)ctx->G[3] * ctx->G[2] * 8,
                                  (cuuint64_t)ctx->G[3] * ctx->G[2] * ctx->G[1] * 8};
   const cuuint32_t box[4] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
@@ -245,6 +247,8 @@ static int launch_rhs4_line(dg4_ctx* ctx, const double* f, const double* fn, con
             make_map4(&P.m_uface, f, ctx, 8, 1, 8, 8, false) && make_map4(&P.m_vface, f, ctx, 2, 8, 8, 8, false);
   if (ok && with_fn) ok = make_map4(&P.m_fn, fn, ctx, 8, 8, 8, 8, true);
   else P.m_fn = P.m_main;
+  if (ok && ctx->desc.bc[0] == DG_BC_HALO) ok = make_map4(&P.m_xhalo, ctx->xhalo, ctx, 8, 8, 8, 1, false, 2);
+  else P.m_xhalo = P.m_xface;
   if (!ok) return fail(DG_ERR_CUDA, "dg4: cuTensorMapEncodeTiled failed");
   const dgsetup::Basis1D& b = ctx->basis[0];
   for (int j = 0; j < 4; ++j) {
@@ -287,8 +291,10 @@ static int launch_rhs4_line(dg4_ctx* ctx, const double* f, const double* fn, con
 static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, const double* Ex, const double* Ey, double* out,
                              int mode, double c0, double c1, double dt, bool want_partials, int* chunks_out, cudaStream_t st) {
   if (chunks_out) *chunks_out = 0;
+  if (ctx->desc.bc[0] == DG_BC_HALO && !ctx->xhalo) return fail(DG_ERR_INVALID_ARG, "dg4: bc[0] = DG_BC_HALO needs dg4_set_xhalo first");
   dg4::Params p;
   memset(&p, 0, sizeof(p));
+  p.xhalo = ctx->xhalo;
   for (int d = 0; d < 4; ++d) {
     p.N[d] = ctx->N[d]; p.n[d] = ctx->n[d]; p.G[d] = ctx->G[d]; p.bc[d] = ctx->desc.bc[d]; p.J[d] = ctx->J[d];
     p.coord[d] = ctx->d_coord[d]; p.ups[d] = ctx->d_ups[d]; p.lift[d] = ctx->d_lift[d];
@@ -319,6 +325,7 @@ static int launch_rhs4_inner(dg4_ctx* ctx, const double* f, const double* fn, co
       while (bxl < 3 && ctx->N[0] % (2 << bxl) == 0 && (double)ctx->N[2] * nvb * (2 << bxl) * tile_bytes <= 32e6) ++bxl;
     }
     p.bx_log2 = bxl;
+    p.wide_st = (((uintptr_t)out & 31) == 0) ? 1 : 0;      // rows are G_v = 4 N_v doubles: every element row starts on 32 bytes
     const dim3 tiles(nvb * (1 << bxl) * ctx->N[2], ctx->N[1], ctx->N[0] >> bxl);
     const bool with_fn = mode != 0 && fn != nullptr;
     const size_t smem = sizeof(double) * (kv == 8 ? dg4::tile_smem_doubles<8>(with_fn) : kv == 4 ? dg4::tile_smem_doubles<4>(with_fn)
@@ -471,6 +478,14 @@ extern "C" int dg4_rk_stage(dg4_ctx* ctx, const double* f_s_dev, const double* f
   if (rc || !rho_out_dev) return rc;
   if (chunks > 0) return launch_density4_finish(ctx, chunks, rho_out_dev, st);
   return dg4_density(ctx, out_dev, rho_out_dev, stream);
+}
+
+extern "C" int dg4_set_xhalo(dg4_ctx* ctx, const double* halo_dev) {
+  if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg4_set_xhalo: null context");
+  if (ctx->desc.bc[0] != DG_BC_HALO) return fail(DG_ERR_INVALID_ARG, "dg4_set_xhalo: the context was not created with bc[0] = DG_BC_HALO");
+  if (!halo_dev || ((uintptr_t)halo_dev & 15) != 0) return fail(DG_ERR_INVALID_ARG, "dg4_set_xhalo: pointer must be non-null and 16-byte aligned");
+  ctx->xhalo = halo_dev;
+  return DG_OK;
 }
 
 extern "C" int dg4_fourier_project(dg4_ctx* ctx, const double* rho_dev, double* c_dev, void* stream) {

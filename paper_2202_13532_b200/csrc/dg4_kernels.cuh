@@ -26,6 +26,8 @@ struct Params {
   double* partials;          // [G0*G1][chunks] per-tile density partials of out, or nullptr
   int chunks;
   int bx_log2;               // tiled kernel: log2 of the x-elements per rasterisation group
+  int wide_st;               // tiled kernel: out is 32-byte aligned (256-bit stores)
+  const double* xhalo;       // bc[0] = DG_BC_HALO: exterior x-face planes [2][G1][G2][G3] of an x-slab (dg4_set_xhalo)
   long long dof;
 };
 
@@ -57,10 +59,12 @@ __global__ void __launch_bounds__(256) rhs4_generic_kernel(const Params p) {
         uR = p.f[base + (long long)(n - 1) * strd[d]];
         if (e > 0) uL = p.f[base - strd[d]];
         else if (p.bc[d] == 0) uL = p.f[base + ((long long)(N - 1) * n + (n - 1)) * strd[d]];
+        else if (p.bc[d] == 2) uL = p.xhalo[idx - (long long)g[0] * strd[0]];                   // x-slab: the left neighbour's last plane
       } else if (a[d] < 0.0) {
         uL = p.f[base];
         if (e < N - 1) uR = p.f[base + (long long)n * strd[d]];
         else if (p.bc[d] == 0) uR = p.f[base - (long long)e * n * strd[d]];
+        else if (p.bc[d] == 2) uR = p.xhalo[strd[0] + idx - (long long)g[0] * strd[0]];         // the right neighbour's first plane
       }
       rhs += (p.J[d] * a[d]) * (vol - p.lift[d][2 * j + 1] * uR + p.lift[d][2 * j] * uL);
     }

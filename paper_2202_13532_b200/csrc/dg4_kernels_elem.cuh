@@ -127,7 +127,11 @@ __global__ void __launch_bounds__(n * n * n, (n == 8 ? 2 : (n == 6 ? 4 : 8))) rh
     const double a = p.coord[2][gu0 + c1];
     const int g = upwind_index(p, 0, ex, n, a);
     const long long node_off = elem_off + c2 * s1 + c1 * s2 + c0;          // + jx * s0
-    const double ext = g >= 0 ? __ldg(p.f + node_off - gx0 * s0 + g * s0) : 0.0;
+    double ext = g >= 0 ? __ldg(p.f + node_off - gx0 * s0 + g * s0) : 0.0;
+    if (p.bc[0] == 2) {        // x-slab: at the slab's two x faces the exterior state comes from the halo planes
+      if (a > 0.0 && ex == 0) ext = __ldg(p.xhalo + node_off - gx0 * s0);
+      else if (a < 0.0 && ex == p.N[0] - 1) ext = __ldg(p.xhalo + s0 + node_off - gx0 * s0);
+    }
     double fnv[n];
     if (use_fn) {
 #pragma unroll

@@ -64,6 +64,7 @@ struct alignas(64) LineParams {
   CUtensorMap m_yface;   // f_s, box (8, 8, 1, 8)
   CUtensorMap m_uface;   // f_s, box (8, 1, 8, 8)
   CUtensorMap m_vface;   // f_s, box (2, 8, 8, 8)
+  CUtensorMap m_xhalo;   // exterior x-face planes [2][G1][G2][G3] of an x-slab (bc[0] = 2), box (8, 8, 8, 1)
   double pe[NN * NN / 4], qo[NN * NN / 4], la[H], lb[H];   // even-odd operator, see dg_kernels_tiled.cuh
   double wref[NN];       // LGL weights on [-1, 1] (Eq. 45)
   const double* cu;      // node coordinates of u = v_x and v = v_y
@@ -153,8 +154,14 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
       // coordinate; zero inflow: outside the tensor, where TMA fills zeros (exterior state 0, reading C2)
       auto below = [&](int d, int e, int g0) { return e > 0 ? g0 - 1 : (P.bc[d] == 0 ? P.G[d] - 1 : -1); };
       auto above = [&](int d, int e, int g0) { return e < P.N[d] - 1 ? g0 + NN : (P.bc[d] == 0 ? 0 : P.G[d]); };
-      if (ax_pos) tma_load_4d(smem_u32(sXL), &P.m_xface, bar, gv0, gu0, gy0, below(0, ex, gx0));
-      if (ax_neg) tma_load_4d(smem_u32(sXR), &P.m_xface, bar, gv0, gu0, gy0, above(0, ex, gx0));
+      if (ax_pos) {
+        if (P.bc[0] == 2 && ex == 0) tma_load_4d(smem_u32(sXL), &P.m_xhalo, bar, gv0, gu0, gy0, 0);
+        else tma_load_4d(smem_u32(sXL), &P.m_xface, bar, gv0, gu0, gy0, below(0, ex, gx0));
+      }
+      if (ax_neg) {
+        if (P.bc[0] == 2 && ex == P.N[0] - 1) tma_load_4d(smem_u32(sXR), &P.m_xhalo, bar, gv0, gu0, gy0, 1);
+        else tma_load_4d(smem_u32(sXR), &P.m_xface, bar, gv0, gu0, gy0, above(0, ex, gx0));
+      }
       if (ay_pos) tma_load_4d(smem_u32(sYL), &P.m_yface, bar, gv0, gu0, below(1, ey, gy0), gx0);
       if (ay_neg) tma_load_4d(smem_u32(sYR), &P.m_yface, bar, gv0, gu0, above(1, ey, gy0), gx0);
       if (au_pos) tma_load_4d(smem_u32(sUL), &P.m_uface, bar, gv0, below(2, eu, gu0), gy0, gx0);

@@ -92,6 +92,10 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
     if (ay > 0.0) hy = ey > 0 ? gy0 - 1 : (p.bc[1] == 0 ? p.G[1] - 1 : -1);
     else if (ay < 0.0) hy = ey < p.N[1] - 1 ? gy0 + 4 : (p.bc[1] == 0 ? 0 : -1);
     const double* px = p.f + hx * s0 + gy0 * s1 + uv;
+    if (p.bc[0] == 2) {        // x-slab: at the slab's two x faces the exterior planes come from the halo buffer
+      if (ax > 0.0 && ex == 0) { hx = 0; px = p.xhalo + gy0 * s1 + uv; }
+      else if (ax < 0.0 && ex == p.N[0] - 1) { hx = 0; px = p.xhalo + s0 + gy0 * s1 + uv; }
+    }
     const double* py = p.f + gx0 * s0 + hy * s1 + uv;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -249,8 +253,12 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
     double o[4] = {sa.x, sa.y, sb.x, sb.y};
 #pragma unroll
     for (int jv = 0; jv < 4; ++jv) o[jv] += p.mode == 0 ? res[ju][jv] : p.c1 * fma(p.dt, res[ju][jv], fb[ju][jv]);
-    __stcs(q, make_double2(o[0], o[1]));
-    __stcs(q + 1, make_double2(o[2], o[3]));
+    if (p.wide_st) {        // the element's four v nodes are one 32-byte sector: a single 256-bit streaming store
+      asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(q), "d"(o[0]), "d"(o[1]), "d"(o[2]), "d"(o[3]) : "memory");
+    } else {
+      __stcs(q, make_double2(o[0], o[1]));
+      __stcs(q + 1, make_double2(o[2], o[3]));
+    }
     q += s2 / 2;
     if (p.partials) {
       const double rowsum = fma(w01.x, o[0], fma(w01.y, o[1], fma(w23.x, o[2], w23.y * o[3])));

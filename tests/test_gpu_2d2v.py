@@ -368,3 +368,131 @@ def test_density_with_more_than_65535_space_nodes():
     assert relerr(rho, o4.density(g, f)) < 1e-13
     ctx.close()
 
+
+
+# ---------------------------------------------------------------------------------------------
+# x-slab halo boundary (DG_BC_HALO, dg4_set_xhalo): two slabs on one GPU against the UNSHARDED oracle
+# ---------------------------------------------------------------------------------------------
+XSLAB_CASES = [
+    # N, n, bc0 of the global grid, x-elements of slab 0, expected kernel
+    ((5, 2, 2, 3), (3, 4, 5, 2), 0, 2, "rhs4_generic"),
+    ((4, 3, 2, 8), (4, 4, 4, 4), 0, 1, "rhs4_tile"),
+    ((4, 2, 3, 4), (4, 4, 4, 4), 1, 3, "rhs4_tile"),
+    ((3, 2, 2, 2), (6, 6, 6, 6), 0, 1, "rhs4_elem"),
+    ((3, 2, 1, 2), (8, 8, 8, 8), 0, 2, "rhs4_line"),
+    ((2, 1, 2, 2), (8, 8, 8, 8), 1, 1, "rhs4_line"),
+]
+
+
+def _slab(A, N, n, lo, hi, bc, omega_c, e0, e1):
+    dx = (hi[0] - lo[0]) / N[0]
+    return A.DG4Context((e1 - e0,) + tuple(N[1:]), n, (lo[0] + e0 * dx,) + tuple(lo[1:]), (lo[0] + e1 * dx,) + tuple(hi[1:]),
+                        bc=(A.BC_HALO,) + tuple(bc[1:]), omega_c=omega_c)
+
+
+def _fill_halos(halos, parts, bc0):
+    """halos[s][0] <- last x plane of the slab below, halos[s][1] <- first plane of the slab above (periodic wrap, or
+    zeros at the outer faces for zero inflow): device copies in stream order."""
+    S = len(parts)
+    for s in range(S):
+        below, above = parts[(s - 1) % S], parts[(s + 1) % S]
+        if s > 0 or bc0 == 0:
+            halos[s][0].copy_(below[-1])
+        else:
+            halos[s][0].zero_()
+        if s < S - 1 or bc0 == 0:
+            halos[s][1].copy_(above[0])
+        else:
+            halos[s][1].zero_()
+
+
+@pytest.mark.parametrize("N,n,bc0,split,kernel", XSLAB_CASES)
+def test_xslab_halo_stage_matches_unsharded_oracle(N, n, bc0, split, kernel):
+    """dg4_rk_stage on two x-slabs (exterior x planes from dg4_set_xhalo) = the stage on the whole grid (oracle)."""
+    A = api()
+    bc = (bc0, 0, 1, 1)
+    g = o4.make_grid(N, n, LO, HI, bc=bc, omega_c=0.8)
+    f, Ex, Ey = seeded_inputs(g)
+    fn = wl.counter_uniform_chunked(wl.SEED_CFG6_NOISE + 1, f.size).reshape(f.shape)
+    c0, c1, dt = 0.75, 0.25, 1e-3
+    ref = c0 * fn + c1 * (f + dt * o4.rhs(g, f, Ex, Ey))
+    cuts = [(0, split), (split, N[0])]
+    ctxs = [_slab(A, N, n, LO, HI, bc, 0.8, a, b) for a, b in cuts]
+    fs = [dev(f[a * n[0]:b * n[0]]) for a, b in cuts]
+    halos = [torch.empty((2,) + tuple(f.shape[1:]), dtype=torch.float64, device="cuda") for _ in cuts]
+    _fill_halos(halos, fs, bc0)
+    for (a, b), ctx, fsl, h in zip(cuts, ctxs, fs, halos):
+        with pytest.raises(A.DGError):
+            ctx.rhs(fsl, None, None)                        # halo context without a halo buffer
+        ctx.set_xhalo(h)
+        sl = slice(a * n[0], b * n[0])
+        rho = torch.empty(fsl.shape[:2], dtype=torch.float64, device="cuda")
+        out = ctx.rk_stage(fsl, dev(fn[sl]), dev(Ex[sl]), dev(Ey[sl]), torch.empty_like(fsl), c0, c1, dt, rho_out=rho)
+        assert ctx.last_kernel.startswith(kernel), ctx.last_kernel
+        assert relerr(out.cpu().numpy(), ref[sl]) < 1e-12 * max(1.0, np.abs(ref).max() / np.abs(ref[sl]).max())
+        assert relerr(rho.cpu().numpy(), o4.density(g, ref)[sl]) < 1e-12
+        r = ctx.rhs(fsl, dev(Ex[sl]), dev(Ey[sl])).cpu().numpy()
+        assert relerr(r, o4.rhs(g, f, Ex, Ey)[sl]) < 1e-12
+        ctx.close()
+
+
+def test_xslab_two_slabs_self_consistent_steps():
+    """Two SSP-RK3 steps with the 2-D Poisson solve at every stage, the phase space cut into two x-slabs: per stage the
+    slab densities are joined, the GLOBAL field is solved on an (x, y)-only context, the face planes are exchanged and each
+    slab runs dg4_rk_stage -- against oracle.vlasov2d2v.ssprk3_step on the whole grid."""
+    A = api()
+    N, n, k = (4, 2, 2, 8), (4, 4, 4, 4), 0.1
+    lo, hi = (0.0, 0.0, -8.5, -8.5), (2 * math.pi / k, 2 * math.pi / k, 8.5, 8.5)
+    bc = (0, 0, 1, 1)
+    g = o4.make_grid(N, n, lo, hi, bc=bc, omega_c=1.0, pmax=(3, 2))
+    x, y, u, v = [c.reshape(-1) for c in g.coords]
+    f0 = wl.add_uniform_noise(wl.ring2d_f0(x, y, u, v, k, k), wl.SEED_CFG6_NOISE, 1e-3)
+    dt, nsteps = 1e-3, 2
+    fo = f0
+    for _ in range(nsteps):
+        fo = o4.ssprk3_step(g, fo, dt)
+    cuts = [(0, 1), (1, 4)]
+    ctxs = [_slab(A, N, n, lo, hi, bc, 1.0, a, b) for a, b in cuts]
+    field = A.DG4Context((N[0], N[1], 1, 1), (n[0], n[1], 2, 2), lo, hi, bc=(0, 0, 1, 1), omega_c=1.0, pmax=(3, 2))
+    mk = lambda: [torch.empty((b - a) * n[0], *f0.shape[1:], dtype=torch.float64, device="cuda") for a, b in cuts]
+    fs, u1, u2 = [dev(f0[a * n[0]:b * n[0]]) for a, b in cuts], mk(), mk()
+    halos = [torch.empty((2,) + tuple(f0.shape[1:]), dtype=torch.float64, device="cuda") for _ in cuts]
+    rho = torch.empty(f0.shape[:2], dtype=torch.float64, device="cuda")
+    rho_parts = [rho[a * n[0]:b * n[0]] for a, b in cuts]
+    for ctx, h in zip(ctxs, halos):
+        ctx.set_xhalo(h)
+
+    def stage(src, fn, dst, stage_no, rho_known):
+        c0, c1 = A.ssprk3_stage_coeffs(stage_no)
+        if not rho_known:
+            for ctx, s, r in zip(ctxs, src, rho_parts):
+                ctx.density(s, r)
+        Ex, Ey = field.poisson_E(rho)
+        _fill_halos(halos, src, 0)
+        for (a, b), ctx, s, fnn, d, r in zip(cuts, ctxs, src, fn, dst, rho_parts):
+            sl = slice(a * n[0], b * n[0])
+            ctx.rk_stage(s, fnn if c0 != 0.0 else None, Ex[sl].contiguous(), Ey[sl].contiguous(), d, c0, c1, dt, rho_out=r)
+
+    for i in range(nsteps):
+        stage(fs, fs, u1, 0, i > 0)
+        stage(u1, fs, u2, 1, True)
+        stage(u2, fs, fs, 2, True)
+    got = np.concatenate([t.cpu().numpy() for t in fs], axis=0)
+    assert relerr(got, fo) < 1e-11
+    for c in ctxs + [field]:
+        c.close()
+
+
+def test_xslab_halo_argument_checks():
+    A = api()
+    ctx = A.DG4Context((2, 2, 2, 2), (4,) * 4, LO, HI, bc=(0, 0, 1, 1))
+    with pytest.raises(A.DGError):
+        ctx.set_xhalo(torch.zeros((2, 8, 8, 8), dtype=torch.float64, device="cuda"))      # not a halo context
+    ctx.close()
+    with pytest.raises(A.DGError):
+        A.DG4Context((2, 2, 2, 2), (4,) * 4, LO, HI, bc=(0, A.BC_HALO, 1, 1))             # only x can be a slab
+    slab = A.DG4Context((2, 2, 2, 2), (4,) * 4, LO, HI, bc=(A.BC_HALO, 0, 1, 1))
+    f = torch.zeros(slab.flat_shape, dtype=torch.float64, device="cuda")
+    with pytest.raises(A.DGError):
+        slab.ssprk3_run(f, 1e-3, 1, True)                                                  # the Poisson solve is global
+    slab.close()
