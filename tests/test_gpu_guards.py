@@ -76,7 +76,7 @@ def guarded_workspace(ctx, A, batch=1):
 
 
 RHS_GRIDS = [
-    # nelem, order, bc (ragged v tails for every tile width: KV = 8, 4, 4, 2)
+    # nelem, order, bc (ragged v tails for every tile width: KV = 8, 8, 4, 2)
     ((3, 3, 11), (4, 4, 4), (0, 1, 1)),
     ((2, 3, 5), (6, 6, 6), (0, 0, 1)),
     ((3, 2, 7), (8, 8, 8), (0, 1, 1)),

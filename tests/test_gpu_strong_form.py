@@ -48,7 +48,7 @@ CASES = [
     ((3, 5, 9), (8, 8, 8), BOX3[0], BOX3[1], (0, 1, 1), 1.0, 0, "auto"),                  # tiled <8,4>, ragged v tile
     ((3, 5, 9), (8, 8, 8), BOX3[0], BOX3[1], (0, 1, 1), 1.0, 0, "generic"),
     ((4, 3, 17), (4, 4, 4), BOX3[0], BOX3[1], (0, 0, 0), 0.7, 0, "auto"),                 # tiled <4,8>, all periodic
-    ((3, 4, 5), (6, 6, 6), BOX3[0], BOX3[1], (0, 1, 1), 1.0, 1, "auto"),                  # tiled <6,4>, lumped mass
+    ((3, 4, 5), (6, 6, 6), BOX3[0], BOX3[1], (0, 1, 1), 1.0, 1, "auto"),                  # tiled <6,8>, lumped mass
     ((2, 3, 4), (10, 10, 10), BOX3[0], BOX3[1], (0, 1, 0), -0.5, 0, "auto"),              # tiled <10,3>
 ]
 
