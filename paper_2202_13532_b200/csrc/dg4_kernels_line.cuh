@@ -112,69 +112,20 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
     if (smem_u32(smem) & 511u) __trap();             // the 64-byte swizzle pattern repeats every 512 bytes
     dgt::mbar_init(bar, 1);
     dgt::fence_mbar_init();
+    // the tile itself (and f_n) first: the loads are in flight while the threads fetch their speeds and work out which halos
+    // the signs need
+    dgt::mbar_expect_tx_noarrive(bar, (FN ? 2u : 1u) * SZ_TILE);
+    tma_load_4d(smem_u32(sF), &P.m_main, bar, gv0, gu0, gy0, gx0);
+    if (FN) tma_load_4d(smem_u32(sN), &P.m_fn, bar, gv0, gu0, gy0, gx0);
   }
   const double cf = (P.mode != 0) ? P.c1 : 0.0;
   const double cr = (P.mode != 0) ? P.c1 * P.dt : 1.0;
-  // the speeds below carry the factor cr; the upwind side of Eq. 23 follows the sign of the speed itself
+  // the speeds below carry the factor cr; the upwind side of Eq. 23 follows the sign of the speed itself (upwind_bits)
   const bool flip = cr < 0.0;
-  auto is_pos = [flip](double a) { return flip ? a < 0.0 : a > 0.0; };
-  auto is_neg = [flip](double a) { return flip ? a > 0.0 : a < 0.0; };
-
-  if (t < 32) {
-    // Which upwind halos can be needed at all: signs of the speeds (Eq. 28) over the tile.  The 64 (x, y) nodes of E_x, E_y
-    // are scanned by warp 0, two per lane.
-    if (t == 0) {
-      dgt::mbar_expect_tx_noarrive(bar, (FN ? 2u : 1u) * SZ_TILE);
-      tma_load_4d(smem_u32(sF), &P.m_main, bar, gv0, gu0, gy0, gx0);
-      if (FN) tma_load_4d(smem_u32(sN), &P.m_fn, bar, gv0, gu0, gy0, gx0);
-    }
-    double exmin = 0.0, exmax = 0.0, eymin = 0.0, eymax = 0.0;
-    {
-      const int jx = t >> 2, jy = (t & 3) * 2;
-      const long long g = (long long)(gx0 + jx) * P.G[1] + gy0 + jy;
-      if (P.Ex) { const double a = P.Ex[g], b = P.Ex[g + 1]; exmin = fmin(a, b); exmax = fmax(a, b); }
-      if (P.Ey) { const double a = P.Ey[g], b = P.Ey[g + 1]; eymin = fmin(a, b); eymax = fmax(a, b); }
-#pragma unroll
-      for (int off = 16; off > 0; off >>= 1) {
-        exmin = fmin(exmin, __shfl_xor_sync(0xffffffffu, exmin, off)); exmax = fmax(exmax, __shfl_xor_sync(0xffffffffu, exmax, off));
-        eymin = fmin(eymin, __shfl_xor_sync(0xffffffffu, eymin, off)); eymax = fmax(eymax, __shfl_xor_sync(0xffffffffu, eymax, off));
-      }
-    }
-    if (t == 0) {
-      const double u_lo = P.cu[gu0], u_hi = P.cu[gu0 + NN - 1], v_lo = P.cv[gv0], v_hi = P.cv[gv0 + NN - 1];
-      const bool ax_pos = u_hi > 0.0, ax_neg = u_lo < 0.0;                        // a_x = u
-      const bool ay_pos = v_hi > 0.0, ay_neg = v_lo < 0.0;                        // a_y = v
-      const double wv_lo = -P.omega_c * v_lo, wv_hi = -P.omega_c * v_hi;          // a_u = -E_x - omega_c v
-      const bool au_pos = (-exmin + fmax(wv_lo, wv_hi)) > 0.0, au_neg = (-exmax + fmin(wv_lo, wv_hi)) < 0.0;
-      const double wu_lo = P.omega_c * u_lo, wu_hi = P.omega_c * u_hi;            // a_v = -E_y + omega_c u
-      const bool av_pos = (-eymin + fmax(wu_lo, wu_hi)) > 0.0, av_neg = (-eymax + fmin(wu_lo, wu_hi)) < 0.0;
-      const uint32_t bytes = (uint32_t)((ax_pos + ax_neg + ay_pos + ay_neg + au_pos + au_neg) * SZ_FACE + (av_pos + av_neg) * SZ_VFACE);
-      dgt::mbar_expect_tx(bar, bytes);          // the one arrival of this phase, with the halo bytes
-      // neighbour node index in dimension d below / above the element: periodic wrap (the paper's roll) by
-      // coordinate; zero inflow: outside the tensor, where TMA fills zeros (exterior state 0, reading C2)
-      auto below = [&](int d, int e, int g0) { return e > 0 ? g0 - 1 : (P.bc[d] == 0 ? P.G[d] - 1 : -1); };
-      auto above = [&](int d, int e, int g0) { return e < P.N[d] - 1 ? g0 + NN : (P.bc[d] == 0 ? 0 : P.G[d]); };
-      if (ax_pos) {
-        if (P.bc[0] == 2 && ex == 0) tma_load_4d(smem_u32(sXL), &P.m_xhalo, bar, gv0, gu0, gy0, 0);
-        else tma_load_4d(smem_u32(sXL), &P.m_xface, bar, gv0, gu0, gy0, below(0, ex, gx0));
-      }
-      if (ax_neg) {
-        if (P.bc[0] == 2 && ex == P.N[0] - 1) tma_load_4d(smem_u32(sXR), &P.m_xhalo, bar, gv0, gu0, gy0, 1);
-        else tma_load_4d(smem_u32(sXR), &P.m_xface, bar, gv0, gu0, gy0, above(0, ex, gx0));
-      }
-      if (ay_pos) tma_load_4d(smem_u32(sYL), &P.m_yface, bar, gv0, gu0, below(1, ey, gy0), gx0);
-      if (ay_neg) tma_load_4d(smem_u32(sYR), &P.m_yface, bar, gv0, gu0, above(1, ey, gy0), gx0);
-      if (au_pos) tma_load_4d(smem_u32(sUL), &P.m_uface, bar, gv0, below(2, eu, gu0), gy0, gx0);
-      if (au_neg) tma_load_4d(smem_u32(sUR), &P.m_uface, bar, gv0, above(2, eu, gu0), gy0, gx0);
-      // v faces: boxes of two nodes (16 bytes, the TMA minimum); the face node is the second of the lower box, the first of the upper
-      if (av_pos) tma_load_4d(smem_u32(sVL), &P.m_vface, bar, ev > 0 ? gv0 - 2 : (P.bc[3] == 0 ? P.G[3] - 2 : -2), gu0, gy0, gx0);
-      if (av_neg) tma_load_4d(smem_u32(sVR), &P.m_vface, bar, ev < P.N[3] - 1 ? gv0 + NN : (P.bc[3] == 0 ? 0 : P.G[3]), gu0, gy0, gx0);
-    }
-  }
   // thread <-> line maps.  x / y / u phases: t = (hi, mid, cv); v phase: rows t and t + 256.
   const int cv = t & 3, mid = (t >> 2) & 7, hi = t >> 5;
   const int c2 = 2 * cv;
-  // E-independent speeds (Eq. 28), scaled by cr J_d, fetched while the TMA loads are in flight
+  // speeds (Eq. 28), scaled by cr J_d: all global reads of the thread in one batch
   const double ax = cr * P.Jx * P.cu[gu0 + mid];                                   // phase x: mid = ju
   const double2 vv = *reinterpret_cast<const double2*>(P.cv + gv0 + c2);
   const double ay0 = cr * P.Jy * vv.x, ay1 = cr * P.Jy * vv.y;                     // phase y: a_y = v
@@ -184,7 +135,6 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
     const double exf = P.Ex ? P.Ex[(long long)(gx0 + hi) * P.G[1] + gy0 + mid] : 0.0;
     au0 = cr * P.Ju * (-exf - P.omega_c * vv.x);                                   // a_u = -E_x - omega_c v
     au1 = cr * P.Ju * (-exf - P.omega_c * vv.y);
-    if (urev) { au0 = -au0; au1 = -au1; }                                          // mirrored line: a' = -a
   }
   double avl[2];
   {
@@ -196,8 +146,53 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
       avl[l] = cr * P.Jv * (-eyf + wu);                                            // a_v = -E_y + omega_c u
     }
   }
-  __syncthreads();           // barrier init visible to all waiters
+  // upwind sides of this thread's lines (Eq. 23): bits 0-1 x, 2-3 / 4-5 y, 6-7 / 8-9 u, 10-11 / 12-13 v; bit 0 of a pair =
+  // a > 0 (the state below the element enters), bit 1 = a < 0.  The threads' lines cover the tile in every phase, so the OR
+  // over the CTA says exactly which face halos are read at all.
+  const int um = dgt::upwind_bits(ax, flip) | (dgt::upwind_bits(ay0, flip) << 2) | (dgt::upwind_bits(ay1, flip) << 4) |
+                 (dgt::upwind_bits(au0, flip) << 6) | (dgt::upwind_bits(au1, flip) << 8) |
+                 (dgt::upwind_bits(avl[0], flip) << 10) | (dgt::upwind_bits(avl[1], flip) << 12);
+  if (urev) { au0 = -au0; au1 = -au1; }                                            // mirrored line: a' = -a
+  int* sAny = reinterpret_cast<int*>(smem + OFF_BAR + 64);                         // one word per warp
+  {
+    const int w_or = __reduce_or_sync(0xffffffffu, um);
+    if ((t & 31) == 0) sAny[t >> 5] = w_or;
+  }
+  __syncthreads();           // also makes the barrier initialisation visible to all waiters
+  if (t == 0) {
+    int any = 0;
+#pragma unroll
+    for (int w = 0; w < NT / 32; ++w) any |= sAny[w];
+    const int ax_pos = any & 1, ax_neg = (any >> 1) & 1;
+    const int ay_pos = ((any >> 2) | (any >> 4)) & 1, ay_neg = ((any >> 3) | (any >> 5)) & 1;
+    const int au_pos = ((any >> 6) | (any >> 8)) & 1, au_neg = ((any >> 7) | (any >> 9)) & 1;
+    const int av_pos = ((any >> 10) | (any >> 12)) & 1, av_neg = ((any >> 11) | (any >> 13)) & 1;
+    const uint32_t bytes = (uint32_t)((ax_pos + ax_neg + ay_pos + ay_neg + au_pos + au_neg) * SZ_FACE + (av_pos + av_neg) * SZ_VFACE);
+    dgt::mbar_expect_tx(bar, bytes);          // the one arrival of this phase, with the halo bytes
+    // neighbour node index in dimension d below / above the element: periodic wrap (the paper's roll) by
+    // coordinate; zero inflow: outside the tensor, where TMA fills zeros (exterior state 0, reading C2)
+    auto below = [&](int d, int e, int g0) { return e > 0 ? g0 - 1 : (P.bc[d] == 0 ? P.G[d] - 1 : -1); };
+    auto above = [&](int d, int e, int g0) { return e < P.N[d] - 1 ? g0 + NN : (P.bc[d] == 0 ? 0 : P.G[d]); };
+    if (ax_pos) {
+      if (P.bc[0] == 2 && ex == 0) tma_load_4d(smem_u32(sXL), &P.m_xhalo, bar, gv0, gu0, gy0, 0);
+      else tma_load_4d(smem_u32(sXL), &P.m_xface, bar, gv0, gu0, gy0, below(0, ex, gx0));
+    }
+    if (ax_neg) {
+      if (P.bc[0] == 2 && ex == P.N[0] - 1) tma_load_4d(smem_u32(sXR), &P.m_xhalo, bar, gv0, gu0, gy0, 1);
+      else tma_load_4d(smem_u32(sXR), &P.m_xface, bar, gv0, gu0, gy0, above(0, ex, gx0));
+    }
+    if (ay_pos) tma_load_4d(smem_u32(sYL), &P.m_yface, bar, gv0, gu0, below(1, ey, gy0), gx0);
+    if (ay_neg) tma_load_4d(smem_u32(sYR), &P.m_yface, bar, gv0, gu0, above(1, ey, gy0), gx0);
+    if (au_pos) tma_load_4d(smem_u32(sUL), &P.m_uface, bar, gv0, below(2, eu, gu0), gy0, gx0);
+    if (au_neg) tma_load_4d(smem_u32(sUR), &P.m_uface, bar, gv0, above(2, eu, gu0), gy0, gx0);
+    // v faces: boxes of two nodes (16 bytes, the TMA minimum); the face node is the second of the lower box, the first of the upper
+    if (av_pos) tma_load_4d(smem_u32(sVL), &P.m_vface, bar, ev > 0 ? gv0 - 2 : (P.bc[3] == 0 ? P.G[3] - 2 : -2), gu0, gy0, gx0);
+    if (av_neg) tma_load_4d(smem_u32(sVR), &P.m_vface, bar, ev < P.N[3] - 1 ? gv0 + NN : (P.bc[3] == 0 ? 0 : P.G[3]), gu0, gy0, gx0);
+  }
   dgt::mbar_wait(bar, 0);
+  // upwind tests on the bits (the mirrored u lines swapped their speeds' signs above, and their faces below)
+  auto pos = [um](int line) { return (um >> (2 * line)) & 1; };
+  auto neg = [um](int line) { return (um >> (2 * line + 1)) & 1; };
 
   // ---------------- phase x: thread = (jy = hi, ju = mid, cv), lines over jx ----------------
   {
@@ -208,9 +203,9 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
       const double2 v = *reinterpret_cast<const double2*>(&sF[chunk_off(k * 64 + rbase, cv)]);
       f[0][k] = v.x; f[1][k] = v.y;
     }
-    if (is_pos(ax)) { const double2 v = *reinterpret_cast<const double2*>(&sXL[rbase * NN + c2]); uL[0] = v.x; uL[1] = v.y; }
+    if (pos(0)) { const double2 v = *reinterpret_cast<const double2*>(&sXL[rbase * NN + c2]); uL[0] = v.x; uL[1] = v.y; }
     else { uL[0] = f[0][0]; uL[1] = f[1][0]; }
-    if (is_neg(ax)) { const double2 v = *reinterpret_cast<const double2*>(&sXR[rbase * NN + c2]); uR[0] = v.x; uR[1] = v.y; }
+    if (neg(0)) { const double2 v = *reinterpret_cast<const double2*>(&sXR[rbase * NN + c2]); uR[0] = v.x; uR[1] = v.y; }
     else { uR[0] = f[0][NN - 1]; uR[1] = f[1][NN - 1]; }
     dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
 #pragma unroll
@@ -232,10 +227,10 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
     }
     const double2 hl = *reinterpret_cast<const double2*>(&sYL[(hi * NN + mid) * NN + c2]);
     const double2 hr = *reinterpret_cast<const double2*>(&sYR[(hi * NN + mid) * NN + c2]);
-    uL[0] = is_pos(ay0) ? hl.x : f[0][0];
-    uL[1] = is_pos(ay1) ? hl.y : f[1][0];
-    uR[0] = is_neg(ay0) ? hr.x : f[0][NN - 1];
-    uR[1] = is_neg(ay1) ? hr.y : f[1][NN - 1];
+    uL[0] = pos(1) ? hl.x : f[0][0];
+    uL[1] = pos(2) ? hl.y : f[1][0];
+    uR[0] = neg(1) ? hr.x : f[0][NN - 1];
+    uR[1] = neg(2) ? hr.y : f[1][NN - 1];
     dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
 #pragma unroll
     for (int j = 0; j < NN; ++j) {
@@ -257,10 +252,11 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
     // the mirrored threads see the element's upper face as their "left" one
     const double2 hl = *reinterpret_cast<const double2*>(&(urev ? sUR : sUL)[(hi * NN + mid) * NN + c2]);
     const double2 hr = *reinterpret_cast<const double2*>(&(urev ? sUL : sUR)[(hi * NN + mid) * NN + c2]);
-    uL[0] = is_pos(au0) ? hl.x : f[0][0];
-    uL[1] = is_pos(au1) ? hl.y : f[1][0];
-    uR[0] = is_neg(au0) ? hr.x : f[0][NN - 1];
-    uR[1] = is_neg(au1) ? hr.y : f[1][NN - 1];
+    // (bits 3, 4 describe the true speeds; a mirrored line sees them with the opposite sign)
+    uL[0] = (urev ? neg(3) : pos(3)) ? hl.x : f[0][0];
+    uL[1] = (urev ? neg(4) : pos(4)) ? hl.y : f[1][0];
+    uR[0] = (urev ? pos(3) : neg(3)) ? hr.x : f[0][NN - 1];
+    uR[1] = (urev ? pos(4) : neg(4)) ? hr.y : f[1][NN - 1];
     dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
 #pragma unroll
     for (int i = 0; i < NN; ++i) {
@@ -284,8 +280,8 @@ __global__ void __launch_bounds__(NT, 2) rhs4_line_kernel(const __grid_constant_
         acc[l][2 * c] = a2.x; acc[l][2 * c + 1] = a2.y;
       }
       uL[l] = f[l][0]; uR[l] = f[l][NN - 1];
-      if (is_pos(avl[l])) uL[l] = sVL[row * 2 + 1];
-      if (is_neg(avl[l])) uR[l] = sVR[row * 2];
+      if (pos(5 + l)) uL[l] = sVL[row * 2 + 1];
+      if (neg(5 + l)) uR[l] = sVR[row * 2];
     }
     dgt::apply_lines2<NN>(P, P.strong != 0, f, uL, uR, s);
     double psum[2] = {0.0, 0.0};
