@@ -31,6 +31,12 @@ __device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
 
+// 8-byte copy that reads `bytes` (8 or 0) from global memory and fills the rest with zeros: an absent neighbour (zero inflow,
+// or a = 0: no flux) costs no branch
+__device__ __forceinline__ void cp_async8_zfill(void* smem, const void* gmem, unsigned bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
@@ -85,6 +91,7 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
     }
   }
   {
+    // x and y faces of phase A: one value per (x or y) line of the thread, from the side the sign of the speed selects
     const long long uv = (long long)(gu0 + ju_a) * s2 + gv0 + rv;
     int hx = -1, hy = -1;
     if (ax > 0.0) hx = ex > 0 ? gx0 - 1 : (p.bc[0] == 0 ? p.G[0] - 1 : -1);
@@ -97,13 +104,15 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
       else if (ax < 0.0 && ex == p.N[0] - 1) { hx = 0; px = p.xhalo + s0 + gy0 * s1 + uv; }
     }
     const double* py = p.f + gx0 * s0 + hy * s1 + uv;
+    const unsigned nx = hx >= 0 ? 8u : 0u, ny = hy >= 0 ? 8u : 0u;
+    if (hx < 0) px = p.f;          // nothing is read, the address only has to be valid
+    if (hy < 0) py = p.f;
+    const long long sx = hx >= 0 ? s1 : 0, sy = hy >= 0 ? s0 : 0;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-      if (hx >= 0) cp_async8(hXs + j * NT + tid, px);
-      else hXs[j * NT + tid] = 0.0;
-      if (hy >= 0) cp_async8(hYs + j * NT + tid, py);
-      else hYs[j * NT + tid] = 0.0;
-      px += s1; py += s0;
+      cp_async8_zfill(hXs + j * NT + tid, px, nx);
+      cp_async8_zfill(hYs + j * NT + tid, py, ny);
+      px += sx; py += sy;
     }
   }
   if (use_fn) {                                                   // f_n lands where the running sums will live
@@ -127,11 +136,15 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
     // u faces: one value per u line (fixed jv), from the row below or above the tile by the sign of a_u
     const int lo = eu > 0 ? gu0 - 1 : (p.bc[2] == 0 ? p.G[2] - 1 : -1);
     const int hi = eu < p.N[2] - 1 ? gu0 + 4 : (p.bc[2] == 0 ? 0 : -1);
+    const double* blo = lo >= 0 ? p.f + xy + lo * s2 + gvb : p.f;
+    const double* bhi = hi >= 0 ? p.f + xy + hi * s2 + gvb : p.f;
+    const unsigned nlo = lo >= 0 ? 8u : 0u, nhi = hi >= 0 ? 8u : 0u;
 #pragma unroll
     for (int jv = 0; jv < 4; ++jv) {
-      const int g = au[jv] > 0.0 ? lo : (au[jv] < 0.0 ? hi : -1);
-      if (g >= 0) cp_async8(hUs + jv * NT + tid, p.f + xy + g * s2 + gvb + jv);
-      else hUs[jv * NT + tid] = 0.0;
+      const bool up = au[jv] > 0.0;
+      const unsigned nb = up ? nlo : (au[jv] < 0.0 ? nhi : 0u);
+      const double* src = up ? blo : bhi;
+      cp_async8_zfill(hUs + jv * NT + tid, src + jv, nb);         // blo / bhi are valid addresses even when nothing is read
     }
   }
   asm volatile("cp.async.commit_group;" ::: "memory");
@@ -140,10 +153,16 @@ __global__ void __launch_bounds__(16 * KV, MINB) rhs4_tile_kernel(const Params p
   {
     const int vlo = evb > 0 ? gv0 - 1 : (p.bc[3] == 0 ? p.G[3] - 1 : -1);
     const int vhi = evb < nvb - 1 ? gv0 + R : (p.bc[3] == 0 ? 0 : -1);
+    // a lane sits on at most one tile edge (KV >= 2): its candidate neighbour column, and the sign of a_v that takes it
+    const bool low = (ev == 0);
+    const int gedge = low ? vlo : (ev == KV - 1 ? vhi : -1);
+    const double* rowp = p.f + xy + gu0 * s2 + (gedge >= 0 ? gedge : 0);
 #pragma unroll
     for (int ju = 0; ju < 4; ++ju) {
-      const int g = (ev == 0 && av[ju] > 0.0) ? vlo : ((ev == KV - 1 && av[ju] < 0.0) ? vhi : -1);
-      if (g >= 0) eV[ju] = __ldg(p.f + xy + (gu0 + ju) * s2 + g);
+      const bool need = gedge >= 0 && (low ? av[ju] > 0.0 : av[ju] < 0.0);
+      double v = 0.0;
+      asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q ld.global.nc.f64 %0, [%1];\n}" : "+d"(v) : "l"(rowp + ju * s2), "r"((int)need) : "memory");
+      eV[ju] = v;
     }
   }
   asm volatile("cp.async.wait_all;" ::: "memory");
