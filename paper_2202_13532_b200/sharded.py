@@ -157,6 +157,12 @@ class CudaBackend:
     def set_push(self, left_dst, right_dst):
         self.slab.set_xhalo_push(left_dst, right_dst)
 
+    def plain_launches(self):
+        """Push mode across devices: no programmatic dependent launch around the collectives that order the peer stores
+        (point 3)."""
+        self.slab.set_option(self.api.OPT_PDL, 0)
+        self.field.set_option(self.api.OPT_PDL, 0)
+
     def stage_coeffs(self, stage):
         """(c0, c1) of Shu-Osher stage 0, 1, 2: the table lives in the library (dg_ssprk3_stage_coeffs)."""
         return self.api.ssprk3_stage_coeffs(stage)
@@ -190,6 +196,8 @@ class XSlabStepper:
             self.H, self.H_left, self.H_right = self.comm.alloc_halos(shp[1:], self.u1.device, periodic=(self.bc[0] == 0))
             self.sidx = 0
             self.halo = self.H[0]
+            if world > 1 and hasattr(self.be, "plain_launches"):
+                self.be.plain_launches()
             self.token = self.be.empty((1,))
         else:
             self.halo = self.be.empty((2,) + shp[1:])
