@@ -376,10 +376,14 @@ inline int launch_field_fused(const FieldFusedParams& P, int grid, bool pdl, cud
   if (ensure_dyn_smem(reinterpret_cast<const void*>(field_fused_kernel), smem) != cudaSuccess) return DG_ERR_CUDA;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = smem; cfg.stream = st;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  // The kernel's CTAs meet at a grid-wide rendezvous: a cooperative launch makes the driver check that all of them can be
+  // resident together (grid <= the SM count by construction, one CTA per SM) instead of assuming it.
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeCooperative;
+  at[0].val.cooperative = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
   return cudaLaunchKernelEx(&cfg, field_fused_kernel, P) == cudaSuccess ? DG_OK : DG_ERR_CUDA;
 }
 
