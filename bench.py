@@ -329,6 +329,8 @@ def run_ours(args, w, name):
         return run_xslab(args, w, name, world, rank, local, dev, barrier, max_over_ranks, parallelism)
     ga = grid_args(w)
     ctx = api.DGContext(device=local, **ga)
+    if args.smem_pad_kb:
+        ctx.set_option(api.OPT_SMEM_PAD_KB, args.smem_pad_kb)      # occupancy sweep of the tiled kernel (profiles/r2_kernels.md)
     f0 = make_f0(ctx.nodes(0), ctx.nodes(1), ctx.nodes(2), w)
     dof = f0.size
     dt = w["dt"]
@@ -411,7 +413,8 @@ def run_ours(args, w, name):
             "config": {"workload": name, "grid": "x".join(str(n * o) for n, o in zip(w["nelem"], w["order"])), "dof": dof,
                        "dt": dt, "self_consistent_poisson_each_stage": True, "mass_mode": 0,
                        "l2": "inputs (3 x %.2f GB) larger than L2; no flush needed" % (dof * 8 / 1e9),
-                       "parallelism": "replicas x%d" % world, "finite": finite},
+                       "parallelism": "replicas x%d" % world, "finite": finite,
+                       **({"smem_pad_kb": args.smem_pad_kb} if args.smem_pad_kb else {})},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "hbm_gbs_algorithmic_whole_step": 64.0 * dof * args.steps / (ms * 1e-3) / 1e9,
             "frac_whole_step": 64.0 * dof * args.steps / (ms * 1e-3) / 1e9 / peak,
@@ -863,6 +866,8 @@ def main():
     ap.add_argument("--no-secondary", action="store_true", help="skip the short runs of configs 2, 4, 5, 6")
     ap.add_argument("--secondary-budget-s", type=float, default=75.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--smem-pad-kb", type=int, default=0,
+                    help="configs 2, 3: unused extra shared memory per CTA of the tiled RHS kernel (DG_OPT_SMEM_PAD_KB), to cap the resident CTAs per SM")
     ap.add_argument("--full", action="store_true", help="oracle_timing: also the single-threaded 512^3 step")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
