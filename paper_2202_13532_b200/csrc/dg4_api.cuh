@@ -520,19 +520,13 @@ extern "C" int dg4_ssprk3_run(dg4_ctx* ctx, double* f_dev, double dt, int32_t ns
   cudaStream_t st = (cudaStream_t)stream;
   const bool sc = self_consistent != 0;
   const double *Ex = sc ? ctx->Ex : nullptr, *Ey = sc ? ctx->Ey : nullptr;
-  int chunks = 0, rc;
-  for (int s = 0; s < nsteps; ++s) {
-    if (sc) { rc = field4_from_partials_or_f(ctx, f_dev, chunks, st); if (rc) return rc; }
-    rc = launch_rhs4(ctx, f_dev, nullptr, Ex, Ey, ctx->u1, 1, 0.0, 1.0, dt, sc, &chunks, st);
-    if (rc) return rc;
-    if (sc) { rc = field4_from_partials_or_f(ctx, ctx->u1, chunks, st); if (rc) return rc; }
-    rc = launch_rhs4(ctx, ctx->u1, f_dev, Ex, Ey, ctx->u2, 1, 0.75, 0.25, dt, sc, &chunks, st);
-    if (rc) return rc;
-    if (sc) { rc = field4_from_partials_or_f(ctx, ctx->u2, chunks, st); if (rc) return rc; }
-    rc = launch_rhs4(ctx, ctx->u2, f_dev, Ex, Ey, f_dev, 1, 1.0 / 3.0, 2.0 / 3.0, dt, sc, &chunks, st);
-    if (rc) return rc;
-  }
-  return DG_OK;
+  int chunks = 0;          // > 0: ctx->partials holds density partials of the current stage input
+  return ssprk3_run_loop(
+      f_dev, ctx->u1, ctx->u2, nsteps, sc,
+      [&](const double* src) { return field4_from_partials_or_f(ctx, src, chunks, st); },
+      [&](int, const double* src, const double* fn, double* dst, double c0, double c1) {
+        return launch_rhs4(ctx, src, fn, Ex, Ey, dst, 1, c0, c1, dt, sc, &chunks, st);
+      });
 }
 
 extern "C" int dg4_ssprk3_run_host(dg4_ctx* ctx, double* f_host, double dt, int32_t nsteps, int32_t self_consistent) {

@@ -11,6 +11,7 @@
 #include "dg_context.hpp"
 #include "dg_kernels_generic.cuh"
 #include "dg_kernels_tiled.cuh"
+#include "dg_stepper.hpp"
 #include "dg_kernels_field.cuh"
 #include "dg_kernels_fft.cuh"
 #include "dg_microbench.cuh"
@@ -626,31 +627,16 @@ extern "C" int dg_ssprk3_run(dg_ctx* ctx, double* f_dev, double dt, int32_t nste
   if (self_consistent && ctx->desc.bc[0] != 0) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: self-consistent E needs periodic x");
   cudaStream_t st = (cudaStream_t)stream;
   int chunks = 0;          // > 0: ctx->partials holds density partials of the current stage input
-  for (int s = 0; s < nsteps; ++s) {
-    const double* E = nullptr;
-    int rc;
-    // stage 1: u1 = u + dt L(u)
-    if (self_consistent) { rc = field_from_partials_or_f(ctx, f_dev, chunks, st); if (rc) return rc; E = ctx->E; }
-    double c0, c1;
-    dg_ssprk3_stage_coeffs(0, &c0, &c1);
-    ctx->cur_stage = 1;
-    rc = launch_rhs(ctx, f_dev, nullptr, E, ctx->u1, 1, c0, c1, dt, self_consistent != 0, &chunks, st);
-    if (rc) { ctx->cur_stage = 0; return rc; }
-    // stage 2: u2 = 3/4 u + 1/4 (u1 + dt L(u1))
-    if (self_consistent) { rc = field_from_partials_or_f(ctx, ctx->u1, chunks, st); if (rc) return rc; }
-    dg_ssprk3_stage_coeffs(1, &c0, &c1);
-    ctx->cur_stage = 2;
-    rc = launch_rhs(ctx, ctx->u1, f_dev, E, ctx->u2, 1, c0, c1, dt, self_consistent != 0, &chunks, st);
-    if (rc) { ctx->cur_stage = 0; return rc; }
-    // stage 3: u = 1/3 u + 2/3 (u2 + dt L(u2)), in place (each node of u is read and written by one thread)
-    if (self_consistent) { rc = field_from_partials_or_f(ctx, ctx->u2, chunks, st); if (rc) return rc; }
-    dg_ssprk3_stage_coeffs(2, &c0, &c1);
-    ctx->cur_stage = 3;
-    rc = launch_rhs(ctx, ctx->u2, f_dev, E, f_dev, 1, c0, c1, dt, self_consistent != 0, &chunks, st);
-    ctx->cur_stage = 0;
-    if (rc) return rc;
-  }
-  return DG_OK;
+  const bool sc = self_consistent != 0;
+  const int rc = ssprk3_run_loop(
+      f_dev, ctx->u1, ctx->u2, nsteps, sc,
+      [&](const double* src) { return field_from_partials_or_f(ctx, src, chunks, st); },
+      [&](int k, const double* src, const double* fn, double* dst, double c0, double c1) {
+        ctx->cur_stage = k + 1;
+        return launch_rhs(ctx, src, fn, sc ? ctx->E : nullptr, dst, 1, c0, c1, dt, sc, &chunks, st);
+      });
+  ctx->cur_stage = 0;
+  return rc;
 }
 
 extern "C" int dg_ssprk3_step(dg_ctx* ctx, double* f_dev, double dt, int32_t self_consistent, void* stream) {
