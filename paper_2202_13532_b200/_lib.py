@@ -1,4 +1,4 @@
-"""ctypes loader for libdgvlasov.so -- the C ABI declared in include/dgvlasov.h and include/dgvlasov2d2v.h.
+"""ctypes loader for libdgvlasov.so -- the C ABI declared in include/dgvlasov.h, include/dgvlasov2d2v.h and include/dgvlasov_nd.h.
 
 There is no fallback: if the library has not been built (python -m paper_2202_13532_b200.build)
 importing the binding raises."""
@@ -37,6 +37,23 @@ class GridDesc4(C.Structure):
         ("bc", C.c_int32 * 4),
         ("omega_c", C.c_double),
         ("pmax", C.c_int32 * 2),
+        ("mass_mode", C.c_int32),
+        ("device", C.c_int32),
+    ]
+
+
+class GridDescN(C.Structure):
+    """dgn_grid_desc of include/dgvlasov_nd.h."""
+    _fields_ = [
+        ("dx", C.c_int32),
+        ("dv", C.c_int32),
+        ("nelem", C.c_int32 * 6),
+        ("order", C.c_int32 * 6),
+        ("lo", C.c_double * 6),
+        ("hi", C.c_double * 6),
+        ("bc", C.c_int32 * 6),
+        ("omega_c", C.c_double),
+        ("pmax", C.c_int32 * 3),
         ("mass_mode", C.c_int32),
         ("device", C.c_int32),
     ]
@@ -99,6 +116,17 @@ SIGNATURES = {
     "dg4_get_profile": (C.c_int, [_vp, _dp, C.POINTER(_i64), _i32]),
     "dg4_launch_count": (_i64, [_vp]),
     "dg4_last_kernel": (C.c_char_p, [_vp]),
+    "dgn_create": (C.c_int, [C.POINTER(GridDescN), C.POINTER(_vp)]),
+    "dgn_destroy": (C.c_int, [_vp]),
+    "dgn_workspace_bytes": (C.c_size_t, [_vp]),
+    "dgn_set_workspace": (C.c_int, [_vp, _vp, C.c_size_t]),
+    "dgn_rhs": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "dgn_rk_stage": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _dbl, _vp]),
+    "dgn_density": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "dgn_poisson_E": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "dgn_ssprk3_run": (C.c_int, [_vp, _vp, _dbl, _i32, _i32, _vp]),
+    "dgn_get_nodes": (C.c_int, [_vp, _i32, _dp]),
+    "dgn_launch_count": (_i64, [_vp]),
 }
 
 

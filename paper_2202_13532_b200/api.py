@@ -366,3 +366,78 @@ class DG4Context:
     @property
     def last_kernel(self):
         return _L.dg4_last_kernel(self._h).decode()
+
+
+class DGNContext:
+    """Dimension-generic variant (include/dgvlasov_nd.h): dgn_create / dgn_destroy plus one method per C entry point.
+    Phase space (x_1..x_dx, v_1..v_dv), 1 <= dx <= dv <= 3; f: [G_x1]..[G_vdv]; E: [dx][G_x1]..[G_xdx]; rho: [G_x1]..[G_xdx]."""
+
+    def __init__(self, dx, dv, nelem, order, lo, hi, bc=None, omega_c=0.0, pmax=None, mass_mode=0, device=0, workspace=True):
+        nd = dx + dv
+        if bc is None:
+            bc = (0,) * dx + (1,) * dv
+        pmax = tuple(pmax) if pmax is not None else (0,) * dx
+        d = _lib.GridDescN()
+        d.dx, d.dv = int(dx), int(dv)
+        for i in range(nd):
+            d.nelem[i], d.order[i], d.lo[i], d.hi[i], d.bc[i] = int(nelem[i]), int(order[i]), float(lo[i]), float(hi[i]), int(bc[i])
+        for i in range(dx):
+            d.pmax[i] = int(pmax[i])
+        d.omega_c, d.mass_mode, d.device = float(omega_c), int(mass_mode), int(device)
+        self._h = C.c_void_p()
+        _check(_L.dgn_create(C.byref(d), C.byref(self._h)), "dgn_create")
+        self.dx, self.dv, self.ndim = int(dx), int(dv), nd
+        self.nelem, self.order = tuple(nelem), tuple(order)
+        self.device = torch.device("cuda", device)
+        self.flat_shape = tuple(int(nelem[i]) * int(order[i]) for i in range(nd))
+        self._ws = None
+        if workspace:
+            nbytes = _L.dgn_workspace_bytes(self._h)
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            _check(_L.dgn_set_workspace(self._h, base, nbytes), "dgn_set_workspace")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            _L.dgn_destroy(self._h)
+            self._h = C.c_void_p()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def rhs(self, f, E=None, out=None):
+        out = torch.empty_like(f) if out is None else out
+        _check(_L.dgn_rhs(self._h, _ptr(f), _ptr(E), _ptr(out), _stream(self.device)), "dgn_rhs")
+        return out
+
+    def rk_stage(self, f_s, f_n, E, out, c0, c1, dt):
+        _check(_L.dgn_rk_stage(self._h, _ptr(f_s), _ptr(f_n), _ptr(E), _ptr(out), float(c0), float(c1), float(dt),
+                               _stream(self.device)), "dgn_rk_stage")
+        return out
+
+    def density(self, f, out=None):
+        out = torch.empty(self.flat_shape[:self.dx], dtype=torch.float64, device=self.device) if out is None else out
+        _check(_L.dgn_density(self._h, _ptr(f), _ptr(out), _stream(self.device)), "dgn_density")
+        return out
+
+    def poisson_E(self, rho, out=None):
+        out = torch.empty((self.dx,) + self.flat_shape[:self.dx], dtype=torch.float64, device=self.device) if out is None else out
+        _check(_L.dgn_poisson_E(self._h, _ptr(rho), _ptr(out), _stream(self.device)), "dgn_poisson_E")
+        return out
+
+    def ssprk3_run(self, f, dt, nsteps, self_consistent=True):
+        _check(_L.dgn_ssprk3_run(self._h, _ptr(f), float(dt), int(nsteps), int(bool(self_consistent)), _stream(self.device)), "dgn_ssprk3_run")
+        return f
+
+    def nodes(self, dim):
+        x = np.empty(self.flat_shape[dim])
+        _check(_L.dgn_get_nodes(self._h, dim, x.ctypes.data_as(C.POINTER(C.c_double))), "dgn_get_nodes")
+        return x
+
+    @property
+    def launch_count(self):
+        return int(_L.dgn_launch_count(self._h))

@@ -789,3 +789,4 @@ extern "C" const char* dg_last_kernel(const dg_ctx* ctx) { return ctx ? ctx->las
 extern "C" const char* dg_last_field_kernel(const dg_ctx* ctx) { return ctx ? ctx->last_field_kernel.c_str() : "none"; }
 
 #include "dg4_api.cuh"
+#include "dgn_api.cuh"

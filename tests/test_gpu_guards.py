@@ -216,3 +216,35 @@ def test_2d2v_kernels_stay_inside(nelem, n):
     twice(run_steps, "dg4_ssprk3_run")
     check({"f": f, "fn": fn, "Ex": Ex, "Ey": Ey, "workspace": ws}, "2D2V inputs / workspace")
     ctx.close()
+
+
+@pytest.mark.parametrize("dx,dv,nelem,order", [(1, 3, (3, 2, 2, 2), (3, 4, 3, 3)), (2, 3, (2, 2, 2, 2, 2), (3, 3, 3, 2, 3)),
+                                               (3, 3, (2, 1, 2, 2, 2, 1), (2, 4, 2, 3, 2, 4))])
+def test_dimension_generic_kernels_stay_inside(dx, dv, nelem, order):
+    A = api()
+    nd = dx + dv
+    lo = (0.0,) * dx + (-2.0,) * dv
+    hi = tuple(1.0 + 0.5 * i for i in range(dx)) + (2.0,) * dv
+    ctx = A.DGNContext(dx, dv, nelem, order, lo, hi, omega_c=0.9, pmax=(2,) * dx, workspace=False)
+    nbytes = A._L.dgn_workspace_bytes(ctx._h)
+    ws = Guarded(((nbytes + 7) // 8,))
+    A._check(A._L.dgn_set_workspace(ctx._h, ws.view.data_ptr(), nbytes), "dgn_set_workspace")
+    G = ctx.flat_shape
+    f0 = 0.5 + wl.uniform_field(G, 51)
+    f, fn = Guarded(G, f0), Guarded(G, wl.uniform_field(G, 52))
+    E = Guarded((dx,) + G[:dx], 0.4 * wl.uniform_field((dx,) + G[:dx], 53) - 0.2)
+
+    def run():
+        out, st, rho, Eo = Guarded(G), Guarded(G), Guarded(G[:dx]), Guarded((dx,) + G[:dx])
+        ctx.rhs(f.view, E.view, out.view)
+        ctx.rk_stage(f.view, fn.view, E.view, st.view, 0.75, 0.25, 1e-3)
+        ctx.density(f.view, rho.view)
+        ctx.poisson_E(rho.view, Eo.view)
+        g = Guarded(G, f0)
+        ctx.ssprk3_run(g.view, 1e-3, 2, True)
+        return {"out": out, "stage": st, "rho": rho, "E": Eo, "f": g}
+
+    twice(run, f"dgn_* {dx}D{dv}V")
+    check({"f": f, "fn": fn, "E": E, "workspace": ws}, "dgn inputs / workspace")
+    assert nd == len(G)
+    ctx.close()
