@@ -659,6 +659,59 @@ def run_config6(args, name, host_inputs=True, with_e2e=True):
     return line
 
 
+def run_config_nd(args, name):
+    """3D3V through the dimension-generic path (include/dgvlasov_nd.h, dgn_*): 8^6 elements x 2^6 LGL nodes = 16^6 DOF,
+    Maxwellian with a 1 % density wave along each space axis + seeded noise, the 3-D Poisson solve at every stage.  The generic
+    kernel family (one thread per node): a correctness-shaped path, reported against the HBM roofline for scale only."""
+    import torch
+    import workloads as wl
+    from paper_2202_13532_b200 import api
+    N, n = 8, 2
+    L = 4 * math.pi
+    ctx = api.DGNContext(3, 3, (N,) * 6, (n,) * 6, (0.0,) * 3 + (-6.0,) * 3, (L,) * 3 + (6.0,) * 3, omega_c=0.5, pmax=(4, 4, 4))
+    xs = [torch.from_numpy(ctx.nodes(d)).cuda() for d in range(6)]
+    shp = lambda d: [-1 if i == d else 1 for i in range(6)]
+    wave = 1.0 + 0.01 * sum(torch.cos(0.5 * xs[d]).reshape(shp(d)) for d in range(3))
+    maxw = 1.0
+    for d in range(3, 6):
+        maxw = maxw * (torch.exp(-0.5 * xs[d] ** 2) / math.sqrt(2 * math.pi)).reshape(shp(d))
+    f = (wave * maxw).contiguous()
+    g = torch.Generator(device="cuda"); g.manual_seed(wl.SEED_CFG6_NOISE + 1)
+    f += 1e-6 * (2.0 * torch.rand(f.shape, dtype=torch.float64, device="cuda", generator=g) - 1.0)
+    dt = 2e-3
+    warm = max(args.warmup, 3)
+    ctx.ssprk3_run(f, dt, warm, True)
+    torch.cuda.synchronize()
+    steps = args.steps
+
+    def region():
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.ssprk3_run(f, dt, steps, True)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    l0 = ctx.launch_count
+    ms, clocks = _clocks_during(region)
+    dof = (n * N) ** 6
+    peak, peak_src = measured_peak_hbm()
+    gbs = 64.0 * dof * steps / (ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": dof * 3.0 * steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": warm,
+        "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "grid": "x".join([str(n * N)] * 6), "order": n, "dof": dof, "dt": dt, "self_consistent_poisson_each_stage": True,
+                   "finite": bool(torch.isfinite(f).all().item()), "inputs": "analytic Maxwellian + waves + seeded torch noise, built on the device",
+                   "l2": "arrays (3 x %.2f GB) comparable to the 126 MB L2" % (dof * 8 / 1e9)},
+        "clocks": clocks, "gpu_launches": ctx.launch_count - l0,
+        "hbm_gbs_algorithmic_whole_step": gbs, "frac_whole_step": gbs / peak,
+        "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                     "kernel": "rhs_nd_kernel (generic, one thread per node)", "peak_source": peak_src,
+                     "how": "whole step (3 RHS launches + 3 three-dimensional field solves) by CUDA events; 64 B per DOF per step"}}
+    ctx.close()
+    return line
+
+
 def _cosine_batch_device(x, batch, seed):
     """Config-5 densities 1 + sum_{i<16} A cos(m x + phi) + N(0, 1e-3) built on the device (same distributions as
     workloads.cosine_sum_density, torch's seeded generator) -- throughput runs only."""
@@ -802,6 +855,8 @@ def run_secondary(args):
     a.steps = 6
     add(run_config6, a, "config6_2d2v_128^4", host_inputs=False, with_e2e=False)
     add(run_config6, a, "config6_2d2v_n8_128^4", host_inputs=False, with_e2e=False)
+    a.steps = 5
+    add(run_config_nd, a, "config7_3d3v_16^6")
     return out
 
 
@@ -854,7 +909,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config3_1d2v_512^3",
-                    choices=sorted(WORKLOADS) + sorted(CONFIG4) + ["config5_field", "fp64_peak", "oracle_timing"] + sorted(CONFIG6))
+                    choices=sorted(WORKLOADS) + sorted(CONFIG4) + ["config5_field", "fp64_peak", "oracle_timing", "config7_3d3v_16^6"] + sorted(CONFIG6))
     ap.add_argument("--batch", type=int, default=4096, help="config5_field only")
     ap.add_argument("--field-kernel", default="auto", choices=["auto", "dmma", "dfma", "fft"], help="config5_field only")
     ap.add_argument("--parallelism", default="auto", choices=["auto", "replicas", "xslab", "xslab-push"],
@@ -883,6 +938,8 @@ def main():
         return print(json.dumps(run_config5(args, args.workload)), flush=True)
     if args.workload in CONFIG6:
         return print(json.dumps(run_config6(args, args.workload)), flush=True)
+    if args.workload == "config7_3d3v_16^6":
+        return print(json.dumps(run_config_nd(args, args.workload)), flush=True)
     w = WORKLOADS[args.workload]
     if args.workload != "config3_1d2v_512^3":
         args.sustained_steps = 0 if args.sustained_steps == 1000 else args.sustained_steps

@@ -134,3 +134,36 @@ def test_argument_checks():
         ctx.ssprk3_run(f, 1e-3, 1, True)                                                     # Poisson needs periodic x
     ctx.ssprk3_run(f, 1e-3, 1, False)
     ctx.close()
+
+
+def test_landau_damping_2d3v_along_y():
+    """End-to-end signs of the d-dimensional path: an unmagnetised Maxwellian in three velocity dimensions with a 1 % density
+    wave of k = 0.5 along y (the SECOND space dimension: E_2 and a_{v_2} = -E_2 carry it).  E(0) has the closed form
+    -(A/k) sin(k y), and the field decays at the textbook Landau rate -0.1533 with omega_r = 1.4156 (a wrong sign of E_2 or of
+    a_{v_2} grows instead)."""
+    A = api()
+    ky = 0.5
+    ctx = A.DGNContext(2, 3, (1, 16, 8, 32, 8), (2, 4, 3, 4, 3), (0.0, 0.0, -6.0, -6.0, -6.0), (10.0, 2 * math.pi / ky, 6.0, 6.0, 6.0),
+                       bc=(0, 0, 1, 1, 1), omega_c=0.0, pmax=(1, 4))
+    x, y, u, v, w = (ctx.nodes(d) for d in range(5))
+    m = lambda s: np.exp(-0.5 * s * s) / math.sqrt(2 * math.pi)
+    f0 = (1.0 + 0.01 * np.cos(ky * y))[None, :, None, None, None] * m(u)[None, None, :, None, None] * m(v)[None, None, None, :, None] \
+        * m(w)[None, None, None, None, :] * np.ones((x.size, 1, 1, 1, 1))
+    f = dev(f0)
+    E = ctx.poisson_E(ctx.density(f)).cpu().numpy()
+    # 5e-4 of the amplitude 0.02: the quadrature error of the Maxwellian on the coarse u and w grids (8 x 3 nodes over +-6)
+    assert np.max(np.abs(E[1] + (0.01 / ky) * np.sin(ky * y)[None, :])) < 1e-5
+    assert np.max(np.abs(E[0])) < 1e-12
+    dt, per, nsamp = 0.008, 6, 400
+    amp = []
+    for _ in range(nsamp):
+        ctx.ssprk3_run(f, dt, per, True)
+        amp.append(float(ctx.poisson_E(ctx.density(f))[1].abs().max()))
+    amp = np.array(amp); t = dt * per * (np.arange(nsamp) + 1)
+    pk = [i for i in range(1, nsamp - 1) if amp[i] > amp[i - 1] and amp[i] > amp[i + 1]]
+    assert len(pk) >= 6
+    rate = np.polyfit(t[pk], np.log(amp[pk]), 1)[0]
+    period = float(np.mean(np.diff(t[pk])))
+    assert -0.165 < rate < -0.143, rate
+    assert abs(period - math.pi / 1.4156) < 0.08
+    ctx.close()
