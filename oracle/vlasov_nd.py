@@ -20,7 +20,9 @@ k^2 = sum k_{p_i}^2: Phi_p = -c_p / k^2, E_p = -i k_p Phi_p, p = 0 dropped (read
 
 Pins: tests/test_oracle_nd.py -- constant state, mass conservation, exact agreement with the pinned 1D2V and 2D2V oracles on
 their shapes, reduction of 3D3V / 2D3V / 1D3V states that do not depend on the extra dimensions to those oracles, plane-wave
-closed form of E in three dimensions.
+closed form of E in three dimensions.  The third force component a_{v_3} = -E_3 (the i >= 2 branch of `speeds`) is pinned by
+the relabelling symmetry (x_1, v_1) <-> (x_3, v_3) of the unmagnetised equation and by a z-only problem that must equal the
+pinned 1D1V oracle on (z, w); flipping that sign fails both.
 """
 from __future__ import annotations
 

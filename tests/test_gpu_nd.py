@@ -167,3 +167,33 @@ def test_landau_damping_2d3v_along_y():
     assert -0.165 < rate < -0.143, rate
     assert abs(period - math.pi / 1.4156) < 0.08
     ctx.close()
+
+
+def test_landau_damping_3d3v_along_z():
+    """The same run with the wave along z in the full 3D3V phase space: E_3 and a_{v_3} = -E_3 carry it (pinned on the oracle
+    side by tests/test_oracle_nd.py's pair-swap and z-only reductions).  Closed-form E(0), textbook rate -0.1533 and
+    omega_r = 1.4156; a wrong sign of E_3 or of a_{v_3} grows instead of damping."""
+    A = api()
+    kz = 0.5
+    ctx = A.DGNContext(3, 3, (1, 1, 16, 8, 8, 32), (2, 2, 4, 3, 3, 4), (0.0, 0.0, 0.0, -6.0, -6.0, -6.0),
+                       (10.0, 7.0, 2 * math.pi / kz, 6.0, 6.0, 6.0), bc=(0, 0, 0, 1, 1, 1), omega_c=0.0, pmax=(1, 1, 4))
+    x, y, z, u, v, w = (ctx.nodes(d) for d in range(6))
+    m = lambda s: np.exp(-0.5 * s * s) / math.sqrt(2 * math.pi)
+    f0 = np.einsum("a,b,c,d,e,f->abcdef", np.ones(x.size), np.ones(y.size), 1.0 + 0.01 * np.cos(kz * z), m(u), m(v), m(w))
+    f = dev(f0)
+    E = ctx.poisson_E(ctx.density(f)).cpu().numpy()
+    assert np.max(np.abs(E[2] + (0.01 / kz) * np.sin(kz * z)[None, None, :])) < 1e-5
+    assert max(np.max(np.abs(E[0])), np.max(np.abs(E[1]))) < 1e-12
+    dt, per, nsamp = 0.008, 6, 400
+    amp = []
+    for _ in range(nsamp):
+        ctx.ssprk3_run(f, dt, per, True)
+        amp.append(float(ctx.poisson_E(ctx.density(f))[2].abs().max()))
+    amp = np.array(amp); t = dt * per * (np.arange(nsamp) + 1)
+    pk = [i for i in range(1, nsamp - 1) if amp[i] > amp[i - 1] and amp[i] > amp[i + 1]]
+    assert len(pk) >= 6
+    rate = np.polyfit(t[pk], np.log(amp[pk]), 1)[0]
+    period = float(np.mean(np.diff(t[pk])))
+    assert -0.165 < rate < -0.143, rate
+    assert abs(period - math.pi / 1.4156) < 0.08
+    ctx.close()

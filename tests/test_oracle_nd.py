@@ -128,3 +128,48 @@ def test_plane_wave_field_closed_form_3d(p):
         exact = -(A / k2) * k[i] * np.sin(arg)
         # discretisation error of the n = 6 projection at 2-5 elements per wavelength; a wrong sign or factor is O(1)
         assert np.max(np.abs(E[i] - exact)) < 1e-4 * A / math.sqrt(k2), (i, np.max(np.abs(E[i] - exact)))
+
+
+# ---------------------------------------------------------------------------------------------
+# the third force component, a_{v_3} = -E_3 (Eq. 28 carried to three space dimensions; "n-dimensions",
+# PAPER.md:43).  Both pins below fail when the sign of E in the i >= 2 branch of `speeds` is flipped.
+# ---------------------------------------------------------------------------------------------
+def test_3d3v_unmagnetised_rhs_commutes_with_swapping_the_first_and_third_pair():
+    """Without B the Vlasov equation does not know which (x_i, v_i) pair is which: relabelling (x_1, v_1) <-> (x_3, v_3) of the
+    state and of the field must relabel the RHS.  The first component is pinned (1D2V / 2D2V oracles), so this carries its sign
+    and its field indexing over to the third."""
+    pair = dict(nelem=(2, 3, 2), order=(3, 2, 3), lo=(0.0, -1.0, 0.0), hi=(1.5, 2.0, 1.5))       # dims 0 and 2 alike
+    vel = dict(nelem=(2, 2, 2), order=(3, 4, 3), lo=(-2.0, -1.5, -2.0), hi=(2.0, 2.5, 2.0))      # dims 3 and 5 alike
+    g = on.make_grid(3, 3, pair["nelem"] + vel["nelem"], pair["order"] + vel["order"], pair["lo"] + vel["lo"], pair["hi"] + vel["hi"],
+                     bc=(0, 0, 0, 1, 0, 1), omega_c=0.0, pmax=(1, 1, 1))
+    f = rnd(g.flat_shape, 51)
+    E = [0.6 * rnd(g.flat_shape[:3], 52 + i) - 0.3 for i in range(3)]
+    swap6 = lambda a: np.ascontiguousarray(np.transpose(a, (2, 1, 0, 5, 4, 3)))
+    swap3 = lambda a: np.ascontiguousarray(np.transpose(a, (2, 1, 0)))
+    lhs = on.rhs(g, swap6(f), [swap3(E[2]), swap3(E[1]), swap3(E[0])])
+    assert relerr(lhs, swap6(on.rhs(g, f, E))) < 1e-13
+    # and the relabelled problem really exercises E_3: dropping it changes the answer at O(1)
+    assert relerr(on.rhs(g, f, [E[0], E[1], None]), on.rhs(g, f, E)) > 1e-2
+
+
+def test_3d3v_z_only_problem_reduces_to_the_1d1v_oracle():
+    """f = h(z, w) a(u) b(v), uniform in x and y, E = (0, 0, E_3(z)), no B: every term but the (z, w) pair vanishes (zero speed
+    in u and v, no gradient in x and y) and the 3D3V RHS is the pinned 1D1V RHS of h on (z, w), times a(u) b(v)."""
+    Nz, nz, Nw, nw = 4, 4, 5, 3
+    loz, hiz, low, hiw = 0.0, 4 * math.pi, -3.0, 3.5
+    g2 = ov.Grid(nelem=(Nz, Nw), order=(nz, nw), lo=(loz, low), hi=(hiz, hiw), bc=(0, 1), pmax=3)
+    g6 = on.make_grid(3, 3, (1, 2, Nz, 2, 1, Nw), (2, 2, nz, 3, 2, nw), (0.0, 0.0, loz, -1.0, -2.0, low), (1.0, 2.0, hiz, 1.0, 2.0, hiw),
+                      bc=(0, 0, 0, 1, 1, 1), omega_c=0.0, pmax=(1, 1, 3))
+    h = rnd(g2.flat_shape, 61)
+    E3 = 0.8 * rnd((g2.flat_shape[0],), 62) - 0.4
+    u, v = g6.coords[3].reshape(-1), g6.coords[4].reshape(-1)
+    au, bv = 1.0 + 0.2 * u, np.exp(-v * v)
+    lift = lambda a2: (a2[None, None, :, None, None, :] * au[None, None, None, :, None, None] * bv[None, None, None, None, :, None]
+                       * np.ones((g6.flat_shape[0], g6.flat_shape[1], 1, 1, 1, 1)))
+    E6 = [None, None, E3[None, None, :] * np.ones(g6.flat_shape[:2] + (1,))]
+    assert relerr(on.rhs(g6, lift(h), E6), lift(ov.rhs(g2, h, E3))) < 1e-13
+    # one self-consistent step: the field of the lifted state is along z only and is the 1D1V field scaled by the u, v quadratures
+    qu = float(np.sum(np.tile(g6.w[3] / g6.J[3], g6.nelem[3]) * au)); qv = float(np.sum(np.tile(g6.w[4] / g6.J[4], g6.nelem[4]) * bv))
+    En = on.field_E(g6, lift(h))
+    assert relerr(En[2], (qu * qv) * ov.field_E(g2, h)[None, None, :] * np.ones(g6.flat_shape[:2] + (1,))) < 1e-12
+    assert max(np.max(np.abs(En[0])), np.max(np.abs(En[1]))) < 1e-12 * np.max(np.abs(En[2]))
