@@ -1,4 +1,5 @@
-"""ctypes loader for libdgvlasov.so -- the C ABI declared in include/dgvlasov.h, include/dgvlasov2d2v.h and include/dgvlasov_nd.h.
+"""ctypes loader for libdgvlasov.so -- the C ABI declared in include/dgvlasov.h, include/dgvlasov2d2v.h, include/dgvlasov_nd.h and
+include/dgvlasov_noalloc.h.
 
 There is no fallback: if the library has not been built (python -m paper_2202_13532_b200.build)
 importing the binding raises."""
@@ -97,6 +98,8 @@ SIGNATURES = {
     "dg_last_field_kernel": (C.c_char_p, [_vp]),
     "dg_last_error": (C.c_char_p, []),
     "dg_version": (C.c_char_p, []),
+    # include/dgvlasov_noalloc.h
+    "dg_density_static": (C.c_int, [_vp, _i32, _i32, _i32, _vp, _vp, _vp, _i32, _vp]),
     # include/dgvlasov2d2v.h
     "dg4_create": (C.c_int, [C.POINTER(GridDesc4), C.POINTER(_vp)]),
     "dg4_destroy": (C.c_int, [_vp]),

@@ -64,6 +64,26 @@ def fp64_peak(device=0, variant=0, iters=20000) -> float:
     return tf.value
 
 
+STATIC_MAX_GX = 16384      # DG_STATIC_MAX_GX of include/dgvlasov_noalloc.h
+
+
+def density_static(f, wq_u, wq_v, out):
+    """dg_density_static: the density moment (Eq. 27) without a context or a workspace, for callers that must not
+    allocate device memory where they stand (a hook inside another code's time loop that owns all of the HBM, a
+    latency-critical callback that cannot afford the device-wide stall of cudaMalloc).  The partial sums go to a 2 MiB
+    array built into the library, shared by every call on the device: keep calls on one stream or order them with
+    events, and make the first call on each device at start-up (it looks up the array's address).
+    f: [G_x][G_u][G_v] or [G_x][G_v]; wq_u / wq_v: per-node quadrature weights [G_u] / [G_v] (wq_v None for 1D1V);
+    out: [G_x], required -- this wrapper allocates nothing either.  G_x <= STATIC_MAX_GX."""
+    if out is None:
+        raise DGError("density_static: pass the output tensor (nothing is allocated on this path)")
+    G_x, G_u = int(f.shape[0]), int(f.shape[1])
+    G_v = int(f.shape[2]) if f.dim() == 3 else 1
+    _check(_L.dg_density_static(_ptr(f), G_x, G_u, G_v, _ptr(wq_u), _ptr(wq_v), _ptr(out), f.device.index or 0,
+                                _stream(f.device)), "dg_density_static")
+    return out
+
+
 class DGContext:
     """dg_create / dg_destroy plus one method per C entry point."""
 

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdgvlasov.so")
-SOURCES = ["dg_api.cu", "dg_setup.cpp"]
+SOURCES = ["dg_api.cu", "dg_density_static.cu", "dg_setup.cpp"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC,-fopenmp,-O3", "-shared", "-lgomp",
@@ -23,8 +23,8 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "dgvlasov.h"), os.path.join(HERE, "..", "include", "dgvlasov2d2v.h"),
-                                                               os.path.abspath(__file__)]
+    inc = os.path.join(HERE, "..", "include")
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(inc, h) for h in os.listdir(inc)] + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

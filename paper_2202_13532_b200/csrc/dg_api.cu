@@ -19,6 +19,8 @@
 static thread_local std::string g_err;
 
 static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+// The same store for the library's other translation unit (dg_density_static.cu).
+int dg_internal_fail(int code, const char* msg) { return fail(code, msg ? msg : ""); }
 
 #define CUDA_TRY(expr)                                                                   \
   do {                                                                                   \
