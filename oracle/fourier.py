@@ -114,3 +114,14 @@ def broken_l2(lo: float, hi: float, nelem: int, n: int, u: np.ndarray, v=None, e
     half = 0.5 * (hi - lo) / nelem if edges is None else 0.5 * np.diff(np.asarray(edges, dtype=np.float64))
     q = np.einsum("...mi,ij,...mj->...m", d, M, d) * half
     return np.sqrt(np.maximum(q, 0.0)).sum(axis=-1) / nelem
+
+
+def field_energy(lo: float, hi: float, nelem: int, n: int, E: np.ndarray, edges=None) -> np.ndarray:
+    """Domain-integrated electric field energy of Fig. 10: W = (1/2) int E(x)^2 dx for nodal vectors
+    E [..., N*n], the integrand being each element's degree-(n-1) interpolant (Eq. 69), integrated exactly:
+    (1/2) sum_m E_m^T M E_m (dx)_m / 2 with the LGL mass matrix M of Eq. 50."""
+    e = np.asarray(E, dtype=np.float64)
+    e = e.reshape(e.shape[:-1] + (nelem, n))
+    M = mass_matrix(n)
+    half = 0.5 * (hi - lo) / nelem if edges is None else 0.5 * np.diff(np.asarray(edges, dtype=np.float64))
+    return 0.5 * (np.einsum("...mi,ij,...mj->...m", e, M, e) * half).sum(axis=-1)

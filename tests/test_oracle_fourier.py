@@ -179,3 +179,30 @@ def test_nonuniform_poisson_single_cosine_closed_form():
     E = fourier.poisson_E(edges[0], edges[-1], x, c)
     assert np.max(np.abs(E + (A / m) * np.sin(m * x + ph))) < 1e-10 * A / m
     assert abs(fourier.broken_l2(0, 0, N, n, np.ones(N * n), edges=edges) - np.sqrt(np.diff(edges)).sum() / N) < 1e-14
+
+
+@pytest.mark.parametrize("n,N", [(2, 5), (4, 3), (8, 4), (10, 2)])
+def test_field_energy_against_exact_polynomial_integrals(n, N):
+    """fourier.field_energy (Fig. 10; mass matrix of Eq. 50) against integrals that need no mass matrix: E = x on
+    [0, 1] gives 1/6 for every order; a random polynomial of degree n - 1 per element, integrated by numpy's polynomial
+    antiderivative of E^2, on equal and on unequal elements; E = P_{n-1} per element (closed form; a lumped quadrature
+    sum_j w_j E_j^2 fails it)."""
+    x01 = fourier.node_coordinates(0.0, 1.0, N, n)
+    assert abs(fourier.field_energy(0.0, 1.0, N, n, x01) - 1.0 / 6.0) < 1e-14
+    rng = np.random.default_rng(n * 100 + N)
+    for edges in (None, np.concatenate(([-1.0], -1.0 + np.cumsum(rng.uniform(0.3, 1.2, N))))):
+        lo, hi = (-1.0, 2.5) if edges is None else (edges[0], edges[-1])
+        ed = np.linspace(lo, hi, N + 1) if edges is None else edges
+        x = fourier.node_coordinates(lo, hi, N, n) if edges is None else fourier.node_coordinates_edges(edges, n)
+        E = np.empty(N * n); exact = 0.0
+        for m in range(N):
+            poly = np.polynomial.Polynomial(rng.uniform(-1, 1, n))
+            E[m * n:(m + 1) * n] = poly(x[m * n:(m + 1) * n])
+            F = (poly * poly).integ()
+            exact += 0.5 * (F(ed[m + 1]) - F(ed[m]))
+        assert abs(fourier.field_energy(lo, hi, N, n, E, edges=edges) - exact) < 1e-13 * abs(exact)
+        # E = P_{n-1}(xi) in every element: int P_{n-1}^2 dxi = 2/(2n-1), so W = L / (2 (2n-1)); the lumped LGL rule gives
+        # 2/(n-1) instead -- the term the exact mass matrix of Eq. 50 corrects
+        xi = basis.lgl_nodes_weights(n)[0]
+        Pn1 = np.tile(npleg.legval(xi, [0.0] * (n - 1) + [1.0]), N)
+        assert abs(fourier.field_energy(lo, hi, N, n, Pn1, edges=edges) - (hi - lo) / (2.0 * (2 * n - 1))) < 1e-13 * (hi - lo)
