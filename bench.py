@@ -143,7 +143,7 @@ def measured_peak_hbm():
 
 def ncu_traffic(workload, kernel, stage=None):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload` from the tracked ncu --set full
-    capture (profiles/ncu_traffic.csv, written from the .ncu-rep of the command named in profiles/ncu_traffic.md).  The
+    capture (profiles/ncu_traffic.csv; the commands of its captures are listed in profiles/r2_kernels.md).  The
     capture records the SHA-256 of the kernel's source file; if the source has changed since, the figure is stale and None
     is returned (with the reason)."""
     if not os.path.exists(TRAFFIC_CSV):
@@ -316,7 +316,7 @@ def run_ours(args, w, name):
         raise SystemExit("bench.py: no CUDA device; the DG kernels have no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    world, rank = du.init("nccl", dev)
+    world, rank = du.init("nccl", dev, log_nccl=True)
 
     def barrier():
         du.barrier(dev)
@@ -329,8 +329,6 @@ def run_ours(args, w, name):
         return run_xslab(args, w, name, world, rank, local, dev, barrier, max_over_ranks, parallelism)
     ga = grid_args(w)
     ctx = api.DGContext(device=local, **ga)
-    if args.smem_pad_kb:
-        ctx.set_option(api.OPT_SMEM_PAD_KB, args.smem_pad_kb)      # occupancy sweep of the tiled kernel (profiles/r2_kernels.md)
     f0 = make_f0(ctx.nodes(0), ctx.nodes(1), ctx.nodes(2), w)
     dof = f0.size
     dt = w["dt"]
@@ -410,11 +408,16 @@ def run_ours(args, w, name):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
+            # the 1000-step form of the config, flat and early in the line so that a truncated stored copy keeps it
+            **({} if sustained is None else {
+                "sustained_ms_per_step": sustained["ms_per_step"], "sustained_frac_whole_step": sustained["frac_whole_step"],
+                "sustained_stage_fracs": None if not sustained["rhs_stages"] else [s["frac"] for s in sustained["rhs_stages"]],
+                "sustained_sm_mhz": (sustained["clocks"] or {}).get("sm_mhz"),
+                "sustained_clock_reasons": (sustained["clocks"] or {}).get("reasons")}),
             "config": {"workload": name, "grid": "x".join(str(n * o) for n, o in zip(w["nelem"], w["order"])), "dof": dof,
                        "dt": dt, "self_consistent_poisson_each_stage": True, "mass_mode": 0,
                        "l2": "inputs (3 x %.2f GB) larger than L2; no flush needed" % (dof * 8 / 1e9),
-                       "parallelism": "replicas x%d" % world, "finite": finite,
-                       **({"smem_pad_kb": args.smem_pad_kb} if args.smem_pad_kb else {})},
+                       "parallelism": "replicas x%d" % world, "finite": finite},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "hbm_gbs_algorithmic_whole_step": 64.0 * dof * args.steps / (ms * 1e-3) / 1e9,
             "frac_whole_step": 64.0 * dof * args.steps / (ms * 1e-3) / 1e9 / peak,
@@ -850,8 +853,8 @@ def run_secondary(args):
         add(run_config4, a, name, host_inputs=False)
     a.steps, a.batch, a.field_kernel = 20, 4096, "auto"
     add(run_config5, a, "config5_field", host_inputs=False)
-    a.steps, a.batch, a.field_kernel = 2, 512, "dmma"
-    add(run_config5, a, "config5_field_dense_dmma_batch512", host_inputs=False)
+    a.steps, a.batch, a.field_kernel = 2, 4096, "dmma"            # the dense contraction at BASELINE config 5's stated batch
+    add(run_config5, a, "config5_field_dense_dmma", host_inputs=False)
     a.steps = 6
     add(run_config6, a, "config6_2d2v_128^4", host_inputs=False, with_e2e=False)
     add(run_config6, a, "config6_2d2v_n8_128^4", host_inputs=False, with_e2e=False)
@@ -921,8 +924,6 @@ def main():
     ap.add_argument("--no-secondary", action="store_true", help="skip the short runs of configs 2, 4, 5, 6")
     ap.add_argument("--secondary-budget-s", type=float, default=75.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--smem-pad-kb", type=int, default=0,
-                    help="configs 2, 3: unused extra shared memory per CTA of the tiled RHS kernel (DG_OPT_SMEM_PAD_KB), to cap the resident CTAs per SM")
     ap.add_argument("--full", action="store_true", help="oracle_timing: also the single-threaded 512^3 step")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:

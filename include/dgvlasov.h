@@ -147,6 +147,11 @@ int dg_poisson_phi(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* ph
  * being each element's nodal interpolant, integrated exactly with the LGL mass matrix of Eq. 50.
  *   u_dev, v_dev [in] [batch][N_x*n_x]; v_dev may be NULL (norm of u)     eps_dev [out] [batch] */
 int dg_broken_l2(dg_ctx* ctx, const double* u_dev, const double* v_dev, int32_t batch, double* eps_dev, void* stream);
+/* Domain-integrated electric field energy, the diagnostic of Fig. 10: W_b = (1/2) int E_b(x)^2 dx over the x
+ * grid, the integrand being each element's nodal interpolant, integrated exactly with the LGL mass matrix of Eq. 50
+ * -- not the lumped sum (1/2) sum w_j E_j^2, which is inexact at degree 2n-2.
+ *   E_dev [in] [batch][N_x*n_x]     W_dev [out] [batch]      any context (ndim = 1, 2, 3); deterministic */
+int dg_field_energy(dg_ctx* ctx, const double* E_dev, int32_t batch, double* W_dev, void* stream);
 size_t dg_field_workspace_bytes(const dg_ctx* ctx, int32_t batch);
 
 /* Introspection (host outputs; any pointer may be NULL to skip it). */
@@ -176,8 +181,6 @@ double dg_max_stable_dt(const dg_ctx* ctx, double E_bound);
 #define DG_OPT_FORM         5   /* 0 (default): weak form, Eq. 14: Upsilon F - Xi F*;  1: strong form, Eq. 15
                                   (PAPER.md:102): -D F + Xi (F - F*), D = Eq. 55.  Same scheme (Upsilon + D = Xi_R e_R^T -
                                   Xi_L e_L^T), different rounding; both RHS kernels, every entry point. */
-#define DG_OPT_SMEM_PAD_KB  6   /* unused extra shared memory (KB) per CTA of the tiled RHS kernel: lowers the number of resident
-                                  CTAs per SM.  For occupancy sweeps (profiles/): 0 (default) in production */
 int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value);
 /* Profile mode: total device time (ms) and count of the RHS-kernel launches since the last reset.
  * Synchronises on the recorded events. */

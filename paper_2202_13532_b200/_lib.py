@@ -98,6 +98,7 @@ SIGNATURES = {
     "dg_last_field_kernel": (C.c_char_p, [_vp]),
     "dg_last_error": (C.c_char_p, []),
     "dg_version": (C.c_char_p, []),
+    "dg_field_energy": (C.c_int, [_vp, _vp, _i32, _vp, _vp]),
     # include/dgvlasov_noalloc.h
     "dg_density_static": (C.c_int, [_vp, _i32, _i32, _i32, _vp, _vp, _vp, _i32, _vp]),
     # include/dgvlasov2d2v.h

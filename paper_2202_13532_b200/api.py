@@ -18,7 +18,6 @@ OPT_FIELD_KERNEL = 2
 OPT_PROFILE = 3
 OPT_PDL = 4
 OPT_FORM = 5
-OPT_SMEM_PAD_KB = 6
 FORM_WEAK, FORM_STRONG = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 FIELD_AUTO, FIELD_SIMPLE, FIELD_DMMA, FIELD_DFMA, FIELD_FFT = 0, 1, 2, 3, 4
@@ -217,6 +216,14 @@ class DGContext:
         batch = u2.shape[0]
         out = torch.empty(batch, dtype=torch.float64, device=self.device) if out is None else out
         _check(_L.dg_broken_l2(self._h, _ptr(u2), _ptr(v2), batch, _ptr(out), _stream(self.device)), "dg_broken_l2")
+        return out
+
+    def field_energy(self, E, out=None):
+        """dg_field_energy: W = (1/2) int E^2 dx per vector (Fig. 10), exact LGL mass matrix."""
+        E2 = E.reshape(-1, self.flat_shape[0])
+        batch = E2.shape[0]
+        out = torch.empty(batch, dtype=torch.float64, device=self.device) if out is None else out
+        _check(_L.dg_field_energy(self._h, _ptr(E2), batch, _ptr(out), _stream(self.device)), "dg_field_energy")
         return out
 
     # --- introspection ------------------------------------------------------------------------

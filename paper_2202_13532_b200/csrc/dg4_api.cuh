@@ -70,6 +70,7 @@ extern "C" int dg4_create(const dg4_grid_desc* desc, dg4_ctx** out) {
   }
   if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dg4_create: mass_mode must be 0 or 1");
   if (desc->pmax[0] < 0 || desc->pmax[1] < 0) return fail(DG_ERR_INVALID_ARG, "dg4_create: pmax must be >= 0");
+  if (int rc = check_device(desc->device, "dg4_create")) return rc;
   DeviceGuard guard(desc->device);      // the caller's current device is restored on return
   dg4_ctx* ctx = new (std::nothrow) dg4_ctx();
   if (!ctx) return fail(DG_ERR_CUDA, "dg4_create: out of host memory");
@@ -515,6 +516,10 @@ extern "C" int dg4_ssprk3_run(dg4_ctx* ctx, double* f_dev, double dt, int32_t ns
   DeviceGuard guard(ctx->desc.device);
   if (nsteps < 0 || !(dt == dt)) return fail(DG_ERR_INVALID_ARG, "dg4_ssprk3_run: bad nsteps or dt");
   if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg4_ssprk3_run: set a workspace first");
+  // An x-slab context reads its exterior x faces from the planes of dg4_set_xhalo, which belong to ONE stage input: a whole
+  // step in one call would feed stages 2 and 3 the faces of the step input.  Slabs step stage by stage (dg4_rk_stage).
+  if (ctx->desc.bc[0] == DG_BC_HALO)
+    return fail(DG_ERR_INVALID_ARG, "dg4_ssprk3_run: an x-slab context (bc[0] = DG_BC_HALO) steps stage by stage through dg4_rk_stage");
   if (self_consistent && (ctx->desc.bc[0] != 0 || ctx->desc.bc[1] != 0))
     return fail(DG_ERR_INVALID_ARG, "dg4_ssprk3_run: the self-consistent field needs periodic x and y");
   cudaStream_t st = (cudaStream_t)stream;

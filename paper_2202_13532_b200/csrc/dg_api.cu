@@ -38,6 +38,15 @@ static int check_launch(dg_ctx* ctx, const char* what) {
   return DG_OK;
 }
 
+// A device ordinal the process cannot see is an argument error at creation, not a silent run on the current device
+// (DeviceGuard does not report a failed switch).  Shared by dg_create, dg4_create, dgn_create and dg_fp64_peak.
+static int check_device(int device, const char* who) {
+  int ndev = 0;
+  CUDA_TRY(cudaGetDeviceCount(&ndev));
+  if (device < 0 || device >= ndev) return fail(DG_ERR_INVALID_ARG, std::string(who) + ": no such device");
+  return DG_OK;
+}
+
 extern "C" const char* dg_last_error(void) { return g_err.c_str(); }
 extern "C" const char* dg_version(void) { return "dgvlasov-b200 0.1 (sm_100a)"; }
 
@@ -74,11 +83,7 @@ static int create_impl(const dg_grid_desc* desc, const double* edges, dg_ctx** o
   }
   if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dg_create: mass_mode must be 0 or 1");
   if (desc->pmax < 0) return fail(DG_ERR_INVALID_ARG, "dg_create: pmax must be >= 0");
-  {
-    int ndev = 0;
-    CUDA_TRY(cudaGetDeviceCount(&ndev));
-    if (desc->device < 0 || desc->device >= ndev) return fail(DG_ERR_INVALID_ARG, "dg_create: no such device");
-  }
+  if (int rc = check_device(desc->device, "dg_create")) return rc;
   DeviceGuard guard(desc->device);      // the caller's current device is restored on return
 
   dg_ctx* ctx = new (std::nothrow) dg_ctx();
@@ -143,11 +148,10 @@ static int create_impl(const dg_grid_desc* desc, const double* edges, dg_ctx** o
   const size_t o_hdx = off; off = align_up(off + sizeof(double) * (edges ? ctx->N[0] : 0), 256);
   const size_t o_AD = off; off = align_up(off + sizeof(double) * AD.size(), 256);
   const size_t o_W = off; off = align_up(off + sizeof(double) * W.size(), 256);
-  size_t o_cpart = 0, o_sync = 0;
+  size_t o_cpart = 0;
   if (desc->ndim >= 2 && dgf::field_fused_supported(ctx->G[0], 2 * ctx->P1)) {
     dgf::field_fused_shape(ctx->G[0], &ctx->fused_rows, &ctx->fused_grid);
     o_cpart = off; off = align_up(off + sizeof(double) * (size_t)ctx->fused_grid * 2 * ctx->P1, 256);
-    o_sync = off;  off = align_up(off + 2 * sizeof(unsigned int), 256);
   }
   cudaError_t e = cudaMalloc(&ctx->dev_block, off);
   if (e != cudaSuccess) { delete ctx; return fail(DG_ERR_CUDA, std::string("dg_create: cudaMalloc: ") + cudaGetErrorString(e)); }
@@ -206,8 +210,6 @@ static int create_impl(const dg_grid_desc* desc, const double* edges, dg_ctx** o
   }
   if (ctx->fused_grid > 0) {
     ctx->d_cpart = (double*)(base + o_cpart);
-    ctx->d_sync = (unsigned int*)(base + o_sync);
-    ok = ok && cudaMemset(ctx->d_sync, 0, 2 * sizeof(unsigned int)) == cudaSuccess;
   }
   if (!ok) {
     cudaFree(ctx->dev_block);
@@ -223,7 +225,6 @@ extern "C" int dg_destroy(dg_ctx* ctx) {
   if (!ctx) return DG_OK;
   DeviceGuard guard(ctx->desc.device);
   if (ctx->dev_block) cudaFree(ctx->dev_block);
-  if (ctx->d_flag) cudaFree(ctx->d_flag);
   if (ctx->dense_block) cudaFree(ctx->dense_block);
   if (ctx->f_stage) cudaFree(ctx->f_stage);
   for (const ProfRecord& r : ctx->prof_events) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
@@ -577,6 +578,18 @@ extern "C" int dg_broken_l2(dg_ctx* ctx, const double* u_dev, const double* v_de
   return check_launch(ctx, "broken_l2_kernel");
 }
 
+extern "C" int dg_field_energy(dg_ctx* ctx, const double* E_dev, int32_t batch, double* W_dev, void* stream) {
+  if (!ctx || !E_dev || !W_dev) return fail(DG_ERR_INVALID_ARG, "dg_field_energy: null argument");
+  DeviceGuard guard(ctx->desc.device);
+  if (batch < 1) return fail(DG_ERR_INVALID_ARG, "dg_field_energy: batch must be >= 1");
+  const int n0 = ctx->n[0];
+  const double alpha = n0 * (n0 - 1) / (2.0 * (2 * n0 - 1));
+  const double half_dx = 0.5 * (ctx->desc.hi[0] - ctx->desc.lo[0]) / ctx->N[0];
+  dgk::field_energy_kernel<<<(unsigned)batch, 256, 0, (cudaStream_t)stream>>>(E_dev, ctx->d_wg, ctx->d_half_dx, ctx->N[0], n0, alpha,
+                                                                            half_dx, W_dev);
+  return check_launch(ctx, "field_energy_kernel");
+}
+
 extern "C" int dg_poisson_E(dg_ctx* ctx, const double* rho_dev, int32_t batch, double* E_dev, void* stream) {
   return poisson_solve(ctx, rho_dev, batch, E_dev, 0, stream);
 }
@@ -597,7 +610,7 @@ static int field_from_partials_or_f(dg_ctx* ctx, const double* f, int partial_ch
     }
     dgf::FieldFusedParams P;
     P.partials = ctx->partials; P.T = ctx->d_T; P.S = ctx->d_S; P.rho = ctx->rho; P.cpart = ctx->d_cpart;
-    P.c = ctx->cbuf; P.E = ctx->E; P.sync = ctx->d_sync;
+    P.c = ctx->cbuf; P.E = ctx->E;
     P.nchunks = partial_chunks; P.G0 = ctx->G[0]; P.Q = 2 * ctx->P1; P.rows = ctx->fused_rows;
     rc = dgf::launch_field_fused(P, ctx->fused_grid, pdl, st);
     if (rc != DG_OK) return fail(rc, std::string("field_fused_kernel launch failed: ") + cudaGetErrorString(cudaGetLastError()));
@@ -626,6 +639,10 @@ extern "C" int dg_ssprk3_run(dg_ctx* ctx, double* f_dev, double dt, int32_t nste
   if (ctx->ndim < 2) return fail(DG_ERR_UNSUPPORTED, "dg_ssprk3: field-only context (ndim = 1)");
   if (nsteps < 0 || !(dt == dt)) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: bad nsteps or dt");
   if (!ctx->ws) return fail(DG_ERR_WORKSPACE, "dg_ssprk3: set a workspace first");
+  // x-slab contexts: the planes of dg_set_xhalo belong to one stage input, so a whole step in one call would give stages 2
+  // and 3 the faces of the step input.  Slabs step stage by stage (dg_rk_stage; sharded.py does).
+  if (ctx->desc.bc[0] == DG_BC_HALO)
+    return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: an x-slab context (bc[0] = DG_BC_HALO) steps stage by stage through dg_rk_stage");
   if (self_consistent && ctx->desc.bc[0] != 0) return fail(DG_ERR_INVALID_ARG, "dg_ssprk3: self-consistent E needs periodic x");
   cudaStream_t st = (cudaStream_t)stream;
   int chunks = 0;          // > 0: ctx->partials holds density partials of the current stage input
@@ -760,7 +777,6 @@ extern "C" int dg_get_profile_stages(dg_ctx* ctx, double* ms_host, int64_t* laun
 extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return fail(DG_ERR_INVALID_ARG, "dg_set_option: null context");
   if (key == DG_OPT_PROFILE && value >= 0 && value <= 1000000) { ctx->opt_profile = (int)value; ctx->prof_seen = 0; return DG_OK; }
-  if (key == DG_OPT_SMEM_PAD_KB && value >= 0 && value <= 180) { ctx->opt_smem_pad_kb = (int)value; return DG_OK; }
   if (key == DG_OPT_RHS_KERNEL && value >= 0 && value <= 2) { ctx->opt_rhs_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_FIELD_KERNEL && value >= 0 && value <= 4) { ctx->opt_field_kernel = (int)value; return DG_OK; }
   if (key == DG_OPT_PDL && (value == 0 || value == 1)) { ctx->opt_pdl = (int)value; return DG_OK; }
@@ -770,6 +786,7 @@ extern "C" int dg_set_option(dg_ctx* ctx, int32_t key, int64_t value) {
 
 extern "C" int dg_fp64_peak(int32_t device, int32_t variant, int32_t iters, double* tflops_host) {
   if (!tflops_host || iters < 1 || (variant != 0 && variant != 1)) return fail(DG_ERR_INVALID_ARG, "dg_fp64_peak: bad argument");
+  if (int rc = check_device(device, "dg_fp64_peak")) return rc;
   DeviceGuard guard(device);
   int sms = 0;
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));

@@ -87,9 +87,8 @@ struct dg_ctx {
   std::vector<double> edges;  // element edges of a non-uniform x-only context (dg_create_field_nonuniform), else empty
   double* d_half_dx = nullptr;  // [N0] half widths of such a context
   double* d_wg = nullptr;     // [2][n0]: w_j and w_j P_{n-1}(xi_j) of the x basis (broken l2 norm, Eq. 50 / 72)
-  // one-launch field solve (field_fused_kernel): per-CTA shares of c_q and the rendezvous words
+  // one-launch field solve (field_fused_kernel): per-CTA shares of c_q
   double* d_cpart = nullptr;  // [2*P1][fused_grid]
-  unsigned int* d_sync = nullptr;
   int fused_rows = 0, fused_grid = 0;
 
   // caller-provided workspace
@@ -108,7 +107,6 @@ struct dg_ctx {
   int64_t launches = 0;
   int opt_rhs_kernel = 0, opt_field_kernel = 0, opt_profile = 0, opt_pdl = 1;
   int opt_form = 0;           // 0 weak form (Eq. 14), 1 strong form (Eq. 15)
-  int opt_smem_pad_kb = 0;    // DG_OPT_SMEM_PAD_KB: extra dynamic shared memory per CTA of the tiled kernel (occupancy sweeps)
   // profile mode: (start, stop) event pairs around RHS launches, tagged with the RK stage (0 = not inside dg_ssprk3_*)
   std::vector<ProfRecord> prof_events;
   int64_t prof_seen = 0;      // RHS launches since profile mode was set (every opt_profile-th one is bracketed)
@@ -116,7 +114,6 @@ struct dg_ctx {
   double prof_ms[4] = {0, 0, 0, 0};
   int64_t prof_n[4] = {0, 0, 0, 0};
   std::map<TmapKey, CUtensorMap> tmaps;   // TMA descriptors of the arrays seen so far (f, u1, u2, halos: a handful)
-  int* d_flag = nullptr;      // library-owned word for dg_ssprk3_run_host's finiteness report
   std::string last_kernel = "none";
   std::string last_field_kernel = "none";
   double cfl_limit = -1.0;    // lazily computed

@@ -5,6 +5,7 @@
 // next k-tile.  FP64-pipe bound.
 #pragma once
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 #include <cstdint>
 
 #include "../../include/dgvlasov.h"
@@ -227,9 +228,9 @@ inline int launch_gemm_tn(const double* A, const double* B, double* C, int M, in
 //   E[gx]   = sum_q S[gx][q] c_q                      (Eq. 71; Poisson factor folded into S)
 // CTA b owns the x nodes [b*rows, (b+1)*rows): it finishes their densities, forms its share of every
 // c_q, and after a grid-wide rendezvous sums all shares in CTA order (deterministic) and synthesises
-// E at its own nodes.  The grid never exceeds the SM count and each CTA needs few resources, so all
-// CTAs are co-resident and the sense-reversing rendezvous (count, generation) cannot deadlock; it
-// resets itself, so the launch may be replayed.
+// E at its own nodes.  The grid never exceeds the SM count and each CTA needs few resources; the launch
+// is cooperative, so the driver checks that all CTAs are co-resident and the rendezvous is the grid
+// barrier of cooperative groups.
 // ------------------------------------------------------------------------------------------------
 struct FieldFusedParams {
   const double* partials;   // [G0][nchunks]
@@ -239,15 +240,8 @@ struct FieldFusedParams {
   double* cpart;            // [Q][grid] scratch (q-major)
   double* c;                // [Q]
   double* E;                // [G0]
-  unsigned int* sync;       // {count, generation}
   int nchunks, G0, Q, rows;
 };
-
-__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
-  unsigned int v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
 
 __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams P) {
   extern __shared__ double fsm[];
@@ -299,25 +293,9 @@ __global__ void __launch_bounds__(256) field_fused_kernel(const FieldFusedParams
     for (int i = 0; i < nrows; ++i) acc = fma(tr[i], rho_s[i], acc);
     P.cpart[(size_t)q * gridDim.x + blockIdx.x] = acc;
   }
-  // C: grid-wide rendezvous
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) {
-    const unsigned int gen = ld_acquire_u32(P.sync + 1);
-    const unsigned int old = atomicAdd(P.sync, 1u);
-    if (old == gridDim.x - 1) {
-      P.sync[0] = 0u;
-      __threadfence();
-      atomicAdd(P.sync + 1, 1u);
-    } else {
-      const long long t0 = clock64();
-      while (ld_acquire_u32(P.sync + 1) == gen) {
-        if (clock64() - t0 > (1LL << 32)) __trap();      // ~2 s: a lost CTA must not hang the device
-      }
-    }
-    __threadfence();
-  }
-  __syncthreads();
+  // C: grid-wide rendezvous.  The launch is cooperative (launch_field_fused), so the grid barrier of cooperative groups
+  // applies: it orders the cpart stores above before the loads of phase D in every CTA.
+  cooperative_groups::this_grid().sync();
   // D: c_q = sum of the shares.  One warp per q (q = warp, warp + 8, ...), lanes along the CTA index (grid <= 128: at
   // most four loads per lane, added in order), then a fixed butterfly: the same association in every CTA and every
   // run.  Eight q per pass: 32 loads in flight per lane.

@@ -266,4 +266,30 @@ __global__ void __launch_bounds__(256) broken_l2_kernel(const double* __restrict
   if (threadIdx.x == 0) eps[blockIdx.x] = red[0] / (double)N;
 }
 
+// Domain-integrated field energy (Fig. 10): W = (1/2) int E^2 dx, each element's interpolant integrated exactly
+// by the mass matrix of Eq. 50 in the same rank-one form as above.  One CTA per vector, fixed order: deterministic.
+__global__ void __launch_bounds__(256) field_energy_kernel(const double* __restrict__ E, const double* __restrict__ wg,
+                                                           const double* __restrict__ half_dx_m, int N, int n, double alpha,
+                                                           double half_dx, double* __restrict__ W) {
+  __shared__ double red[256];
+  const size_t off = (size_t)blockIdx.x * N * n;
+  double acc = 0.0;
+  for (int m = threadIdx.x; m < N; m += 256) {
+    double s2 = 0.0, sp = 0.0;
+    for (int j = 0; j < n; ++j) {
+      const double e = E[off + (size_t)m * n + j];
+      s2 = fma(wg[j] * e, e, s2);
+      sp = fma(wg[n + j], e, sp);
+    }
+    acc = fma(fma(-alpha * sp, sp, s2), half_dx_m ? half_dx_m[m] : half_dx, acc);
+  }
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) W[blockIdx.x] = 0.5 * red[0];
+}
+
 }  // namespace dgk

@@ -260,7 +260,12 @@ __global__ void __launch_bounds__(NN * NN * KV / 2, tiled_min_ctas(NN)) rhs_tile
   // all; the barrier also makes the mbarrier initialisation visible to the waiters.
   int* sAny = reinterpret_cast<int*>(smem + Cfg::OFF_BAR + 64);      // one word per warp
   {
-    const int w_or = __reduce_or_sync(__activemask(), um);      // NT need not be a multiple of 32
+    // The member mask comes from the compile-time thread count, never from __activemask(): the warp of thread 0 has
+    // just left a divergent block and need not have reconverged.  NT need not be a multiple of 32: the last warp is ragged.
+    constexpr unsigned kTail = (Cfg::NT & 31) ? ((1u << (Cfg::NT & 31)) - 1u) : 0xffffffffu;
+    const unsigned wmask = ((t >> 5) == (Cfg::NT >> 5)) ? kTail : 0xffffffffu;
+    __syncwarp(wmask);
+    const int w_or = __reduce_or_sync(wmask, um);
     if ((t & 31) == 0) sAny[t >> 5] = w_or;
   }
   __syncthreads();
@@ -562,8 +567,12 @@ int launch_rhs_tiled_t(dg_ctx* ctx, const double* f, const double* fn, const dou
   P.want_partials = (want_partials && ctx->partials && chunks * ctx->G[0] <= ctx->partials_doubles) ? 1 : 0;
   if (partial_chunks) *partial_chunks = P.want_partials ? (int)chunks : 0;
 
-  // DG_OPT_SMEM_PAD_KB: unused extra shared memory per CTA, to lower the number of resident CTAs (occupancy sweeps)
-  const size_t smem_bytes = (size_t)Cfg::SMEM_BYTES + (size_t)ctx->opt_smem_pad_kb * 1024;
+  // DG_TILED_SMEM_PAD_KB (build-time, default 0): unused extra shared memory per CTA, to lower the number of resident CTAs
+  // in occupancy sweeps.  Not part of the ABI.
+#ifndef DG_TILED_SMEM_PAD_KB
+#define DG_TILED_SMEM_PAD_KB 0
+#endif
+  const size_t smem_bytes = (size_t)Cfg::SMEM_BYTES + (size_t)DG_TILED_SMEM_PAD_KB * 1024;
   {
     cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(rhs_tiled_kernel<NN, KV, STRONG>), smem_bytes);
     if (e != cudaSuccess) { g_tiled_err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return DG_ERR_CUDA; }

@@ -56,6 +56,7 @@ extern "C" int dgn_create(const dgn_grid_desc* desc, dgn_ctx** out) {
   }
   if (desc->mass_mode != 0 && desc->mass_mode != 1) return fail(DG_ERR_INVALID_ARG, "dgn_create: mass_mode must be 0 or 1");
   for (int i = 0; i < desc->dx; ++i) if (desc->pmax[i] < 0) return fail(DG_ERR_INVALID_ARG, "dgn_create: pmax must be >= 0");
+  if (int rc = check_device(desc->device, "dgn_create")) return rc;
   DeviceGuard guard(desc->device);
   dgn_ctx* ctx = new (std::nothrow) dgn_ctx();
   if (!ctx) return fail(DG_ERR_CUDA, "dgn_create: out of host memory");

@@ -14,18 +14,20 @@ def env_world():
     return (int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")))
 
 
-def init(backend: str, device=None):
+def init(backend: str, device=None, log_nccl: bool = False):
+    """log_nccl (bench.py passes it; off for every other caller): send NCCL's communicator lines to a per-process file and
+    have rank 0 echo its "Init COMPLETE" line to stderr after the first collective, so that a reader of the bench log can
+    see the N ranks.  Without it the caller's environment is left alone and no file is written."""
     world, rank, _ = env_world()
     if world > 1 and not dist.is_initialized():
         kw = {}
         log = None
         if backend == "nccl" and device is not None:
             kw["device_id"] = device
-            # NCCL's communicator lines go to a per-process file (stdout carries the one JSON line); rank 0 echoes its
-            # "Init COMPLETE" line to stderr after the first collective so that a reader can see the N ranks
-            os.environ.setdefault("NCCL_DEBUG", "INFO")
-            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
-            log = os.environ.setdefault("NCCL_DEBUG_FILE", "/tmp/dg_nccl_%h_%p.log")
+            if log_nccl:
+                os.environ.setdefault("NCCL_DEBUG", "INFO")
+                os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+                log = os.environ.setdefault("NCCL_DEBUG_FILE", "/tmp/dg_nccl_%h_%p.log")
         dist.init_process_group(backend, **kw)
         if log is not None:
             dist.barrier()
@@ -38,7 +40,8 @@ def _echo_nccl_init(pattern: str, rank: int):
     import sys
     path = pattern.replace("%h", socket.gethostname()).replace("%p", str(os.getpid()))
     try:
-        lines = [l.rstrip() for l in open(path) if "Init COMPLETE" in l or "nranks" in l]
+        with open(path) as fh:
+            lines = [l.rstrip() for l in fh if "Init COMPLETE" in l or "nranks" in l]
     except OSError:
         return
     if rank == 0:

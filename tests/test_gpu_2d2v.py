@@ -495,4 +495,7 @@ def test_xslab_halo_argument_checks():
     f = torch.zeros(slab.flat_shape, dtype=torch.float64, device="cuda")
     with pytest.raises(A.DGError):
         slab.ssprk3_run(f, 1e-3, 1, True)                                                  # the Poisson solve is global
+    slab.set_xhalo(torch.zeros((2,) + tuple(f.shape[1:]), dtype=torch.float64, device="cuda"))
+    with pytest.raises(A.DGError, match="stage by stage"):
+        slab.ssprk3_run(f, 1e-3, 1, False)          # one halo buffer cannot serve three stage inputs: dg4_rk_stage only
     slab.close()

@@ -123,6 +123,23 @@ def test_fft_config5_grid_closed_form_and_sampled_oracle():
 
 
 @pytest.mark.parametrize("N,n,batch", [(10, 3, 1), (25, 8, 4), (64, 8, 40), (300, 5, 7), (2048, 8, 3)])
+def test_field_energy_matches_oracle(N, n, batch):
+    """dg_field_energy (Fig. 10; mass matrix of Eq. 50) against the oracle; the P_{n-1} closed form
+    L / (2 (2n - 1)) that a lumped quadrature gets wrong; deterministic."""
+    A = api()
+    lo, hi = -0.5, 2.0
+    ctx = A.DGContext((N,), (n,), (lo,), (hi,), pmax=4, workspace=False)
+    E = wl.uniform_field((batch, N * n), 41) - 0.5
+    W = ctx.field_energy(dev(E)).cpu().numpy()
+    assert relerr(W, ofr.field_energy(lo, hi, N, n, E)) <= 1e-13
+    assert np.array_equal(W, ctx.field_energy(dev(E)).cpu().numpy())
+    xi = ctx.operators(0)[0]
+    Pn1 = np.tile(np.polynomial.legendre.legval(xi, [0.0] * (n - 1) + [1.0]), N)
+    assert abs(float(ctx.field_energy(dev(Pn1))[0]) - (hi - lo) / (2.0 * (2 * n - 1))) < 1e-13 * (hi - lo)
+    ctx.close()
+
+
+@pytest.mark.parametrize("N,n,batch", [(10, 3, 1), (25, 8, 4), (64, 8, 40), (300, 5, 7), (2048, 8, 3)])
 def test_broken_l2_matches_oracle(N, n, batch):
     """dg_broken_l2 (Eq. 72 with the LGL mass matrix of Eq. 50) against the oracle, with and without v."""
     A = api()
@@ -187,6 +204,7 @@ def test_nonuniform_element_widths_match_oracle(n, N, pmax, batch, kernel):
     assert np.max(np.abs(ctx.poisson_phi(dev(rho)).cpu().numpy() - Phio)) <= 1e-12 * np.max(np.abs(Phio)) + 1e-14 * np.max(np.abs(rho))
     u, v = wl.uniform_field((batch, N * n), 5), wl.uniform_field((batch, N * n), 6)
     assert relerr(ctx.broken_l2(dev(u), dev(v)).cpu().numpy(), ofr.broken_l2(0, 0, N, n, u, v, edges=edges)) <= 1e-13
+    assert relerr(ctx.field_energy(dev(u)).cpu().numpy(), ofr.field_energy(0, 0, N, n, u, edges=edges)) <= 1e-13
     ctx.set_option(A.OPT_FIELD_KERNEL, A.FIELD_FFT)
     with pytest.raises(A.DGError):
         ctx.poisson_E(dev(rho))

@@ -113,17 +113,6 @@ def test_profile_stage_samples():
     ctx.close()
 
 
-def test_smem_pad_option_changes_nothing_but_occupancy():
-    A = api()
-    ctx = A.DGContext((2, 2, 8), (8, 8, 8), LO, HI, bc=(0, 1, 1), omega_c=1.0)
-    f = torch.rand(ctx.flat_shape, dtype=torch.float64, device="cuda")
-    a = ctx.rhs(f)
-    ctx.set_option(A.OPT_SMEM_PAD_KB, 20)
-    b = ctx.rhs(f)
-    assert torch.equal(a, b)
-    ctx.close()
-
-
 def test_create_restores_the_callers_device_and_two_contexts_coexist():
     A = api()
     cur = torch.cuda.current_device()

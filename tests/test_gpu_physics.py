@@ -29,8 +29,7 @@ def _run(k_larmor, omega, t_end, t_diag, nelem, amp=2e-4, sense=-1):
     wx = np.tile(ctx.operators(0)[1] * 0.5 * L / nelem[0], nelem[0])          # LGL quadrature weights in x
 
     def energy():
-        E = ctx.poisson_E(ctx.density(f)).cpu().numpy()
-        return 0.5 * float(np.sum(wx * E * E))
+        return float(ctx.field_energy(ctx.poisson_E(ctx.density(f)))[0])      # dg_field_energy: Fig. 10's diagnostic on the device
 
     mass0 = float(np.sum(wx * ctx.density(f).cpu().numpy()))
     steps = max(1, math.ceil(t_diag / (0.9 * ctx.max_stable_dt(0.3))))
