@@ -160,6 +160,9 @@ def ncu_traffic(workload, kernel, stage=None):
         if any(r["source_sha16"] != sha for r in rows):
             return None, "stale: %s changed since the capture" % src
     per_launch = [float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]) for r in rows]
+    per_launch = [v for v in per_launch if v == v]            # a launch whose DRAM counters ncu could not collect
+    if not per_launch:
+        return None, "capture holds no DRAM byte counts for this kernel"
     return sum(per_launch) / len(per_launch), "profiles/ncu_traffic.csv (%s)" % rows[0]["capture"]
 
 

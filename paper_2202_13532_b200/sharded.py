@@ -122,6 +122,60 @@ class TorchDistComm:
         return out
 
 
+class HostStagedComm(TorchDistComm):
+    """The same two collectives with every message staged through host memory, over a CPU process group (gloo).
+    For ranks that cannot talk NCCL to each other -- above all several ranks sharing ONE GPU (NCCL refuses duplicate
+    devices), which is how the sharded step is exercised as concurrent processes on a single-GPU box.  Each transfer
+    synchronises the rank's stream (the .cpu() copies), so no kernel ever waits for another process's kernel; the ranks
+    meet in gloo on the host.  Plain exchange only: the fused face push needs peer-mapped halo buffers."""
+
+    def exchange_faces(self, first_plane, last_plane, halo, periodic: bool):
+        if self.world == 1:
+            return super().exchange_faces(first_plane, last_plane, halo, periodic)
+        r, w = self.rank, self.world
+        left, right = (r - 1) % w, (r + 1) % w
+        has_left, has_right = periodic or r > 0, periodic or r < w - 1
+        first_h, last_h = first_plane.cpu().contiguous(), last_plane.cpu().contiguous()
+        in_l, in_r = torch.empty_like(first_h), torch.empty_like(first_h)
+        ops = []
+        if has_right:
+            ops.append(dist.P2POp(dist.isend, last_h, right, self.group, 0))
+        if has_left:
+            ops.append(dist.P2POp(dist.isend, first_h, left, self.group, 1))
+        if has_left:
+            ops.append(dist.P2POp(dist.irecv, in_l, left, self.group, 0))
+        if has_right:
+            ops.append(dist.P2POp(dist.irecv, in_r, right, self.group, 1))
+        for work in dist.batch_isend_irecv(ops):
+            work.wait()
+        halo[0].copy_(in_l) if has_left else halo[0].zero_()
+        halo[1].copy_(in_r) if has_right else halo[1].zero_()
+
+    def alloc_halos(self, plane_shape, device, periodic: bool):
+        if self.world == 1:
+            return super().alloc_halos(plane_shape, device, periodic)
+        raise RuntimeError("HostStagedComm: the fused face push needs peer-mapped halo buffers (use TorchDistComm over NCCL)")
+
+    def device_barrier(self, token):
+        if self.world > 1:
+            torch.cuda.synchronize(token.device) if token.is_cuda else None
+            dist.barrier(group=self.group)
+
+    def all_gather_rho(self, rho_loc, counts, out):
+        if self.world == 1:
+            return super().all_gather_rho(rho_loc, counts, out)
+        m = max(counts)
+        send = torch.zeros(m, dtype=rho_loc.dtype)
+        send[:rho_loc.numel()].copy_(rho_loc)                       # device -> host (synchronises the stream)
+        buf = torch.empty(self.world * m, dtype=rho_loc.dtype)
+        dist.all_gather_into_tensor(buf, send, group=self.group)
+        off = 0
+        for r, c in enumerate(counts):
+            out[off:off + c].copy_(buf[r * m:r * m + c])
+            off += c
+        return out
+
+
 class CudaBackend:
     """The arithmetic of one slab, through the C ABI: a slab context (bc[0] = DG_BC_HALO) for density and the fused
     RHS + stage kernel, and an x-only context over the GLOBAL grid for the Poisson solve."""

@@ -107,9 +107,11 @@ if __name__ == "__main__":
     from paper_2202_13532_b200 import dist_util as du
     world, rank = du.init("gloo")
     out = {}
+    staged = len(sys.argv) > 1 and sys.argv[1] == "hoststaged"      # the host-staged transport (sharded.HostStagedComm)
     for sc in (True, False):
         for bc0 in ((0, 1) if not sc else (0,)):
-            err, part = run_sharded(rank, world, self_consistent=sc, bc0=bc0)
+            err, part = run_sharded(rank, world, comm=sharded.HostStagedComm(rank, world) if staged else None,
+                                    self_consistent=sc, bc0=bc0)
             err = du.max_over_ranks(err)
             out[f"err_sc{int(sc)}_bc{bc0}"] = err
     du.barrier()

@@ -5,6 +5,8 @@ import socket
 import subprocess
 import sys
 
+import pytest
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
@@ -75,10 +77,12 @@ def test_xslab_world1_wraps_through_the_halo_planes():
     assert err <= 1e-13
 
 
-def test_xslab_two_rank_gloo_matches_unsharded_oracle():
-    """world = 2 over gloo, uneven slabs (2 + 3 x-elements): face-plane exchange + all-gather of rho."""
+@pytest.mark.parametrize("transport", ["direct", "hoststaged"])
+def test_xslab_two_rank_gloo_matches_unsharded_oracle(transport):
+    """world = 2 over gloo, uneven slabs (2 + 3 x-elements): face-plane exchange + all-gather of rho; through TorchDistComm
+    and through HostStagedComm (the transport of the two-processes-on-one-GPU test)."""
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
-           "--master-port", str(_free_port()), os.path.join(ROOT, "tests", "_xslab_worker.py")]
+           "--master-port", str(_free_port()), os.path.join(ROOT, "tests", "_xslab_worker.py"), transport]
     res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert res.returncode == 0, res.stderr[-3000:]
     out = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])

@@ -233,3 +233,29 @@ def test_two_gpu_xslab_matches_unsharded_oracle(mode):
     for k, v in out.items():
         if k.startswith("err_"):
             assert v <= 1e-11, (k, v)
+
+
+def test_two_processes_one_gpu_xslab_host_staged():
+    """Two RANKS AS TWO PROCESSES sharing cuda:0 (torchrun, gloo, sharded.HostStagedComm: faces and densities travel through
+    host memory), uneven slabs (2 + 3 x-elements), XSlabStepper + CudaBackend: three self-consistent steps with the global
+    Poisson solve and three without (periodic and zero-inflow x), against the UNSHARDED oracle.  The cross-process ordering
+    of the sharded step through the library's kernels on the one GPU there is; the NCCL / peer-memory transports stay
+    unmeasured across devices."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(root, "tests", "_xslab_gpu_worker.py"), "hoststaged"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=root)
+    assert res.returncode == 0, res.stderr[-3000:]
+    out = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])
+    assert out["world"] == 2 and out["staged"] and len(set(out["pids"])) == 2
+    assert out["slab_sc1_bc0"] == [0, 2]                       # rank 0 of the uneven 2 + 3 split
+    errs = {k: v for k, v in out.items() if k.startswith("err_")}
+    assert set(errs) == {"err_sc1_bc0", "err_sc0_bc0", "err_sc0_bc1"}
+    for k, v in errs.items():
+        assert v <= 1e-11, (k, v)
